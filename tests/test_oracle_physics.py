@@ -1,0 +1,265 @@
+"""Pins for the oracle's H apply, Chebyshev filter, Hartree solve and split-operator step (CPU only).
+
+The pins are the ones SURVEY.md section 8(c) lists: closed forms (plane waves, constant V, erf
+potential of a Gaussian charge), invariants (Hermiticity, unitarity, reversibility, order 2) and
+brute force (a dense H built here with numpy, independent of the oracle, diagonalised with eigh).
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy.linalg import expm
+from scipy.special import erf
+
+from paper_2601_21005_b200 import workloads as W
+
+
+def kgrid(g):
+    def k1(n, h):
+        return 2 * np.pi * np.fft.fftfreq(n, d=h)       # library's ordering: m in [-n/2, n/2)
+    kz, ky, kx = np.meshgrid(k1(g.nz, g.hz), k1(g.ny, g.hy), k1(g.nx, g.hx), indexing="ij")
+    return kx, ky, kz
+
+
+def dense_H(g, vloc, kb):
+    """H as a dense matrix, built with numpy.fft and outer products (independent of the oracle)."""
+    ng = g.ng
+    kx, ky, kz = kgrid(g)
+    k2 = 0.5 * (kx ** 2 + ky ** 2 + kz ** 2)
+    eye = np.eye(ng, dtype=np.complex128).reshape((ng,) + g.shape)
+    T = np.fft.ifftn(k2[None] * np.fft.fftn(eye, axes=(1, 2, 3)), axes=(1, 2, 3)).reshape(ng, ng).T
+    H = T + np.diag(vloc.ravel())
+    if kb is not None:
+        for s in range(kb.nsphere):
+            sl = slice(kb.sph_ptr[s], kb.sph_ptr[s + 1])
+            idx = kb.sph_idx[sl]
+            for p in range(kb.nproj):
+                b = np.zeros(ng)
+                b[idx] = kb.beta[sl, p]
+                H += g.dV * kb.D[s, p] * np.outer(b, b)
+    return H
+
+
+def small_problem(n=8, h=0.7, with_kb=True, seed=3):
+    g = W.Grid(n, n, n, h, h, h)
+    rng = np.random.default_rng(seed)
+    centers = rng.uniform(0, n * h, size=(3, 3))
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    kb = W.kb_projectors(g, centers[:2], radius=1.8, sigma=0.7) if with_kb else None
+    return g, vloc, kb, rng
+
+
+def rvec(rng, g, nvec=1):
+    return rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+
+
+# ------------------------------------------------------------------ kinetic / local V pins
+@pytest.mark.parametrize("ld", [False, True])
+def test_plane_waves_are_kinetic_eigenvectors_including_nyquist(oracle, ld):
+    g = W.Grid(8, 6, 12, 0.5, 0.6, 0.45)
+    z, y, x = np.meshgrid(np.arange(g.nz), np.arange(g.ny), np.arange(g.nx), indexing="ij")
+    zero = np.zeros(g.shape)
+    for mx, my, mz in [(0, 0, 0), (1, 0, 0), (0, -2, 0), (0, 0, 5), (-4, 3, -6), (3, -3, 2), (-4, -3, -6)]:
+        pw = np.exp(2j * np.pi * (mx * x / g.nx + my * y / g.ny + mz * z / g.nz))[None]
+        k2 = (2 * np.pi * mx / (g.nx * g.hx)) ** 2 + (2 * np.pi * my / (g.ny * g.hy)) ** 2 + \
+             (2 * np.pi * mz / (g.nz * g.hz)) ** 2
+        out = oracle.apply_H(g, zero, None, pw, ld)
+        assert np.abs(out - 0.5 * k2 * pw).max() < 1e-12 * max(1.0, k2)
+        out = oracle.apply_H(g, zero + 0.37, None, pw, ld)           # V = const c: eigenvalue k^2/2 + c
+        assert np.abs(out - (0.5 * k2 + 0.37) * pw).max() < 1e-12 * max(1.0, k2)
+
+
+def test_dense_matrix_and_hermiticity(oracle):
+    g, vloc, kb, rng = small_problem(8)
+    H = dense_H(g, vloc, kb)
+    assert np.abs(H - H.conj().T).max() < 1e-12
+    v = rvec(rng, g, 3)
+    out = oracle.apply_H(g, vloc, kb, v)
+    want = (H @ v.reshape(3, -1).T).T.reshape(v.shape)
+    assert np.abs(out - want).max() < 1e-11
+    out_ld = oracle.apply_H(g, vloc, kb, v, ld=True)
+    assert np.linalg.norm(out_ld - out) / np.linalg.norm(out) < 1e-14
+    # Hermiticity of the oracle's own operator on a non-cubic grid: <u|Hv> = conj <v|Hu>
+    g2 = W.Grid(12, 10, 6, 0.5, 0.55, 0.7)
+    c2 = np.array([[2.0, 2.2, 2.1], [3.4, 3.0, 1.0]])
+    v2 = W.gaussian_vloc(g2, c2, [1.0, 2.0], [0.8, 1.0])
+    kb2 = W.kb_projectors(g2, c2, radius=1.9, sigma=0.7)
+    u, w = rvec(rng, g2), rvec(rng, g2)
+    a = np.vdot(u, oracle.apply_H(g2, v2, kb2, w))
+    b = np.vdot(w, oracle.apply_H(g2, v2, kb2, u))
+    assert abs(a - np.conj(b)) < 1e-11 * abs(a)
+
+
+def test_kb_single_projector_is_eigenvector_of_vnl(oracle):
+    g = W.Grid(12, 12, 12, 0.5, 0.5, 0.5)
+    kb = W.kb_projectors(g, np.array([[3.0, 3.0, 3.0]]), radius=2.0, sigma=0.7)   # on a grid point
+    zero = np.zeros(g.shape)
+    for p in range(4):
+        b = np.zeros(g.ng, dtype=np.complex128)
+        b[kb.sph_idx] = kb.beta[:, p]
+        b = b.reshape((1,) + g.shape)
+        vnl = oracle.apply_H(g, zero, kb, b) - oracle.apply_H(g, zero, None, b)
+        assert np.abs(vnl - kb.D[0, p] * b).max() < 1e-13
+
+
+# ------------------------------------------------------------------ Chebyshev pins
+def test_cheb_polynomial_vs_dense_diagonalisation(oracle):
+    g, vloc, kb, rng = small_problem(8)
+    H = dense_H(g, vloc, kb)
+    ev, U = np.linalg.eigh(H)
+    emin, emax = W.spectral_bounds(g, vloc, True)
+    assert emin < ev[0] and ev[-1] < emax                           # spectrum inside analytic bounds
+    eb, de = 0.5 * (emax + emin), 0.5 * (emax - emin)
+    nterms = 40
+    coeffs = rng.standard_normal(nterms)                            # ANY coefficients
+    v = rvec(rng, g, 2)
+    got = oracle.cheb_filter(g, vloc, kb, v, coeffs, emin, emax)
+    x = (ev - eb) / de
+    p = sum(coeffs[n] * np.cos(n * np.arccos(x)) for n in range(nterms))
+    want = ((U * p[None, :]) @ (U.conj().T @ v.reshape(2, -1).T)).T.reshape(v.shape)
+    assert np.linalg.norm(got - want) / np.linalg.norm(want) < 1e-12
+    got_ld = oracle.cheb_filter(g, vloc, kb, v, coeffs, emin, emax, ld=True)
+    assert np.linalg.norm(got_ld - want) / np.linalg.norm(want) < 1e-12
+
+
+def test_cheb_unit_coefficient_gives_Tn_closed_form(oracle):
+    g = W.Grid(8, 8, 8, 0.6, 0.6, 0.6)
+    z, y, x = np.meshgrid(np.arange(8), np.arange(8), np.arange(8), indexing="ij")
+    pw = np.exp(2j * np.pi * (2 * x - 3 * y + z) / 8)[None]
+    eps = 0.5 * (2 * np.pi / (8 * 0.6)) ** 2 * (4 + 9 + 1) + 0.25
+    vloc = np.full(g.shape, 0.25)
+    emin, emax = -1.0, 45.0
+    xt = (eps - 0.5 * (emax + emin)) / (0.5 * (emax - emin))
+    for n in (0, 1, 2, 7, 30):
+        c = np.zeros(n + 1)
+        c[n] = 1.0
+        got = oracle.cheb_filter(g, vloc, None, pw, c, emin, emax)
+        assert np.abs(got - math.cos(n * math.acos(xt)) * pw).max() < 1e-11
+
+
+def test_cheb_converged_filter_equals_f_of_H(oracle):
+    g, vloc, kb, rng = small_problem(8, h=1.0)
+    H = dense_H(g, vloc, kb)
+    ev, U = np.linalg.eigh(H)
+    emin, emax = W.spectral_bounds(g, vloc, True)
+
+    def f(e):
+        return W.sqrt_fermi(e, mu=-0.2, beta=4.0)
+    coeffs = W.cheb_coeffs(f, emin, emax, 300)
+    assert abs(coeffs[-1]) < 1e-13
+    v = rvec(rng, g, 1)
+    got = oracle.cheb_filter(g, vloc, kb, v, coeffs, emin, emax)
+    want = ((U * f(ev)[None, :]) @ (U.conj().T @ v.reshape(1, -1).T)).T.reshape(v.shape)
+    assert np.linalg.norm(got - want) / np.linalg.norm(want) < 1e-11
+
+
+# ------------------------------------------------------------------ Hartree pins
+def test_hartree_gaussian_charge_matches_erf_closed_form(oracle):
+    n, h, sigma, Q = 48, 0.5, 1.0, 1.7
+    g = W.Grid(n, n, n, h, h, h)
+    c = np.array([12.13, 11.9, 12.31])                              # off-grid centre
+    ax = np.arange(n) * h
+    z, y, x = np.meshgrid(ax, ax, ax, indexing="ij")
+    d = np.sqrt((x - c[0]) ** 2 + (y - c[1]) ** 2 + (z - c[2]) ** 2)
+    rho = Q * (2 * np.pi * sigma ** 2) ** -1.5 * np.exp(-d ** 2 / (2 * sigma ** 2))
+    vh = oracle.poisson(g, rho)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        want = np.where(d > 0, Q * erf(d / (math.sqrt(2) * sigma)) / d, Q * math.sqrt(2 / np.pi) / sigma)
+    Rc = n * h / 2
+    m = d < Rc - 6 * sigma
+    assert m.sum() > 5000
+    assert (np.abs(vh - want)[m] / np.abs(want[m])).max() < 1e-9
+    m7 = d < Rc - 7 * sigma
+    assert (np.abs(vh - want)[m7] / np.abs(want[m7])).max() < 1e-11
+
+
+def test_hartree_density_and_linearity(oracle):
+    g = W.Grid(10, 8, 6, 0.5, 0.6, 0.7)
+    rng = np.random.default_rng(5)
+    psi = rvec(rng, g, 3)
+    vh, rho = oracle.hartree(g, psi, 0.37)
+    assert np.abs(rho - 0.37 * np.sum(np.abs(psi) ** 2, axis=0)).max() < 1e-13
+    vh2, _ = oracle.hartree(g, psi, 0.74)
+    assert np.abs(vh2 - 2 * vh).max() < 1e-12 * np.abs(vh).max()
+    # against numpy.fft with the same kernel, written out independently
+    kx, ky, kz = kgrid(g)
+    k = np.sqrt(kx ** 2 + ky ** 2 + kz ** 2)
+    Rc = min(g.box) / 2
+    with np.errstate(divide="ignore", invalid="ignore"):
+        vk = np.where(k > 0, 4 * np.pi * (1 - np.cos(k * Rc)) / k ** 2, 2 * np.pi * Rc ** 2)
+    want = np.fft.ifftn(vk * np.fft.fftn(rho)).real
+    assert np.abs(vh - want).max() < 1e-12 * np.abs(want).max()
+
+
+# ------------------------------------------------------------------ TD pins
+def test_td_local_only_is_unitary_and_const_V_is_a_phase(oracle):
+    g, vloc, _, rng = small_problem(8, with_kb=False)
+    psi = rvec(rng, g, 2)
+    out = oracle.td_propagate(g, vloc, None, psi, 0.05, 20)
+    assert np.abs(oracle.norms(out) / oracle.norms(psi) - 1).max() < 1e-13
+    # V = const, single plane wave: exact phase e^{-i (k^2/2 + c) t}
+    z, y, x = np.meshgrid(np.arange(8), np.arange(8), np.arange(8), indexing="ij")
+    pw = np.exp(2j * np.pi * (x - 2 * y + 3 * z) / 8)[None]
+    eps = 0.5 * (2 * np.pi / (8 * g.hx)) ** 2 * 14
+    for c in (0.0, 0.4):
+        out = oracle.td_propagate(g, np.full(g.shape, c), None, pw, 0.05, 7)
+        assert np.abs(out - np.exp(-1j * (eps + c) * 0.35) * pw).max() < 1e-12
+
+
+def test_td_frozen_V_is_second_order_and_reversible(oracle):
+    g = W.Grid(6, 6, 6, 0.8, 0.8, 0.8)
+    rng = np.random.default_rng(11)
+    centers = rng.uniform(0, 4.8, size=(2, 3))
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0], [0.9, 1.1])
+    H = dense_H(g, vloc, None)
+    psi = rvec(rng, g, 1)
+    t = 0.4
+    exact = (expm(-1j * H * t) @ psi.reshape(-1)).reshape(psi.shape)
+    errs = []
+    for nst in (4, 8, 16):
+        out = oracle.td_propagate(g, vloc, None, psi, t / nst, nst)
+        errs.append(np.linalg.norm(out - exact))
+    assert 3.5 < errs[0] / errs[1] < 4.5 and 3.5 < errs[1] / errs[2] < 4.5
+    fwd = oracle.td_propagate(g, vloc, None, psi, 0.05, 5)
+    back = oracle.td_propagate(g, vloc, None, fwd, -0.05, 5)
+    assert np.linalg.norm(back - psi) / np.linalg.norm(psi) < 1e-13
+
+
+def test_td_kb_orthonormal_projectors_exact_and_unitary(oracle):
+    """With ONE sphere centred on a grid point the 4 projectors are orthonormal, so NL(tau) is
+    exactly exp(-i V_NL tau); with T = V = 0 removed we check the factor through a full step against
+    the dense split-operator product."""
+    g = W.Grid(8, 8, 8, 0.6, 0.6, 0.6)
+    rng = np.random.default_rng(2)
+    kb = W.kb_projectors(g, np.array([[2.4, 2.4, 2.4]]), radius=1.7, sigma=0.6)
+    vloc = W.gaussian_vloc(g, np.array([[2.0, 2.5, 2.2]]), [1.5], [1.0])
+    psi = rvec(rng, g, 1)
+    dt = 0.05
+    out = oracle.td_propagate(g, vloc, kb, psi, dt, 1)
+    zero = np.zeros(g.shape)
+    T = dense_H(g, zero, None)
+    VNL = dense_H(g, zero, kb) - T
+    Uv = np.exp(-0.5j * dt * vloc.ravel())
+    Unl = expm(-0.5j * dt * VNL)
+    x = Uv * psi.reshape(-1)
+    x = Unl @ x
+    x = expm(-1j * dt * T) @ x
+    x = Unl @ x
+    x = Uv * x
+    assert np.linalg.norm(out.reshape(-1) - x) / np.linalg.norm(x) < 1e-12
+    out = oracle.td_propagate(g, vloc, kb, psi, dt, 10)
+    assert abs(oracle.norms(out)[0] / oracle.norms(psi)[0] - 1) < 1e-12
+
+
+def test_td_hartree_mode_uses_start_of_step_density(oracle):
+    """One step with hartree_mode=1 equals one frozen-V step with V = V_loc + V_H[rho(psi_0)]."""
+    g, vloc, _, rng = small_problem(8, with_kb=False)
+    psi = rvec(rng, g, 3)
+    rs = 2.0 / (3 * g.dV) * 0.01
+    vh, _ = oracle.hartree(g, psi, rs)
+    a = oracle.td_propagate(g, vloc, None, psi, 0.05, 1, hartree_mode=1, rho_scale=rs)
+    b = oracle.td_propagate(g, vloc + vh, None, psi, 0.05, 1)
+    assert np.linalg.norm(a - b) / np.linalg.norm(b) < 1e-14
+    # and it stays unitary over several steps (V real at every step)
+    c = oracle.td_propagate(g, vloc, None, psi, 0.05, 6, hartree_mode=1, rho_scale=rs)
+    assert np.abs(oracle.norms(c) / oracle.norms(psi) - 1).max() < 1e-13
