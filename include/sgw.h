@@ -1,0 +1,116 @@
+/* sgw.h -- C ABI of libsgw: the data-parallel hot path of stochastic GW on one B200 (sm_100a).
+ *
+ * The path (arXiv 2601.21005; "P:NN" = line NN of the paper text, "R-n" = reading n in DESIGN.md):
+ * batched application of the Fourier-grid Kohn-Sham Hamiltonian H = -1/2 nabla^2 + V_loc + V_NL
+ * to many stochastic vectors, the Chebyshev filter built on it (Eq. 3), and
+ * split-operator propagation under a time-dependent Hartree potential.
+ *
+ * Conventions
+ *  - Every call returns 0 on success or a negative code; nothing aborts or throws.
+ *      SGW_EINVAL (-1) bad argument        SGW_ESIZE (-2) unsupported grid length
+ *      SGW_ENOMEM (-3) allocation failed   SGW_ECUDA (-4) CUDA runtime error
+ *    sgw_last_error() returns a thread-local message for the last failing call.
+ *  - d_* are DEVICE pointers into caller-owned memory; h_* are HOST pointers read during the call.
+ *  - Complex vectors are interleaved (re,im) IEEE double, 16 B per element, layout
+ *    [nvec][nz][ny][nx] with x fastest; flat grid index g = ix + nx*(iy + ny*iz) (packed
+ *    (N_g x n) multi-index arrays).  Real fields (V_loc, rho, V_H) are [nz][ny][nx] doubles.
+ *  - All work is enqueued on the CUDA stream given to sgw_init_grid and is asynchronous with
+ *    respect to the host; the library synchronises only inside sgw_init_grid / sgw_set_* /
+ *    sgw_destroy (setup) and on error paths.  k-space data never crosses the boundary.
+ *  - Supported axis lengths: 8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256, 384 (products of 2 and
+ *    3 with a compiled two-stage factorisation); nx must be a multiple of 4.  Others: SGW_ESIZE.
+ *  - The library owns only its context (tables, workspace for max_nvec vectors).  Calls with
+ *    nvec > max_nvec are processed in sub-batches of max_nvec (vectors are independent in the
+ *    filter; in the TD step the density is accumulated over all sub-batches first).
+ *  - There is no CPU fallback: without a CUDA device sgw_init_grid fails with SGW_ECUDA.
+ */
+#ifndef SGW_H
+#define SGW_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SGW_OK 0
+#define SGW_EINVAL (-1)
+#define SGW_ESIZE (-2)
+#define SGW_ENOMEM (-3)
+#define SGW_ECUDA (-4)
+
+typedef struct sgw_ctx sgw_ctx;
+
+/* Create a context for an nx*ny*nz periodic grid with spacings hx,hy,hz (bohr) (N_g =
+ * N_x N_y N_z).  k_i = 2 pi m/(N_i h_i), m in [-N_i/2, N_i/2) (R: SURVEY 8(a) a3).  max_nvec
+ * sizes the internal workspace (3 complex arrays of max_nvec*N_g, allocated lazily by the first
+ * call that needs them).  cuda_stream is a cudaStream_t owned by the caller (NULL = default
+ * stream).  *ctx is written on success only. */
+int sgw_init_grid(sgw_ctx** ctx, int nx, int ny, int nz, double hx, double hy, double hz,
+                  int max_nvec, void* cuda_stream);
+
+/* Free the context and everything it allocated.  Synchronises the stream first. */
+int sgw_destroy(sgw_ctx* ctx);
+
+/* Set the local potential V_loc(r) (Ha), N_g device doubles; copied into the context (the
+ * potential-energy operator is diagonal in position).  NULL clears it (V_loc = 0). */
+int sgw_set_vloc(sgw_ctx* ctx, const double* d_vloc);
+
+/* Set the Kleinman-Bylander nonlocal term V_NL = sum_{s,p} |beta_sp> D_sp dV <beta_sp| as sparse
+ * sphere lists ("pseudopotential contribution ... applied via atomic operations on grid
+ * points where pseudopotentials for neighboring atoms overlap"; R-12).  d_sph_ptr[nsphere+1]
+ * (int64) delimits each sphere's points in d_sph_idx (int32 flat grid indices) and d_beta
+ * ([point][nproj] doubles); d_D is [nsphere][nproj] (Ha).  All four arrays are copied.
+ * nproj_per_sphere must be 1..8.  nsphere = 0 clears the term. */
+int sgw_set_nonlocal(sgw_ctx* ctx, int nsphere, const int64_t* d_sph_ptr, const int32_t* d_sph_idx,
+                     int nproj_per_sphere, const double* d_beta, const double* d_D);
+
+/* White-noise start vectors (R-4, R-5): element g of vector first_vec+j is
+ * (h >> 63) ? -1.0 : +1.0 with h = sm64(sm64(sm64(seed) ^ (first_vec+j)) ^ g), imaginary part 0,
+ * where sm64 is the splitmix64 output function.  Writes nvec*N_g complex to d_psi.  Bit-exact
+ * and independent of batching. */
+int sgw_random_vectors(sgw_ctx* ctx, uint64_t seed, int first_vec, int nvec, void* d_psi);
+
+/* d_out = H d_in for nvec vectors, out of place (d_out must not alias d_in):
+ * H psi = F^-1[ 1/2 |k|^2 F psi ] + V_loc psi + V_NL psi. */
+int sgw_apply_H(sgw_ctx* ctx, int nvec, const void* d_in, void* d_out);
+
+/* Chebyshev filter in place (Eq. 3; R-1): d_psi <- sum_{n<nterms} h_coeffs[n] T_n(Ht) d_psi,
+ * Ht = (H - Eb)/dE, Eb = (Emax+Emin)/2, dE = (Emax-Emin)/2; three-term recurrence, nterms-1
+ * applications of H.  h_coeffs: nterms host doubles.  Requires nterms >= 1 and Emax > Emin. */
+int sgw_cheb_filter(sgw_ctx* ctx, int nvec, void* d_psi, const double* h_coeffs, double Emin,
+                    double Emax, int nterms);
+
+/* rho(r) = rho_scale * sum_l |psi_l(r)|^2 over the nvec vectors (all N_eta orbitals on
+ * one rank so the density needs no communication), and the Hartree potential
+ * V_H = F^-1[ v(k) F rho ], v(k) = 4 pi (1 - cos(|k| Rc))/|k|^2, v(0) = 2 pi Rc^2,
+ * Rc = min(Lx,Ly,Lz)/2 (R-10: spherically cut Coulomb kernel).  d_vh: N_g doubles out;
+ * d_rho: N_g doubles out or NULL. */
+int sgw_hartree(sgw_ctx* ctx, int nvec, const void* d_psi, double rho_scale, double* d_vh, double* d_rho);
+
+/* Select the time-dependent part of the propagation Hamiltonian ("time-dependent
+ * Hartree"; R-9): hartree_mode 0: V = V_loc frozen; 1: V = V_loc + V_H[rho(t_n)], rebuilt at the
+ * start of every step from the current vectors with the given rho_scale. */
+int sgw_set_td(sgw_ctx* ctx, int hartree_mode, double rho_scale);
+
+/* nsteps symmetric split-operator steps in place (P:84, P:155 dt = 0.05; R-8, R-11):
+ * psi <- e^{-iV dt/2} NL(dt/2) F^-1 e^{-i |k|^2 dt/2} F NL(dt/2) e^{-iV dt/2} psi,
+ * NL(tau) psi = psi + sum_{s,p} beta_sp (e^{-i D_sp tau} - 1) dV <beta_sp|psi>.
+ * dt may be negative (reverse-time propagation). */
+int sgw_td_propagate(sgw_ctx* ctx, int nvec, void* d_psi, double dt, int nsteps);
+
+/* d_out[l] = sum_g |psi_l(g)|^2 (no dV factor), nvec doubles (normalisations as segmented
+ * sums with one atomic add per segment).  Test helper. */
+int sgw_norms(sgw_ctx* ctx, int nvec, const void* d_psi, double* d_out);
+
+/* Number of kernels the library has launched on this context since creation (for bench.py's
+ * gpu_launches).  Host counter; never fails (returns 0 for NULL). */
+int64_t sgw_launch_count(const sgw_ctx* ctx);
+
+/* Message for the last error on the calling thread ("" if none). */
+const char* sgw_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SGW_H */
