@@ -1,0 +1,57 @@
+// sgw_ctx.h -- the library context (host-side state) shared by the translation units of libsgw.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/sgw.h"
+#include "sgw_ops.cuh"
+
+struct sgw_ctx {
+    int nx, ny, nz;
+    double hx, hy, hz;
+    long long ng;
+    int max_nvec;
+    cudaStream_t stream;
+    int B;                                   // pencils per CTA on the strided axes (y, z)
+    int Bx;                                  // pencils per CTA on the contiguous axis (x)
+    sgw::pass_launch_fn pass[3];             // per-axis launcher (x, y, z)
+    int dims[3];
+    double hs[3];
+    sgw::cd* tw[3];                          // exp(-2 pi i j/N) per axis
+    std::vector<double> h_kin[3];            // 1/2 k^2 per axis (host)
+    double* kin[3];                          // 1/2 k^2 / N per axis (device)
+    double* cheb_kin[3];                     // s * 1/2 k^2 / N (rebuilt per filter call)
+    sgw::cd* td_kin[3];                      // exp(-i 1/2 k^2 dt)/N (rebuilt when dt changes)
+    double td_dt;
+    bool td_kin_valid;
+    double* vloc;                            // N_g or NULL
+    double* vtab;                            // scaled potential for the filter, N_g
+    double* vk3d;                            // Poisson kernel v(k)/N_g, N_g
+    // Kleinman-Bylander lists
+    int nsphere, nproj;
+    int64_t* sph_ptr;
+    int32_t* sph_idx;
+    double* beta;
+    double* D;
+    sgw::cd* kbc;                            // [nvec][nsphere][nproj] projections
+    long long kbc_cap;
+    // workspace
+    sgw::cd* ws[3];
+    sgw::cd* pois;                           // N_g complex scratch for the Poisson solve
+    double* rho;
+    double* vh;
+    sgw::cd* phase;                          // exp(-i V dt/2), N_g
+    int hartree_mode;
+    double rho_scale;
+    int64_t launches;
+};
+
+namespace sgw {
+int set_error(int code, const std::string& msg);
+int check_cuda(cudaError_t e, const char* what);
+PassGeom geom_for_axis(const sgw_ctx* c, int axis, int nvec, long long* ntiles);
+int run_pass(sgw_ctx* c, int axis, int kind, int nvec, const cd* in, const OpParams& p);
+}  // namespace sgw

@@ -1,0 +1,195 @@
+// sgw_kernels.cuh -- the non-FFT kernels of the hot path: counter RNG, density, phases, the sparse
+// Kleinman-Bylander gather-dot-scatter, segmented norms.
+#pragma once
+#include "sgw_fft.cuh"
+
+namespace sgw {
+
+// ---- a1: white-noise vectors (R-4, R-5) -------------------------------------------------
+__host__ __device__ __forceinline__ uint64_t sm64(uint64_t x) {
+    x += 0x9E3779B97F4A7C15ULL;
+    x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    x = (x ^ (x >> 27)) * 0x94D049BB133111EBULL;
+    return x ^ (x >> 31);
+}
+
+// grid (ceil(ng/ (256*4)), nvec): each thread writes 4 consecutive elements (64 B)
+static __global__ void rng_kernel(cd* __restrict__ psi, uint64_t seed_mixed, int first_vec, long long ng) {
+    const int v = blockIdx.y;
+    const uint64_t key = sm64(seed_mixed ^ (uint64_t)(first_vec + v));
+    const long long g0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    cd* dst = psi + (long long)v * ng;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const long long g = g0 + j;
+        if (g < ng) {
+            const uint64_t h = sm64(key ^ (uint64_t)g);
+            dst[g] = make_double2((h >> 63) ? -1.0 : 1.0, 0.0);
+        }
+    }
+}
+
+// ---- a9: density --------------------------------------------------------------------
+static __global__ void density_kernel(const cd* __restrict__ psi, int nvec, long long ng, double scale,
+                                      double* __restrict__ rho, double* __restrict__ rho2) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ng) return;
+    double s = 0.0;
+    for (int v = 0; v < nvec; ++v) {
+        const cd a = psi[(long long)v * ng + i];
+        s += a.x * a.x + a.y * a.y;
+    }
+    s *= scale;
+    rho[i] = s;
+    if (rho2) rho2[i] = s;
+}
+
+static __global__ void real_to_complex_kernel(const double* __restrict__ r, cd* __restrict__ c, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) c[i] = make_double2(r[i], 0.0);
+}
+static __global__ void complex_to_real_kernel(const cd* __restrict__ c, double* __restrict__ r, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) r[i] = c[i].x;
+}
+
+// phase[g] = exp(-i (vloc[g] + vh[g]) * half_dt)
+static __global__ void phase_kernel(const double* __restrict__ vloc, const double* __restrict__ vh, double half_dt,
+                                    cd* __restrict__ phase, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double v = vloc ? vloc[i] : 0.0;
+    if (vh) v += vh[i];
+    double s, c;
+    sincos(v * half_dt, &s, &c);
+    phase[i] = make_double2(c, -s);
+}
+
+// psi[v][g] *= phase[g]
+static __global__ void apply_phase_kernel(cd* __restrict__ psi, const cd* __restrict__ phase, long long ng) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ng) return;
+    cd* p = psi + (long long)blockIdx.y * ng;
+    p[i] = cmul(p[i], phase[i]);
+}
+
+static __global__ void scale_kernel(cd* __restrict__ psi, double a, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) psi[i] = cscale(psi[i], a);
+}
+
+// vtab[g] = s * (vloc[g] - Eb)
+static __global__ void vtab_kernel(const double* __restrict__ vloc, double s, double Eb, double* __restrict__ vtab,
+                                   long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) vtab[i] = s * ((vloc ? vloc[i] : 0.0) - Eb);
+}
+
+static __global__ void scale_table_kernel(const double* __restrict__ in, double s, double* __restrict__ out, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = s * in[i];
+}
+
+// ---- norms as segmented sums + one atomic per segment -------------------------------
+static __global__ void norms_kernel(const cd* __restrict__ psi, long long ng, double* __restrict__ out) {
+    const int v = blockIdx.y;
+    const cd* p = psi + (long long)v * ng;
+    double s = 0.0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ng; i += (long long)gridDim.x * blockDim.x) {
+        const cd a = p[i];
+        s += a.x * a.x + a.y * a.y;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    __shared__ double part[8];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += part[w];
+        atomicAdd(out + v, t);
+    }
+}
+
+// ---- a6: Kleinman-Bylander gather-dot (R-12) --------------------------------------------
+// grid (nsphere, nvec), 128 threads: c[v][s][p] = dV * sum_j beta[j][p] * psi_v[idx[j]]
+template <int NP>
+static __global__ void __launch_bounds__(128) kb_project_kernel(const cd* __restrict__ psi, long long ng,
+                                                                 const int64_t* __restrict__ ptr,
+                                                                 const int32_t* __restrict__ idx,
+                                                                 const double* __restrict__ beta, double dV,
+                                                                 cd* __restrict__ cout, int nsphere) {
+    const int s = blockIdx.x, v = blockIdx.y;
+    const cd* p = psi + (long long)v * ng;
+    double ar[NP], ai[NP];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) ar[q] = ai[q] = 0.0;
+    for (int64_t j = ptr[s] + threadIdx.x; j < ptr[s + 1]; j += blockDim.x) {
+        const cd a = p[idx[j]];
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            const double b = beta[j * NP + q];
+            ar[q] += b * a.x;
+            ai[q] += b * a.y;
+        }
+    }
+    __shared__ double red[4][2 * NP];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            ar[q] += __shfl_down_sync(0xffffffffu, ar[q], o);
+            ai[q] += __shfl_down_sync(0xffffffffu, ai[q], o);
+        }
+        if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5][2 * q] = ar[q]; red[threadIdx.x >> 5][2 * q + 1] = ai[q]; }
+    }
+    __syncthreads();
+    if (threadIdx.x < NP) {
+        const int q = threadIdx.x;
+        double re = 0.0, im = 0.0;
+        for (int w = 0; w < 4; ++w) { re += red[w][2 * q]; im += red[w][2 * q + 1]; }
+        cout[((long long)v * nsphere + s) * NP + q] = make_double2(re * dV, im * dV);
+    }
+}
+
+// scatter: dst_v[idx[j]] += sum_p beta[j][p] * f_p * c[v][s][p], atomics where spheres overlap
+//   mode 0: f_p = scale * D[s][p]                         (H apply / Chebyshev term)
+//   mode 1: f_p = exp(-i D[s][p] tau) - 1                 (propagator factor NL(tau), R-11)
+template <int NP>
+static __global__ void __launch_bounds__(128) kb_scatter_kernel(cd* __restrict__ dst, long long ng,
+                                                                 const int64_t* __restrict__ ptr,
+                                                                 const int32_t* __restrict__ idx,
+                                                                 const double* __restrict__ beta,
+                                                                 const double* __restrict__ D,
+                                                                 const cd* __restrict__ cin, int nsphere, int mode,
+                                                                 double scale_or_tau) {
+    const int s = blockIdx.x, v = blockIdx.y;
+    __shared__ cd f[NP];
+    if (threadIdx.x < NP) {
+        const int q = threadIdx.x;
+        const cd c = cin[((long long)v * nsphere + s) * NP + q];
+        const double d = D[s * NP + q];
+        if (mode == 0) f[q] = cscale(c, scale_or_tau * d);
+        else {
+            double sn, cs;
+            sincos(d * scale_or_tau, &sn, &cs);
+            f[q] = cmul(make_double2(cs - 1.0, -sn), c);
+        }
+    }
+    __syncthreads();
+    double* out = reinterpret_cast<double*>(dst + (long long)v * ng);
+    for (int64_t j = ptr[s] + threadIdx.x; j < ptr[s + 1]; j += blockDim.x) {
+        double re = 0.0, im = 0.0;
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            const double b = beta[j * NP + q];
+            re += b * f[q].x;
+            im += b * f[q].y;
+        }
+        const long long g = idx[j];
+        atomicAdd(out + 2 * g, re);
+        atomicAdd(out + 2 * g + 1, im);
+    }
+}
+
+}  // namespace sgw

@@ -1,0 +1,252 @@
+// sgw_solvers.cu -- the hot-path entry points of libsgw (include/sgw.h): random vectors, H apply,
+// Chebyshev filter, Hartree, split-operator propagation, norms.
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "sgw_ctx.h"
+#include "sgw_kernels.cuh"
+
+using namespace sgw;
+
+namespace {
+
+inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) / t); }
+
+#define SGW_TRY(expr)            \
+    do {                         \
+        int rc_ = (expr);        \
+        if (rc_ != 0) return rc_; \
+    } while (0)
+
+int launched(sgw_ctx* c, const char* what) {
+    c->launches++;
+    return check_cuda(cudaGetLastError(), what);
+}
+
+int ensure_ws(sgw_ctx* c, int n) {
+    for (int a = 0; a < n; ++a)
+        if (!c->ws[a])
+            SGW_TRY(check_cuda(cudaMalloc((void**)&c->ws[a], (size_t)c->max_nvec * c->ng * sizeof(cd)), "workspace"));
+    return 0;
+}
+
+int ensure_kbc(sgw_ctx* c, int nvec) {
+    const long long need = (long long)nvec * c->nsphere * c->nproj;
+    if (need <= c->kbc_cap) return 0;
+    SGW_TRY(check_cuda(cudaStreamSynchronize(c->stream), "sync"));
+    cudaFree(c->kbc);
+    c->kbc = nullptr; c->kbc_cap = 0;
+    SGW_TRY(check_cuda(cudaMalloc((void**)&c->kbc, need * sizeof(cd)), "kb buffer"));
+    c->kbc_cap = need;
+    return 0;
+}
+
+template <int NP>
+int kb_apply_np(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau) {
+    dim3 grid(c->nsphere, nvec);
+    const double dV = c->hx * c->hy * c->hz;
+    kb_project_kernel<NP><<<grid, 128, 0, c->stream>>>(src, c->ng, c->sph_ptr, c->sph_idx, c->beta, dV, c->kbc, c->nsphere);
+    SGW_TRY(launched(c, "kb_project"));
+    kb_scatter_kernel<NP><<<grid, 128, 0, c->stream>>>(dst, c->ng, c->sph_ptr, c->sph_idx, c->beta, c->D, c->kbc,
+                                                       c->nsphere, mode, scale_or_tau);
+    return launched(c, "kb_scatter");
+}
+
+// dst += sum beta f <beta|src>, all projections taken from src before any scatter (R-11)
+int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau) {
+    if (c->nsphere == 0) return 0;
+    SGW_TRY(ensure_kbc(c, nvec));
+    switch (c->nproj) {
+        case 1: return kb_apply_np<1>(c, nvec, src, dst, mode, scale_or_tau);
+        case 2: return kb_apply_np<2>(c, nvec, src, dst, mode, scale_or_tau);
+        case 3: return kb_apply_np<3>(c, nvec, src, dst, mode, scale_or_tau);
+        case 4: return kb_apply_np<4>(c, nvec, src, dst, mode, scale_or_tau);
+        case 5: return kb_apply_np<5>(c, nvec, src, dst, mode, scale_or_tau);
+        case 6: return kb_apply_np<6>(c, nvec, src, dst, mode, scale_or_tau);
+        case 7: return kb_apply_np<7>(c, nvec, src, dst, mode, scale_or_tau);
+        case 8: return kb_apply_np<8>(c, nvec, src, dst, mode, scale_or_tau);
+    }
+    return set_error(SGW_EINVAL, "bad nproj");
+}
+
+OpParams zero_params() {
+    OpParams p;
+    memset(&p, 0, sizeof(p));
+    return p;
+}
+
+// rho = scale * sum |psi|^2 ; V_H by the cut-Coulomb Poisson solve (R-10).  Results in c->vh (and rho/rho2).
+int hartree_into(sgw_ctx* c, int nvec, const cd* psi, double rho_scale, double* rho2) {
+    const long long ng = c->ng;
+    density_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(psi, nvec, ng, rho_scale, c->rho, rho2);
+    SGW_TRY(launched(c, "density"));
+    real_to_complex_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->rho, c->pois, ng);
+    SGW_TRY(launched(c, "r2c"));
+    OpParams p = zero_params();
+    p.out = c->pois;
+    SGW_TRY(run_pass(c, 0, K_FWD, 1, c->pois, p));
+    SGW_TRY(run_pass(c, 1, K_FWD, 1, c->pois, p));
+    p.mul3d = c->vk3d;
+    SGW_TRY(run_pass(c, 2, K_RT_MUL3D, 1, c->pois, p));
+    p.mul3d = nullptr;
+    SGW_TRY(run_pass(c, 1, K_INV, 1, c->pois, p));
+    SGW_TRY(run_pass(c, 0, K_INV, 1, c->pois, p));
+    complex_to_real_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->pois, c->vh, ng);
+    return launched(c, "c2r");
+}
+
+}  // namespace
+
+extern "C" int sgw_random_vectors(sgw_ctx* c, uint64_t seed, int first_vec, int nvec, void* d_psi) {
+    if (!c || nvec < 0 || first_vec < 0 || (nvec > 0 && !d_psi)) return set_error(SGW_EINVAL, "sgw_random_vectors: bad argument");
+    if (nvec == 0) return SGW_OK;
+    dim3 grid(blocks_for(c->ng, 1024), nvec);
+    rng_kernel<<<grid, 256, 0, c->stream>>>((cd*)d_psi, sm64(seed), first_vec, c->ng);
+    return launched(c, "rng_kernel");
+}
+
+extern "C" int sgw_norms(sgw_ctx* c, int nvec, const void* d_psi, double* d_out) {
+    if (!c || nvec < 0 || (nvec > 0 && (!d_psi || !d_out))) return set_error(SGW_EINVAL, "sgw_norms: bad argument");
+    if (nvec == 0) return SGW_OK;
+    SGW_TRY(check_cuda(cudaMemsetAsync(d_out, 0, nvec * sizeof(double), c->stream), "memset"));
+    const long long seg = 256LL * 256;          // segments of length L ~ 256 per thread block row
+    dim3 grid((unsigned)((c->ng + seg - 1) / seg), nvec);
+    norms_kernel<<<grid, 256, 0, c->stream>>>((const cd*)d_psi, c->ng, d_out);
+    return launched(c, "norms_kernel");
+}
+
+extern "C" int sgw_apply_H(sgw_ctx* c, int nvec, const void* d_in, void* d_out) {
+    if (!c || nvec < 0 || (nvec > 0 && (!d_in || !d_out)) || d_in == d_out) return set_error(SGW_EINVAL, "sgw_apply_H: bad argument");
+    const cd* in = (const cd*)d_in;
+    cd* out = (cd*)d_out;
+    for (int v0 = 0; v0 < nvec; v0 += c->max_nvec) {
+        const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
+        const cd* i0 = in + (long long)v0 * c->ng;
+        cd* o0 = out + (long long)v0 * c->ng;
+        OpParams p = zero_params();
+        p.out = o0;
+        p.mul_re = c->kin[0];
+        SGW_TRY(run_pass(c, 0, K_RT_STORE, nv, i0, p));
+        p.mul_re = c->kin[1]; p.acc = o0;
+        SGW_TRY(run_pass(c, 1, K_RT_ACC, nv, i0, p));
+        SGW_TRY(kb_apply(c, nv, i0, o0, 0, 1.0));
+        p.mul_re = c->kin[2]; p.vtab = c->vloc;
+        SGW_TRY(run_pass(c, 2, K_RT_HFIN, nv, i0, p));
+    }
+    return SGW_OK;
+}
+
+extern "C" int sgw_hartree(sgw_ctx* c, int nvec, const void* d_psi, double rho_scale, double* d_vh, double* d_rho) {
+    if (!c || nvec < 0 || (nvec > 0 && !d_psi) || !d_vh) return set_error(SGW_EINVAL, "sgw_hartree: bad argument");
+    SGW_TRY(hartree_into(c, nvec, (const cd*)d_psi, rho_scale, d_rho));
+    return check_cuda(cudaMemcpyAsync(d_vh, c->vh, c->ng * sizeof(double), cudaMemcpyDeviceToDevice, c->stream), "copy vh");
+}
+
+extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, double Emin, double Emax,
+                               int nterms) {
+    if (!c || nvec < 0 || (nvec > 0 && !d_psi) || !h_coeffs || nterms < 1 || !(Emax > Emin))
+        return set_error(SGW_EINVAL, "sgw_cheb_filter: bad argument");
+    if (nvec == 0) return SGW_OK;
+    const long long ng = c->ng;
+    const double Eb = 0.5 * (Emax + Emin), dE = 0.5 * (Emax - Emin), s = 2.0 / dE;
+    if (nterms == 1) {
+        scale_kernel<<<blocks_for(ng * nvec, 256), 256, 0, c->stream>>>((cd*)d_psi, h_coeffs[0], ng * nvec);
+        return launched(c, "scale");
+    }
+    SGW_TRY(ensure_ws(c, 3));
+    // tables scaled by s = 2/dE so that one pass yields 2*Ht*phi directly (R-1; Eq. 3 mapping to [-1,1])
+    for (int a = 0; a < 3; ++a) {
+        scale_table_kernel<<<blocks_for(c->dims[a], 128), 128, 0, c->stream>>>(c->kin[a], s, c->cheb_kin[a], c->dims[a]);
+        SGW_TRY(launched(c, "scale_table"));
+    }
+    vtab_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, s, Eb, c->vtab, ng);
+    SGW_TRY(launched(c, "vtab"));
+    for (int v0 = 0; v0 < nvec; v0 += c->max_nvec) {
+        const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
+        cd* X0 = (cd*)d_psi + (long long)v0 * ng;
+        cd *P1 = c->ws[0], *W = c->ws[1], *O = c->ws[2];
+        cd* cur = X0;
+        cd* other = P1;              // receives phi_n; holds phi_{n-2} for n >= 2
+        // series terms not yet added to O: flags for degrees n-2 and n-1 (phi_{n-2}, phi_{n-1}, phi_n are
+        // all in registers in the last pass of term n, so O is touched only every third term)
+        bool pend_m2 = false, pend_m1 = true;  // before n = 1: degree 0 (= n-1) is pending
+        bool series_started = false;
+        for (int n = 1; n < nterms; ++n) {
+            OpParams p = zero_params();
+            p.out = W; p.mul_re = c->cheb_kin[0];
+            SGW_TRY(run_pass(c, 0, K_RT_STORE, nv, cur, p));
+            p.mul_re = c->cheb_kin[1]; p.acc = W;
+            SGW_TRY(run_pass(c, 1, K_RT_ACC, nv, cur, p));
+            SGW_TRY(kb_apply(c, nv, cur, W, 0, s));
+            p.mul_re = c->cheb_kin[2]; p.vtab = c->vtab;
+            p.out = other; p.prev = other; p.use_prev = (n >= 2);
+            p.hs = (n == 1) ? 0.5 : 1.0;
+            const bool last = (n == nterms - 1);
+            const bool flush = last || pend_m2;
+            p.flush = flush; p.series = O; p.series_init = !series_started;
+            p.c0 = pend_m2 ? h_coeffs[n - 2] : 0.0;
+            p.c1 = pend_m1 ? h_coeffs[n - 1] : 0.0;
+            p.c2 = h_coeffs[n];
+            SGW_TRY(run_pass(c, 2, K_RT_CHEB, nv, cur, p));
+            if (flush) { series_started = true; pend_m2 = false; pend_m1 = false; }
+            else { pend_m2 = pend_m1; pend_m1 = true; }
+            cd* t = cur; cur = other; other = t;
+        }
+        SGW_TRY(check_cuda(cudaMemcpyAsync(X0, O, (size_t)nv * ng * sizeof(cd), cudaMemcpyDeviceToDevice, c->stream), "copy out"));
+    }
+    return SGW_OK;
+}
+
+extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, int nsteps) {
+    if (!c || nvec < 0 || (nvec > 0 && !d_psi) || nsteps < 0) return set_error(SGW_EINVAL, "sgw_td_propagate: bad argument");
+    if (nvec == 0 || nsteps == 0) return SGW_OK;
+    const long long ng = c->ng;
+    cd* psi = (cd*)d_psi;
+    if (!c->td_kin_valid || c->td_dt != dt) {
+        for (int a = 0; a < 3; ++a) {
+            const int N = c->dims[a];
+            std::vector<cd> t(N);
+            for (int j = 0; j < N; ++j) {
+                const long double ph = (long double)c->h_kin[a][j] * (long double)dt;
+                t[j] = make_double2((double)(cosl(ph) / N), (double)(-sinl(ph) / N));
+            }
+            SGW_TRY(check_cuda(cudaMemcpyAsync(c->td_kin[a], t.data(), N * sizeof(cd), cudaMemcpyHostToDevice, c->stream), "td table"));
+            SGW_TRY(check_cuda(cudaStreamSynchronize(c->stream), "td table sync"));
+        }
+        c->td_dt = dt; c->td_kin_valid = true;
+    }
+    const bool kb = c->nsphere > 0;
+    for (int step = 0; step < nsteps; ++step) {
+        if (c->hartree_mode || step == 0) {
+            const double* vh = nullptr;
+            if (c->hartree_mode) { SGW_TRY(hartree_into(c, nvec, psi, c->rho_scale, nullptr)); vh = c->vh; }
+            phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, vh, 0.5 * dt, c->phase, ng);
+            SGW_TRY(launched(c, "phase"));
+        }
+        OpParams p = zero_params();
+        p.out = psi;
+        if (kb) {
+            dim3 g2(blocks_for(ng, 256), nvec);
+            apply_phase_kernel<<<g2, 256, 0, c->stream>>>(psi, c->phase, ng);
+            SGW_TRY(launched(c, "apply_phase"));
+            SGW_TRY(kb_apply(c, nvec, psi, psi, 1, 0.5 * dt));
+        } else {
+            p.pro_phase = c->phase;
+        }
+        p.mul_c = c->td_kin[0];
+        SGW_TRY(run_pass(c, 0, K_RT_TD, nvec, psi, p));
+        p.pro_phase = nullptr; p.mul_c = c->td_kin[1];
+        SGW_TRY(run_pass(c, 1, K_RT_TD, nvec, psi, p));
+        p.mul_c = c->td_kin[2];
+        if (!kb) p.epi_phase = c->phase;
+        SGW_TRY(run_pass(c, 2, K_RT_TD, nvec, psi, p));
+        if (kb) {
+            SGW_TRY(kb_apply(c, nvec, psi, psi, 1, 0.5 * dt));
+            dim3 g2(blocks_for(ng, 256), nvec);
+            apply_phase_kernel<<<g2, 256, 0, c->stream>>>(psi, c->phase, ng);
+            SGW_TRY(launched(c, "apply_phase"));
+        }
+    }
+    return SGW_OK;
+}

@@ -1,0 +1,269 @@
+"""GPU parity: libsgw (through the C ABI binding) against the CPU oracle, element by element.
+
+Tolerances are BASELINE.json's: +-1 vectors bit-exact; relative L2 per vector <= 1e-11 per H apply
+and <= 1e-8 after a full filter or propagation (max over vectors).
+"""
+import numpy as np
+import pytest
+
+from paper_2601_21005_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_H = 1e-11
+TOL_FULL = 1e-8
+SIZES = [8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256, 384]
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def api(torch_cuda):
+    from paper_2601_21005_b200 import api as a
+    a.load()
+    return a
+
+
+def relerr(got, want):
+    """max over vectors of ||got - want|| / ||want||"""
+    got = got.reshape(got.shape[0], -1)
+    want = want.reshape(want.shape[0], -1)
+    return float(np.max(np.linalg.norm(got - want, axis=1) / np.linalg.norm(want, axis=1)))
+
+
+def rvec(rng, g, nvec):
+    return rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+
+
+def problem(nx, ny, nz, h=(0.5, 0.55, 0.6), kb=True, seed=0):
+    g = W.Grid(nx, ny, nz, *h)
+    rng = np.random.default_rng(seed)
+    L = np.array(g.box)
+    centers = rng.uniform(0, 1, size=(3, 3)) * L
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    kbl = W.kb_projectors(g, centers[:2], radius=min(1.8, 0.45 * L.min()), sigma=0.7) if kb else W.KB.empty()
+    return g, vloc, kbl, rng
+
+
+def make_ctx(api, torch, g, vloc, kb, max_nvec):
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, max_nvec)
+    if vloc is not None:
+        ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    if kb is not None and kb.nsphere:
+        ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                             torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+    return ctx
+
+
+# ------------------------------------------------------------------ RNG: bit exact
+def test_random_vectors_bit_exact(api, torch_cuda, oracle):
+    torch = torch_cuda
+    for (nx, ny, nz) in [(32, 32, 32), (12, 8, 24), (96, 16, 8)]:
+        g = W.Grid(nx, ny, nz, 0.5, 0.5, 0.5)
+        ctx = api.Context(nx, ny, nz, 0.5, 0.5, 0.5, 4)
+        for seed, first, nvec in [(W.SEED_VEC, 0, 4), (1, 2, 3), (0, 0, 1), (2 ** 63 + 12345, 61, 3)]:
+            got = ctx.sgw_random_vectors(seed, first, nvec).cpu().numpy()
+            want = oracle.random_vectors(g, seed, first, nvec)
+            assert got.shape == want.shape
+            assert np.array_equal(got.view(np.uint64), want.view(np.uint64))     # bit for bit
+        ctx.close()
+
+
+def test_random_vectors_golden_entries(api, torch_cuda):
+    g = W.Grid(32, 32, 32, 0.5, 0.5, 0.5)
+    ctx = api.Context(32, 32, 32, 0.5, 0.5, 0.5, 4)
+    assert ctx.sgw_random_vectors(0, 0, 1).flatten()[0].item() == 1.0        # tests/golden/keyed_hash.txt
+    assert ctx.sgw_random_vectors(1, 0, 1).flatten()[0].item() == -1.0
+    assert ctx.sgw_random_vectors(1, 2, 1).flatten()[3].item() == -1.0
+    assert ctx.sgw_random_vectors(5, 0, 0).shape[0] == 0                     # empty batch
+    assert g.ng == 32768
+
+
+# ------------------------------------------------------------------ H apply
+@pytest.mark.parametrize("n", SIZES)
+def test_apply_H_every_length_on_every_axis(api, torch_cuda, oracle, n):
+    torch = torch_cuda
+    for dims in [(n, 8, 16), (8, n, 16), (16, 8, n)]:
+        g, vloc, kb, rng = problem(*dims, seed=n)
+        psi = rvec(rng, g, 3)
+        ctx = make_ctx(api, torch, g, vloc, kb, 3)
+        got = ctx.sgw_apply_H(torch.from_numpy(psi).cuda()).cpu().numpy()
+        want = oracle.apply_H(g, vloc, kb, psi, ld=True)
+        assert relerr(got, want) < TOL_H, dims
+        ctx.close()
+
+
+def test_apply_H_cfg0_shape_and_plane_wave(api, torch_cuda, oracle):
+    torch = torch_cuda
+    w = W.make_workload("cfg0")
+    g = w.grid
+    ctx = api.context_for(w)
+    psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, 4)
+    got = ctx.sgw_apply_H(psi).cpu().numpy()
+    want = oracle.apply_H(g, w.vloc, None, psi.cpu().numpy(), ld=True)
+    assert relerr(got, want) < TOL_H
+    # closed form without the oracle: V = c, plane wave (incl. Nyquist) is an eigenvector
+    ctx.sgw_set_vloc(torch.full(g.shape, 0.37, dtype=torch.float64, device="cuda"))
+    z, y, x = np.meshgrid(np.arange(32), np.arange(32), np.arange(32), indexing="ij")
+    for m in [(1, 0, 0), (-16, 5, 3), (7, -16, -16)]:
+        pw = np.exp(2j * np.pi * (m[0] * x + m[1] * y + m[2] * z) / 32)[None]
+        eig = 0.5 * (2 * np.pi / 16.0) ** 2 * (m[0] ** 2 + m[1] ** 2 + m[2] ** 2) + 0.37
+        got = ctx.sgw_apply_H(torch.from_numpy(pw).cuda()).cpu().numpy()
+        assert relerr(got, eig * pw) < 1e-12
+    ctx.close()
+
+
+def test_apply_H_sub_batching_and_no_potential(api, torch_cuda, oracle):
+    torch = torch_cuda
+    g, vloc, kb, rng = problem(24, 16, 12, seed=5)
+    psi = rvec(rng, g, 5)
+    ctx = make_ctx(api, torch, g, None, kb, 2)            # max_nvec 2 < nvec 5: ragged sub-batches
+    got = ctx.sgw_apply_H(torch.from_numpy(psi).cuda()).cpu().numpy()
+    want = oracle.apply_H(g, None, kb, psi, ld=True)
+    assert relerr(got, want) < TOL_H
+    ctx.close()
+
+
+# ------------------------------------------------------------------ Chebyshev filter
+def test_cheb_cfg0_full(api, torch_cuda, oracle):
+    """BASELINE.json configs[0] in full: 32^3, 4 vectors, 128 terms, against the long-double oracle."""
+    w = W.make_workload("cfg0")
+    ctx = api.context_for(w)
+    psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
+    ref_in = psi.cpu().numpy()
+    ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
+    want = oracle.cheb_filter(w.grid, w.vloc, None, ref_in, w.coeffs, w.emin, w.emax, ld=True)
+    assert relerr(psi.cpu().numpy(), want) < TOL_FULL
+    ctx.close()
+
+
+@pytest.mark.parametrize("nterms", [1, 2, 3, 4, 5, 6, 7, 33])
+def test_cheb_term_counts_with_kb_and_sub_batches(api, torch_cuda, oracle, nterms):
+    torch = torch_cuda
+    g, vloc, kb, rng = problem(16, 12, 24, seed=nterms)
+    emin, emax = W.spectral_bounds(g, vloc, True)
+    coeffs = rng.standard_normal(nterms)
+    psi = rvec(rng, g, 3)
+    ctx = make_ctx(api, torch, g, vloc, kb, 2)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+    want = oracle.cheb_filter(g, vloc, kb, psi, coeffs, emin, emax, ld=True)
+    assert relerr(t.cpu().numpy(), want) < TOL_FULL
+    ctx.close()
+
+
+def test_cheb_against_dense_diagonalisation(api, torch_cuda):
+    """No oracle: 8^3 grid, dense H from numpy.fft, eigh, polynomial of the eigenvalues."""
+    torch = torch_cuda
+    from test_oracle_physics import dense_H
+    g, vloc, kb, rng = problem(8, 8, 8, h=(0.7, 0.7, 0.7), seed=3)
+    H = dense_H(g, vloc, kb)
+    ev, U = np.linalg.eigh(H)
+    emin, emax = W.spectral_bounds(g, vloc, True)
+    coeffs = rng.standard_normal(40)
+    v = rvec(rng, g, 2)
+    x = (ev - 0.5 * (emax + emin)) / (0.5 * (emax - emin))
+    p = sum(coeffs[n] * np.cos(n * np.arccos(x)) for n in range(40))
+    want = ((U * p[None, :]) @ (U.conj().T @ v.reshape(2, -1).T)).T.reshape(v.shape)
+    ctx = make_ctx(api, torch, g, vloc, kb, 2)
+    t = torch.from_numpy(v).cuda()
+    ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+    assert relerr(t.cpu().numpy(), want) < 1e-11
+    ctx.close()
+
+
+# ------------------------------------------------------------------ Hartree
+def test_hartree_vs_oracle_and_erf(api, torch_cuda, oracle):
+    torch = torch_cuda
+    g, vloc, kb, rng = problem(24, 32, 16, kb=False, seed=9)
+    psi = rvec(rng, g, 3)
+    ctx = make_ctx(api, torch, g, None, None, 3)
+    vh, rho = ctx.sgw_hartree(torch.from_numpy(psi).cuda(), 0.37, want_rho=True)
+    want_vh, want_rho = oracle.hartree(g, psi, 0.37, ld=True)
+    assert np.abs(rho.cpu().numpy() - want_rho).max() < 1e-13 * np.abs(want_rho).max()
+    assert np.linalg.norm(vh.cpu().numpy() - want_vh) / np.linalg.norm(want_vh) < 1e-12
+    ctx.close()
+    # closed form: Gaussian charge -> Q erf(d / sqrt2 sigma) / d  (SURVEY 8(c) pin "Hartree")
+    from scipy.special import erf
+    n, h, sigma, Q = 48, 0.5, 1.0, 1.7
+    g = W.Grid(n, n, n, h, h, h)
+    c = np.array([12.13, 11.9, 12.31])
+    ax = np.arange(n) * h
+    z, y, x = np.meshgrid(ax, ax, ax, indexing="ij")
+    d = np.sqrt((x - c[0]) ** 2 + (y - c[1]) ** 2 + (z - c[2]) ** 2)
+    rho = Q * (2 * np.pi * sigma ** 2) ** -1.5 * np.exp(-d ** 2 / (2 * sigma ** 2))
+    ctx = make_ctx(api, torch, g, None, None, 1)
+    psi = torch.from_numpy(np.sqrt(rho).astype(np.complex128)[None]).cuda()
+    vh = ctx.sgw_hartree(psi, 1.0).cpu().numpy()
+    want = Q * erf(d / (np.sqrt(2) * sigma)) / d
+    m = d < n * h / 2 - 7 * sigma
+    assert (np.abs(vh - want)[m] / np.abs(want[m])).max() < 1e-10
+    ctx.close()
+
+
+# ------------------------------------------------------------------ TD propagation
+@pytest.mark.parametrize("mode,use_kb", [(0, False), (1, False), (0, True), (1, True)])
+def test_td_steps_vs_oracle(api, torch_cuda, oracle, mode, use_kb):
+    torch = torch_cuda
+    g, vloc, kb, rng = problem(16, 24, 12, kb=use_kb, seed=21)
+    psi = rvec(rng, g, 3)
+    rs = 2.0 / (3 * g.dV) * 0.01
+    ctx = make_ctx(api, torch, g, vloc, kb, 3)
+    ctx.sgw_set_td(mode, rs)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_td_propagate(t, 0.05, 12)
+    want = oracle.td_propagate(g, vloc, kb if use_kb else None, psi, 0.05, 12, mode, rs, ld=True)
+    assert relerr(t.cpu().numpy(), want) < TOL_FULL
+    if not use_kb:                                   # exactly unitary for local V (SURVEY 8(c) "TD")
+        n0 = np.sum(np.abs(psi.reshape(3, -1)) ** 2, axis=1)
+        n1 = ctx.sgw_norms(t).cpu().numpy()
+        assert np.abs(n1 / n0 - 1).max() < 1e-12
+    ctx.close()
+
+
+def test_td_reverse_and_plane_wave(api, torch_cuda):
+    torch = torch_cuda
+    g, vloc, kb, rng = problem(32, 16, 8, kb=False, seed=4)
+    psi = rvec(rng, g, 2)
+    ctx = make_ctx(api, torch, g, vloc, None, 2)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_td_propagate(t, 0.05, 5)
+    ctx.sgw_td_propagate(t, -0.05, 5)
+    assert relerr(t.cpu().numpy(), psi) < 1e-12
+    ctx.sgw_set_vloc(None)
+    z, y, x = np.meshgrid(np.arange(8), np.arange(16), np.arange(32), indexing="ij")
+    pw = np.exp(2j * np.pi * (3 * x / 32 - 2 * y / 16 + z / 8))[None]
+    eps = 0.5 * ((2 * np.pi * 3 / (32 * g.hx)) ** 2 + (2 * np.pi * 2 / (16 * g.hy)) ** 2 + (2 * np.pi / (8 * g.hz)) ** 2)
+    t = torch.from_numpy(pw).cuda()
+    ctx.sgw_td_propagate(t, 0.05, 7)
+    assert relerr(t.cpu().numpy(), np.exp(-1j * eps * 0.35) * pw) < 1e-12
+    ctx.close()
+
+
+# ------------------------------------------------------------------ helpers and errors
+def test_norms_and_error_codes(api, torch_cuda):
+    torch = torch_cuda
+    g = W.Grid(48, 16, 8, 0.5, 0.5, 0.5)
+    rng = np.random.default_rng(0)
+    psi = rvec(rng, g, 3)
+    ctx = api.Context(48, 16, 8, 0.5, 0.5, 0.5, 3)
+    n = ctx.sgw_norms(torch.from_numpy(psi).cuda()).cpu().numpy()
+    assert np.allclose(n, np.sum(np.abs(psi.reshape(3, -1)) ** 2, axis=1), rtol=1e-13)
+    t = torch.from_numpy(psi).cuda()
+    with pytest.raises(api.SGWError) as e:
+        ctx.lib.sgw_apply_H.restype = int
+        api._check(ctx.lib.sgw_apply_H(ctx._h, 3, api._ptr(t), api._ptr(t)))      # aliasing
+    assert e.value.code == -1
+    with pytest.raises(api.SGWError) as e:
+        api.Context(30, 16, 8, 0.5, 0.5, 0.5, 1)
+    assert e.value.code == -2
+    with pytest.raises(api.SGWError) as e:
+        ctx.sgw_cheb_filter(t, np.ones(4), 1.0, -1.0)
+    assert e.value.code == -1
+    assert ctx.sgw_launch_count() > 0
+    ctx.close()
