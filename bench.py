@@ -1,0 +1,270 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the sGW hot path on B200 (contract: see DESIGN.md "Measurement").
+
+A step = one pass of the whole hot path over one batch: the Chebyshev filter of BASELINE.json
+configs[1] (96^3 grid, Si35H36-shaped potential, 64 +-1 vectors, 512 terms = 511 H applications).
+value = grid-pt * vector * H-applies per second, inputs resident in HBM.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2601_21005_b200 import workloads as W  # noqa: E402
+
+METRIC = "grid-pt*vector H-applies/s (Chebyshev filter)"
+UNIT = "grid-pt*vec*H-applies/s"
+WORKLOAD = "cfg1"
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled during the timed region."""
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "200"], stdout=subprocess.PIPE, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.rows.append([x.strip() for x in ln.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample(w, nvec, napplies):
+    """Time the oracle (double, OpenMP over vectors) on nvec vectors x napplies H applications."""
+    from oracle import sgw_oracle as o
+    o.build()
+    threads = o.max_threads()
+    nvec = min(nvec, max(1, threads))
+    psi = o.random_vectors(w.grid, W.SEED_VEC, 0, nvec)
+    coeffs = np.ascontiguousarray(w.coeffs[:napplies + 1])
+    t0 = time.perf_counter()
+    o.cheb_filter(w.grid, w.vloc, w.kb, psi, coeffs, w.emin, w.emax, ld=False)
+    dt = time.perf_counter() - t0
+    units = w.grid.ng * nvec * napplies
+    return units / dt, dt, nvec, min(threads, nvec)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = W.make_workload(WORKLOAD)
+    cores = os.cpu_count() or 1
+    nv, nap = min(w.nvec, cores), 4
+    for _ in range(args.warmup):
+        oracle_sample(w, nv, 1)
+    tot_units, tot_t, used = 0.0, 0.0, 1
+    for _ in range(args.steps):
+        v, dt, nvec, used = oracle_sample(w, nv, nap)
+        tot_units += v * dt
+        tot_t += dt
+    val = tot_units / tot_t
+    sample = f"{nv} vectors x {nap} H applies of the {w.nterms}-term filter per step, {WORKLOAD} grid and potential"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{WORKLOAD}: 96^3 grid h=0.45, {w.atoms}-shaped V_loc, 512-term sqrt-Fermi-Dirac filter",
+                   "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2601_21005_b200 import api
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = W.make_workload(WORKLOAD)
+    g = w.grid
+    nvec, napply = w.nvec, w.nterms - 1
+    units_rank = g.ng * nvec * napply
+    stream = torch.cuda.current_stream(dev)
+    ctx = api.context_for(w, max_nvec=nvec, stream=stream, device=f"cuda:{local}")
+    psi0 = ctx.sgw_random_vectors(W.SEED_VEC, rank * nvec, nvec)     # each rank filters its own vectors
+    psi = torch.empty_like(psi0)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def step():
+        psi.copy_(psi0)
+        ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ctx.sgw_profile_reset()
+    ctx.sgw_profile_enable(1)
+    l0 = ctx.sgw_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = ctx.sgw_launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    prof = {(a, k): ctx.sgw_profile_get(a, k) for a in range(3) for k in range(8)}
+    ctx.sgw_profile_enable(0)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = units_rank * world * args.steps / (ms * 1e-3)
+
+    # ---- end to end: host buffers, H2D of the inputs and D2H of the result inside the timed region
+    h_in = psi0.cpu().pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    nbytes = h_in.numel() * 16
+
+    def step_e2e():
+        psi.copy_(h_in, non_blocking=True)
+        ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
+        h_out.copy_(psi, non_blocking=True)
+
+    step_e2e()
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step_e2e()
+    e1.record(stream)
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    e2e_value = units_rank * world * args.steps / (ms_e2e * 1e-3)
+    checksum = float(torch.view_as_real(h_out).abs().sum())
+
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        names = {0: "x", 1: "y", 2: "z"}
+        kinds = ["store", "acc", "hfin", "cheb", "td", "mul3d", "fwd", "inv"]
+        passes = {f"{names[a]}_{kinds[k]}": {"launches": n, "ms_total": t_} for (a, k), (n, t_) in prof.items() if n}
+        dom = max(passes.items(), key=lambda kv: kv[1]["ms_total"])
+        # algorithmic bytes per grid-pt*vector of each pass: complex = 16 B
+        series_share = 32.0 / 3.0                                   # series r/w every third term
+        bytes_per_unit = {"x_store": 32.0, "y_acc": 48.0, "z_cheb": 64.0 + series_share + 8.0 / nvec}
+        dn, dv = dom
+        units_launch = g.ng * nvec
+        avg_ms = dv["ms_total"] / dv["launches"]
+        ach = bytes_per_unit.get(dn, 32.0) * units_launch / (avg_ms * 1e-3) / 1e9
+        strict_bytes = 80.0 + 8.0 / nvec                            # compulsory bytes per term
+        term_gbs = strict_bytes * units_rank * args.steps / (ms * 1e-3) / 1e9
+        moved = sum(bytes_per_unit.get(k_, 32.0) * units_launch * v_["launches"] for k_, v_ in passes.items())
+        cpu_val, cpu_dt, cpu_nv, cpu_cores = oracle_sample(w, os.cpu_count() or 1, 16)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{WORKLOAD}: 96^3 grid h=0.45, {w.atoms}-shaped V_loc, {nvec} +-1 vectors per GPU, "
+                                   f"{w.nterms}-term sqrt-Fermi-Dirac Chebyshev filter ({napply} H applies)",
+                       "l2": "inputs larger than L2 (each array 906 MB per GPU)", "passes_per_term": 3},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                    "ms_per_step": ms_e2e / args.steps, "checksum": checksum},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "kernel": f"pass_kernel<96,RT,{dn}>", "achieved": ach, "peak": peak,
+                         "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                         "avg_launch_ms": avg_ms, "bytes_per_unit": bytes_per_unit.get(dn, 32.0),
+                         "kernel_share_of_step": dv["ms_total"] / ms,
+                         "term_strict": {"bytes_per_unit": strict_bytes, "achieved": term_gbs, "frac": term_gbs / peak},
+                         "term_moved": {"achieved": moved / (ms * 1e-3) / 1e9, "frac": moved / (ms * 1e-3) / 1e9 / peak},
+                         "passes": passes},
+            "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",
+                             "sample": f"{cpu_nv} vectors x 16 H applies of the same filter, {WORKLOAD} grid ({cpu_dt:.1f} s)"},
+        }
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="sgw", choices=["sgw", "reference"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -107,6 +107,16 @@ int sgw_norms(sgw_ctx* ctx, int nvec, const void* d_psi, double* d_out);
  * gpu_launches).  Host counter; never fails (returns 0 for NULL). */
 int64_t sgw_launch_count(const sgw_ctx* ctx);
 
+/* Per-pass device timing for measurement (bench.py's roofline): while enabled, every FFT pass launch
+ * is bracketed by a pair of CUDA events on the context's stream (at most 60000 launches between
+ * collections).  sgw_profile_get synchronises the stream and returns, for passes along `axis`
+ * (0 x, 1 y, 2 z) of `kind` (0 store, 1 accumulate, 2 H-final, 3 Chebyshev, 4 TD, 5 Poisson kernel,
+ * 6 forward, 7 inverse), the number of launches timed and their summed duration in ms since the
+ * last sgw_profile_reset. */
+int sgw_profile_enable(sgw_ctx* ctx, int on);
+int sgw_profile_reset(sgw_ctx* ctx);
+int sgw_profile_get(sgw_ctx* ctx, int axis, int kind, int64_t* count, double* total_ms);
+
 /* Message for the last error on the calling thread ("" if none). */
 const char* sgw_last_error(void);
 

@@ -19,7 +19,7 @@ _lib = None
 ERRORS = {-1: "SGW_EINVAL", -2: "SGW_ESIZE", -3: "SGW_ENOMEM", -4: "SGW_ECUDA"}
 EXPORTS = ["sgw_init_grid", "sgw_destroy", "sgw_set_vloc", "sgw_set_nonlocal", "sgw_random_vectors",
            "sgw_apply_H", "sgw_cheb_filter", "sgw_hartree", "sgw_set_td", "sgw_td_propagate", "sgw_norms",
-           "sgw_launch_count", "sgw_last_error"]
+           "sgw_launch_count", "sgw_last_error", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get"]
 
 
 class SGWError(RuntimeError):
@@ -50,6 +50,9 @@ def load():
         lib.sgw_launch_count.argtypes = [vp]
         lib.sgw_launch_count.restype = i64
         lib.sgw_last_error.restype = C.c_char_p
+        lib.sgw_profile_enable.argtypes = [vp, i]
+        lib.sgw_profile_reset.argtypes = [vp]
+        lib.sgw_profile_get.argtypes = [vp, i, i, C.POINTER(i64), C.POINTER(d)]
         _lib = lib
     return _lib
 
@@ -158,6 +161,17 @@ class Context:
         out = torch.empty(nvec, dtype=torch.float64, device=self.device)
         _check(self.lib.sgw_norms(self._h, nvec, _ptr(psi), _ptr(out)))
         return out
+
+    def sgw_profile_enable(self, on):
+        _check(self.lib.sgw_profile_enable(self._h, int(on)))
+
+    def sgw_profile_reset(self):
+        _check(self.lib.sgw_profile_reset(self._h))
+
+    def sgw_profile_get(self, axis, kind):
+        n, ms = C.c_int64(), C.c_double()
+        _check(self.lib.sgw_profile_get(self._h, axis, kind, C.byref(n), C.byref(ms)))
+        return n.value, ms.value
 
     def sgw_launch_count(self):
         return int(self.lib.sgw_launch_count(self._h))

@@ -64,10 +64,37 @@ int run_pass(sgw_ctx* c, int axis, int kind, int nvec, const cd* in, const OpPar
     call.stream = c->stream;
     if (call.ntiles <= 0) return 0;
     if (call.ntiles > 0x7fffffffLL) return set_error(SGW_EINVAL, "too many tiles for one launch");
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (c->prof_on && c->prof_used < 60000) {
+        if (c->prof_ev.size() < 2 * (c->prof_used + 1)) {
+            cudaEvent_t a, b;
+            if (cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) {
+                c->prof_ev.push_back(a); c->prof_ev.push_back(b); c->prof_tag.push_back(0);
+            }
+        }
+        if (c->prof_ev.size() >= 2 * (c->prof_used + 1)) {
+            e0 = c->prof_ev[2 * c->prof_used]; e1 = c->prof_ev[2 * c->prof_used + 1];
+            c->prof_tag[c->prof_used] = axis * K_NKINDS + kind;
+            cudaEventRecord(e0, c->stream);
+        }
+    }
     int rc = c->pass[axis](&call);
     if (rc != 0) return set_error(rc, std::string("pass launch failed: ") + cudaGetErrorString(cudaGetLastError()));
+    if (e1) { cudaEventRecord(e1, c->stream); c->prof_used++; }
     c->launches++;
     return 0;
+}
+
+static void prof_collect(sgw_ctx* c) {
+    cudaStreamSynchronize(c->stream);
+    for (size_t i = 0; i < c->prof_used; ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]) == cudaSuccess) {
+            c->prof_ms[c->prof_tag[i]] += ms;
+            c->prof_n[c->prof_tag[i]]++;
+        }
+    }
+    c->prof_used = 0;
 }
 
 template <class T>
@@ -105,9 +132,33 @@ extern "C" const char* sgw_last_error(void) { return g_err.c_str(); }
 
 extern "C" int64_t sgw_launch_count(const sgw_ctx* c) { return c ? c->launches : 0; }
 
+extern "C" int sgw_profile_enable(sgw_ctx* c, int on) {
+    if (!c) return set_error(SGW_EINVAL, "sgw_profile_enable: null context");
+    if (c->prof_on) sgw::prof_collect(c);
+    c->prof_on = on != 0;
+    return SGW_OK;
+}
+
+extern "C" int sgw_profile_reset(sgw_ctx* c) {
+    if (!c) return set_error(SGW_EINVAL, "sgw_profile_reset: null context");
+    sgw::prof_collect(c);
+    for (int i = 0; i < 3 * K_NKINDS; ++i) { c->prof_ms[i] = 0; c->prof_n[i] = 0; }
+    return SGW_OK;
+}
+
+extern "C" int sgw_profile_get(sgw_ctx* c, int axis, int kind, int64_t* count, double* total_ms) {
+    if (!c || axis < 0 || axis > 2 || kind < 0 || kind >= K_NKINDS || !count || !total_ms)
+        return set_error(SGW_EINVAL, "sgw_profile_get: bad argument");
+    sgw::prof_collect(c);
+    *count = c->prof_n[axis * K_NKINDS + kind];
+    *total_ms = c->prof_ms[axis * K_NKINDS + kind];
+    return SGW_OK;
+}
+
 extern "C" int sgw_destroy(sgw_ctx* c) {
     if (!c) return SGW_OK;
     cudaStreamSynchronize(c->stream);
+    for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
     for (int a = 0; a < 3; ++a) {
         cudaFree(c->tw[a]); cudaFree(c->kin[a]); cudaFree(c->cheb_kin[a]); cudaFree(c->td_kin[a]); cudaFree(c->ws[a]);
     }
@@ -169,6 +220,8 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     c->kbc = nullptr; c->kbc_cap = 0;
     c->pois = nullptr; c->rho = nullptr; c->vh = nullptr; c->phase = nullptr;
     c->hartree_mode = 0; c->rho_scale = 0; c->launches = 0;
+    c->prof_on = false; c->prof_used = 0;
+    for (int i = 0; i < 3 * K_NKINDS; ++i) { c->prof_ms[i] = 0; c->prof_n[i] = 0; }
     if (!rc) rc = dev_alloc(&c->vtab, c->ng);
     if (!rc) rc = dev_alloc(&c->vk3d, c->ng);
     if (!rc) rc = dev_alloc(&c->pois, c->ng);

@@ -47,6 +47,13 @@ struct sgw_ctx {
     int hartree_mode;
     double rho_scale;
     int64_t launches;
+    // optional per-pass device timing (sgw_profile_*): event pairs around pass launches
+    bool prof_on;
+    std::vector<cudaEvent_t> prof_ev;        // 2 per recorded launch
+    std::vector<int> prof_tag;               // axis * K_NKINDS + kind
+    size_t prof_used;                        // pairs recorded since the last collect
+    double prof_ms[3 * sgw::K_NKINDS];
+    long long prof_n[3 * sgw::K_NKINDS];
 };
 
 namespace sgw {
