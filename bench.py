@@ -139,7 +139,7 @@ def run_gpu(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    w = W.make_workload(WORKLOAD)
+    w = W.make_workload(WORKLOAD, nterms=args.nterms)
     g = w.grid
     nvec, napply = w.nvec, w.nterms - 1
     units_rank = g.ng * nvec * napply
@@ -259,6 +259,8 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="sgw", choices=["sgw", "reference"])
+    ap.add_argument("--nterms", type=int, default=None,
+                    help="shorten the filter (profiling runs under ncu only; the default is the config's 512)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

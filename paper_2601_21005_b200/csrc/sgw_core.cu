@@ -1,6 +1,7 @@
 // sgw_core.cu -- context, tables, pass geometry, setup entry points of libsgw (include/sgw.h).
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "sgw_ctx.h"
@@ -40,15 +41,15 @@ PassGeom geom_for_axis(const sgw_ctx* c, int axis, int nvec, long long* ntiles) 
     const long long nxy = (long long)c->nx * c->ny;
     if (axis == 0) {                 // contiguous pencils: tile = Bx consecutive rows
         g.fastn = 1; g.B = c->Bx; g.sN = 1; g.sB = c->nx;
-        *ntiles = (long long)c->ny * c->nz * nvec / c->Bx;
-        g.TI = 0x7fffffff; g.SI = (long long)c->Bx * c->nx; g.SO = 0;
+        g.TI = (int)((long long)c->ny * c->nz / c->Bx); g.SI = (long long)c->Bx * c->nx; g.SO = c->ng; g.GO = 1;
+        *ntiles = (long long)g.TI * nvec;
     } else if (axis == 1) {          // tile = B consecutive x at fixed (z, vec)
         g.fastn = 0; g.B = c->B; g.sN = c->nx; g.sB = 1;
-        g.TI = c->nx / c->B; g.SI = c->B; g.SO = nxy;
+        g.TI = c->nx / c->B; g.SI = c->B; g.SO = nxy; g.GO = c->nz;
         *ntiles = (long long)g.TI * c->nz * nvec;
     } else {                         // tile = B consecutive xy points at fixed vec
         g.fastn = 0; g.B = c->B; g.sN = nxy; g.sB = 1;
-        g.TI = (int)(nxy / c->B); g.SI = c->B; g.SO = c->ng;
+        g.TI = (int)(nxy / c->B); g.SI = c->B; g.SO = c->ng; g.GO = 1;
         *ntiles = (long long)g.TI * nvec;
     }
     return g;
@@ -221,6 +222,7 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     c->pois = nullptr; c->rho = nullptr; c->vh = nullptr; c->phase = nullptr;
     c->hartree_mode = 0; c->rho_scale = 0; c->launches = 0;
     c->prof_on = false; c->prof_used = 0;
+    { const char* e = getenv("SGW_L2_CHUNK"); c->l2_chunk = e ? atoi(e) : 0; }
     for (int i = 0; i < 3 * K_NKINDS; ++i) { c->prof_ms[i] = 0; c->prof_n[i] = 0; }
     if (!rc) rc = dev_alloc(&c->vtab, c->ng);
     if (!rc) rc = dev_alloc(&c->vk3d, c->ng);

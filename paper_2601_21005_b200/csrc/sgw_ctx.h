@@ -47,6 +47,7 @@ struct sgw_ctx {
     int hartree_mode;
     double rho_scale;
     int64_t launches;
+    int l2_chunk;                            // vectors per L2-resident chunk (0 = whole batch)
     // optional per-pass device timing (sgw_profile_*): event pairs around pass launches
     bool prof_on;
     std::vector<cudaEvent_t> prof_ev;        // 2 per recorded launch

@@ -135,9 +135,10 @@ SGW_FACT(384, 24, 16)
 // Geometry of one pass: which pencils a CTA owns and how they sit in memory.
 //   tile t -> base = (t / TI) * SO + (t % TI) * SI;   element (n, b) at base + n*sN + b*sB
 //   fastn != 0: the transform axis is the contiguous one (x); lanes run along n for coalescing.
+//   grid index of the tile's first element: g0 = ((t / TI) % GO) * SO + (t % TI) * SI
 struct PassGeom {
     long long SO, SI, sN, sB, ng;
-    int TI, B, fastn;
+    int TI, GO, B, fastn;
 };
 
 enum { MODE_RT = 0, MODE_FWD = 1, MODE_INV = 2 };

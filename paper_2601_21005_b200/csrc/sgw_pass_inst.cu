@@ -1,6 +1,8 @@
 // sgw_pass_inst.cu -- compiled once per supported axis length (-DSGW_N=<N>): instantiates every
 // fused pass kernel for that length and exports one launcher, sgw_pass_launch_<N>.
-#include "sgw_ops.cuh"
+#include <cstdlib>
+
+#include "sgw_pipe.cuh"
 
 #ifndef SGW_N
 #error "compile with -DSGW_N=<axis length>"
@@ -29,6 +31,78 @@ static int launch(const PassCall* c) {
     return cudaGetLastError() == cudaSuccess ? 0 : -4;
 }
 
+// Pipelined persistent variant.  Returns 1 if it does not apply (caller falls back to launch<>).
+template <int B, bool FASTN, class Op>
+static int launch_pipe_b(const PassCall* c, int num_sms) {
+    constexpr int N = SGW_N;
+    using Cfg = PipeCfg<N, B>;
+    const OpParams& p = c->p;
+    PipeArgs pa;
+    const void* ptrs[NSLOT] = {c->in, nullptr, nullptr, nullptr, nullptr};
+    int esz[NSLOT] = {16, 16, 16, 16, 16}, grid[NSLOT] = {0, 0, 0, 0, 1};
+    switch (c->kind) {
+        case K_RT_STORE: break;
+        case K_RT_ACC: ptrs[SLOT_ACC] = p.acc; break;
+        case K_RT_HFIN: ptrs[SLOT_ACC] = p.acc; ptrs[SLOT_TAB] = p.vtab; esz[SLOT_TAB] = 8; break;
+        case K_RT_CHEB:
+            ptrs[SLOT_ACC] = p.acc; ptrs[SLOT_TAB] = p.vtab; esz[SLOT_TAB] = 8;
+            if (p.use_prev) ptrs[SLOT_PREV] = p.prev;
+            if (p.flush && !p.series_init) ptrs[SLOT_SERIES] = p.series;
+            break;
+        case K_RT_TD: ptrs[SLOT_TAB] = p.pro_phase ? p.pro_phase : p.epi_phase; break;
+        default: return 1;
+    }
+    if (c->kind == K_RT_TD && p.pro_phase && p.epi_phase && p.pro_phase != p.epi_phase) return 1;
+    int off = 0;
+    for (int s = 0; s < NSLOT; ++s) {
+        pa.src[s].ptr = (const char*)ptrs[s];
+        pa.src[s].esz = esz[s];
+        pa.src[s].grid = grid[s];
+        pa.src[s].slot_off = off;
+        if (ptrs[s]) off += B * N * esz[s];
+    }
+    pa.stage_bytes = off;
+    pa.ntiles = (unsigned)c->ntiles;
+    const size_t smem = (size_t)Cfg::FIXED_BYTES + 2 * (size_t)pa.stage_bytes;
+    if (smem > 227 * 1024 || Cfg::T > 1024) return 1;
+    if ((long long)N * c->gm.sN + (long long)B * c->gm.sB >= (1LL << 31)) return 1;
+    auto kern = pipe_kernel<N, B, FASTN, Op>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -4;
+        attr_done = true;
+    }
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::T, smem) != cudaSuccess || per_sm < 1) return 1;
+    long long grid_x = (long long)per_sm * num_sms;
+    if (grid_x > c->ntiles) grid_x = c->ntiles;
+    Op op;
+    op.p = c->p;
+    kern<<<(unsigned)grid_x, Cfg::T, smem, c->stream>>>(c->gm, pa, c->tw, op);
+    return cudaGetLastError() == cudaSuccess ? 0 : -4;
+}
+
+template <class Op>
+static int launch_pipe(const PassCall* c) {
+    static int disabled = -1, num_sms = 0;
+    if (disabled < 0) {
+        const char* e = getenv("SGW_NOPIPE");
+        disabled = (e && atoi(e)) ? 1 : 0;
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    if (disabled || c->gm.B != 8) return 1;
+    return c->gm.fastn ? launch_pipe_b<8, true, Op>(c, num_sms) : launch_pipe_b<8, false, Op>(c, num_sms);
+}
+
+template <class POp, class Op>
+static int launch_rt(const PassCall* c) {
+    const int rc = launch_pipe<POp>(c);
+    if (rc != 1) return rc;
+    return launch<MODE_RT, Op>(c);
+}
+
 }  // namespace sgw
 
 #define SGW_CAT_(a, b) a##b
@@ -37,11 +111,11 @@ static int launch(const PassCall* c) {
 extern "C" int SGW_CAT(sgw_pass_launch_, SGW_N)(const sgw::PassCall* c) {
     using namespace sgw;
     switch (c->kind) {
-        case K_RT_STORE: return launch<MODE_RT, OpStore>(c);
-        case K_RT_ACC: return launch<MODE_RT, OpAcc>(c);
-        case K_RT_HFIN: return launch<MODE_RT, OpHFin>(c);
-        case K_RT_CHEB: return launch<MODE_RT, OpCheb>(c);
-        case K_RT_TD: return launch<MODE_RT, OpTD>(c);
+        case K_RT_STORE: return launch_rt<POpStore, OpStore>(c);
+        case K_RT_ACC: return launch_rt<POpAcc, OpAcc>(c);
+        case K_RT_HFIN: return launch_rt<POpHFin, OpHFin>(c);
+        case K_RT_CHEB: return launch_rt<POpCheb, OpCheb>(c);
+        case K_RT_TD: return launch_rt<POpTD, OpTD>(c);
         case K_RT_MUL3D: return launch<MODE_RT, OpMul3D>(c);
         case K_FWD: return launch<MODE_FWD, OpStore>(c);
         case K_INV: return launch<MODE_INV, OpStore>(c);

@@ -173,22 +173,27 @@ extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* 
         bool pend_m2 = false, pend_m1 = true;  // before n = 1: degree 0 (= n-1) is pending
         bool series_started = false;
         for (int n = 1; n < nterms; ++n) {
-            OpParams p = zero_params();
-            p.out = W; p.mul_re = c->cheb_kin[0];
-            SGW_TRY(run_pass(c, 0, K_RT_STORE, nv, cur, p));
-            p.mul_re = c->cheb_kin[1]; p.acc = W;
-            SGW_TRY(run_pass(c, 1, K_RT_ACC, nv, cur, p));
-            SGW_TRY(kb_apply(c, nv, cur, W, 0, s));
-            p.mul_re = c->cheb_kin[2]; p.vtab = c->vtab;
-            p.out = other; p.prev = other; p.use_prev = (n >= 2);
-            p.hs = (n == 1) ? 0.5 : 1.0;
             const bool last = (n == nterms - 1);
             const bool flush = last || pend_m2;
-            p.flush = flush; p.series = O; p.series_init = !series_started;
-            p.c0 = pend_m2 ? h_coeffs[n - 2] : 0.0;
-            p.c1 = pend_m1 ? h_coeffs[n - 1] : 0.0;
-            p.c2 = h_coeffs[n];
-            SGW_TRY(run_pass(c, 2, K_RT_CHEB, nv, cur, p));
+            const int chunk = (c->l2_chunk > 0 && c->l2_chunk < nv) ? c->l2_chunk : nv;
+            for (int cv = 0; cv < nv; cv += chunk) {          // vector chunks sized so that W stays L2-resident
+                const int nc = (nv - cv < chunk) ? nv - cv : chunk;
+                const long long co = (long long)cv * ng;
+                OpParams p = zero_params();
+                p.out = W; p.mul_re = c->cheb_kin[0];
+                SGW_TRY(run_pass(c, 0, K_RT_STORE, nc, cur + co, p));
+                p.mul_re = c->cheb_kin[1]; p.acc = W;
+                SGW_TRY(run_pass(c, 1, K_RT_ACC, nc, cur + co, p));
+                SGW_TRY(kb_apply(c, nc, cur + co, W, 0, s));
+                p.mul_re = c->cheb_kin[2]; p.vtab = c->vtab;
+                p.out = other + co; p.prev = other + co; p.use_prev = (n >= 2);
+                p.hs = (n == 1) ? 0.5 : 1.0;
+                p.flush = flush; p.series = O + co; p.series_init = !series_started;
+                p.c0 = pend_m2 ? h_coeffs[n - 2] : 0.0;
+                p.c1 = pend_m1 ? h_coeffs[n - 1] : 0.0;
+                p.c2 = h_coeffs[n];
+                SGW_TRY(run_pass(c, 2, K_RT_CHEB, nc, cur + co, p));
+            }
             if (flush) { series_started = true; pend_m2 = false; pend_m1 = false; }
             else { pend_m2 = pend_m1; pend_m1 = true; }
             cd* t = cur; cur = other; other = t;
@@ -224,28 +229,33 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, vh, 0.5 * dt, c->phase, ng);
             SGW_TRY(launched(c, "phase"));
         }
-        OpParams p = zero_params();
-        p.out = psi;
-        if (kb) {
-            dim3 g2(blocks_for(ng, 256), nvec);
-            apply_phase_kernel<<<g2, 256, 0, c->stream>>>(psi, c->phase, ng);
-            SGW_TRY(launched(c, "apply_phase"));
-            SGW_TRY(kb_apply(c, nvec, psi, psi, 1, 0.5 * dt));
-        } else {
-            p.pro_phase = c->phase;
-        }
-        p.mul_c = c->td_kin[0];
-        SGW_TRY(run_pass(c, 0, K_RT_TD, nvec, psi, p));
-        p.pro_phase = nullptr; p.mul_c = c->td_kin[1];
-        SGW_TRY(run_pass(c, 1, K_RT_TD, nvec, psi, p));
-        p.mul_c = c->td_kin[2];
-        if (!kb) p.epi_phase = c->phase;
-        SGW_TRY(run_pass(c, 2, K_RT_TD, nvec, psi, p));
-        if (kb) {
-            SGW_TRY(kb_apply(c, nvec, psi, psi, 1, 0.5 * dt));
-            dim3 g2(blocks_for(ng, 256), nvec);
-            apply_phase_kernel<<<g2, 256, 0, c->stream>>>(psi, c->phase, ng);
-            SGW_TRY(launched(c, "apply_phase"));
+        const int chunk = (!kb && c->l2_chunk > 0 && c->l2_chunk < nvec) ? c->l2_chunk : nvec;
+        for (int cv = 0; cv < nvec; cv += chunk) {            // chunks small enough to stay in L2 across the 3 passes
+            const int nc = (nvec - cv < chunk) ? nvec - cv : chunk;
+            cd* ps = psi + (long long)cv * ng;
+            OpParams p = zero_params();
+            p.out = ps;
+            if (kb) {
+                dim3 g2(blocks_for(ng, 256), nc);
+                apply_phase_kernel<<<g2, 256, 0, c->stream>>>(ps, c->phase, ng);
+                SGW_TRY(launched(c, "apply_phase"));
+                SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt));
+            } else {
+                p.pro_phase = c->phase;
+            }
+            p.mul_c = c->td_kin[0];
+            SGW_TRY(run_pass(c, 0, K_RT_TD, nc, ps, p));
+            p.pro_phase = nullptr; p.mul_c = c->td_kin[1];
+            SGW_TRY(run_pass(c, 1, K_RT_TD, nc, ps, p));
+            p.mul_c = c->td_kin[2];
+            if (!kb) p.epi_phase = c->phase;
+            SGW_TRY(run_pass(c, 2, K_RT_TD, nc, ps, p));
+            if (kb) {
+                SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt));
+                dim3 g2(blocks_for(ng, 256), nc);
+                apply_phase_kernel<<<g2, 256, 0, c->stream>>>(ps, c->phase, ng);
+                SGW_TRY(launched(c, "apply_phase"));
+            }
         }
     }
     return SGW_OK;
