@@ -6,7 +6,9 @@
 
 #include "sgw_ctx.h"
 
-#define SGW_DECL(N) extern "C" int sgw_pass_launch_##N(const sgw::PassCall*);
+#define SGW_DECL(N)                                             \
+    extern "C" int sgw_pass_launch_##N(const sgw::PassCall*);   \
+    extern "C" int sgw_plane_launch_##N(const sgw::PlaneCall*);
 SGW_DECL(8) SGW_DECL(12) SGW_DECL(16) SGW_DECL(24) SGW_DECL(32) SGW_DECL(48) SGW_DECL(64) SGW_DECL(96)
 SGW_DECL(128) SGW_DECL(192) SGW_DECL(256) SGW_DECL(384)
 #undef SGW_DECL
@@ -33,6 +35,52 @@ static pass_launch_fn launcher_for(int n) {
 #undef SGW_CASE
         default: return nullptr;
     }
+}
+
+static plane_launch_fn plane_launcher_for(int n) {
+    switch (n) {
+#define SGW_CASE(N) case N: return sgw_plane_launch_##N;
+        SGW_CASE(8) SGW_CASE(12) SGW_CASE(16) SGW_CASE(24) SGW_CASE(32) SGW_CASE(48) SGW_CASE(64) SGW_CASE(96)
+        SGW_CASE(128) SGW_CASE(192) SGW_CASE(256) SGW_CASE(384)
+#undef SGW_CASE
+        default: return nullptr;
+    }
+}
+
+int run_plane(sgw_ctx* c, int mode, int nvec, const cd* in, cd* out, const cd* phase, bool cheb_tables) {
+    if (!c->plane || nvec <= 0) return 1;
+    PlaneCall call;
+    call.mode = mode;
+    call.a.in = in; call.a.out = out; call.a.phase = phase;
+    call.a.kre_x = cheb_tables ? c->cheb_kin[0] : c->kin[0];
+    call.a.kre_y = cheb_tables ? c->cheb_kin[1] : c->kin[1];
+    call.a.kc_x = c->td_kin[0]; call.a.kc_y = c->td_kin[1];
+    call.a.nplanes = (unsigned)((long long)c->nz * nvec);
+    call.a.nz = (unsigned)c->nz;
+    call.a.G = c->plane_G;
+    call.tw = c->tw[0];
+    call.ctas_per_sm = c->plane_ctas;
+    call.stream = c->stream;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (c->prof_on && c->prof_used < 60000) {
+        if (c->prof_ev.size() < 2 * (c->prof_used + 1)) {
+            cudaEvent_t a, b;
+            if (cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) {
+                c->prof_ev.push_back(a); c->prof_ev.push_back(b); c->prof_tag.push_back(0);
+            }
+        }
+        if (c->prof_ev.size() >= 2 * (c->prof_used + 1)) {
+            e0 = c->prof_ev[2 * c->prof_used]; e1 = c->prof_ev[2 * c->prof_used + 1];
+            c->prof_tag[c->prof_used] = 1 * K_NKINDS + (mode == PL_TD ? K_RT_TD : K_RT_ACC);   // booked as the y pass
+            cudaEventRecord(e0, c->stream);
+        }
+    }
+    const int rc = c->plane(&call);
+    if (rc == 1) return 1;
+    if (rc != 0) return set_error(rc, std::string("plane launch failed: ") + cudaGetErrorString(cudaGetLastError()));
+    if (e1) { cudaEventRecord(e1, c->stream); c->prof_used++; }
+    c->launches++;
+    return 0;
 }
 
 PassGeom geom_for_axis(const sgw_ctx* c, int axis, int nvec, long long* ntiles) {
@@ -223,6 +271,10 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     c->hartree_mode = 0; c->rho_scale = 0; c->launches = 0;
     c->prof_on = false; c->prof_used = 0;
     { const char* e = getenv("SGW_L2_CHUNK"); c->l2_chunk = e ? atoi(e) : 0; }
+    c->plane = nullptr; c->plane_G = 2; c->plane_ctas = 0;
+    if (nx == ny && nx % 8 == 0 && !(getenv("SGW_NOPLANE") && atoi(getenv("SGW_NOPLANE")))) c->plane = plane_launcher_for(nx);
+    { const char* e = getenv("SGW_PLANE_G"); if (e && atoi(e) > 0) c->plane_G = atoi(e); }
+    { const char* e = getenv("SGW_PLANE_CTAS"); if (e) c->plane_ctas = atoi(e); }
     for (int i = 0; i < 3 * K_NKINDS; ++i) { c->prof_ms[i] = 0; c->prof_n[i] = 0; }
     if (!rc) rc = dev_alloc(&c->vtab, c->ng);
     if (!rc) rc = dev_alloc(&c->vk3d, c->ng);

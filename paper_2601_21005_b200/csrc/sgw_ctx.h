@@ -7,7 +7,7 @@
 #include <vector>
 
 #include "../../include/sgw.h"
-#include "sgw_ops.cuh"
+#include "sgw_plane.cuh"
 
 struct sgw_ctx {
     int nx, ny, nz;
@@ -18,6 +18,8 @@ struct sgw_ctx {
     int B;                                   // pencils per CTA on the strided axes (y, z)
     int Bx;                                  // pencils per CTA on the contiguous axis (x)
     sgw::pass_launch_fn pass[3];             // per-axis launcher (x, y, z)
+    sgw::plane_launch_fn plane;              // fused xy-plane launcher (nx == ny) or NULL
+    int plane_G, plane_ctas;                 // planes per group, CTAs per SM (0 = auto)
     int dims[3];
     double hs[3];
     sgw::cd* tw[3];                          // exp(-2 pi i j/N) per axis
@@ -62,4 +64,6 @@ int set_error(int code, const std::string& msg);
 int check_cuda(cudaError_t e, const char* what);
 PassGeom geom_for_axis(const sgw_ctx* c, int axis, int nvec, long long* ntiles);
 int run_pass(sgw_ctx* c, int axis, int kind, int nvec, const cd* in, const OpParams& p);
+// fused x+y pass; returns 1 when unavailable for this grid (caller runs the two passes instead)
+int run_plane(sgw_ctx* c, int mode, int nvec, const cd* in, cd* out, const cd* phase, bool cheb_tables);
 }  // namespace sgw

@@ -2,7 +2,7 @@
 // fused pass kernel for that length and exports one launcher, sgw_pass_launch_<N>.
 #include <cstdlib>
 
-#include "sgw_pipe.cuh"
+#include "sgw_plane.cuh"
 
 #ifndef SGW_N
 #error "compile with -DSGW_N=<axis length>"
@@ -103,6 +103,40 @@ static int launch_rt(const PassCall* c) {
     return launch<MODE_RT, Op>(c);
 }
 
+// rows/columns per plane tile: wide tiles keep one CTA (8-9 warps) on few planes so the x->y
+// transpose stays L2-resident
+constexpr int plane_B(int n) {
+    return n == 32 ? 32 : n == 48 ? 24 : n == 64 ? 32 : n == 96 ? 24 : n == 128 ? 16 : 8;
+}
+
+template <int MODE>
+static int launch_plane(const PlaneCall* c) {
+    constexpr int N = SGW_N, B = plane_B(SGW_N);
+    using Cfg = PlaneCfg<N, B>;
+    static int num_sms = 0;
+    if (!num_sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    if (Cfg::SMEM_BYTES > 227 * 1024 || N % B) return 1;
+    auto kern = plane_kernel<N, B, MODE>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -4;
+        attr_done = true;
+    }
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::T, Cfg::SMEM_BYTES) != cudaSuccess || per_sm < 1)
+        return 1;
+    if (c->ctas_per_sm > 0 && c->ctas_per_sm < per_sm) per_sm = c->ctas_per_sm;
+    const unsigned ngroups = (c->a.nplanes + c->a.G - 1) / c->a.G;
+    long long grid_x = (long long)per_sm * num_sms;
+    if (grid_x > ngroups) grid_x = ngroups;
+    kern<<<(unsigned)grid_x, Cfg::T, Cfg::SMEM_BYTES, c->stream>>>(c->a, c->tw);
+    return cudaGetLastError() == cudaSuccess ? 0 : -4;
+}
+
 }  // namespace sgw
 
 #define SGW_CAT_(a, b) a##b
@@ -121,4 +155,14 @@ extern "C" int SGW_CAT(sgw_pass_launch_, SGW_N)(const sgw::PassCall* c) {
         case K_INV: return launch<MODE_INV, OpStore>(c);
         default: return -1;
     }
+}
+
+// Fused xy-plane pass (nx == ny == SGW_N).  Returns 1 if this length has no plane kernel.
+extern "C" int SGW_CAT(sgw_plane_launch_, SGW_N)(const sgw::PlaneCall* c) {
+#if SGW_N >= 32
+    return c->mode == sgw::PL_TD ? sgw::launch_plane<sgw::PL_TD>(c) : sgw::launch_plane<sgw::PL_SUM>(c);
+#else
+    (void)c;
+    return 1;
+#endif
 }

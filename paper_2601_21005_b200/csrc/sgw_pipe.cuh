@@ -108,6 +108,50 @@ struct PipeCfg {
     static constexpr int FIXED_BYTES = XCH_BYTES + TW_BYTES;
 };
 
+// One round trip (forward, k-space multiply, inverse) of the staged tile: the three register phases
+// with their two shared-memory exchanges.  Contains two __syncthreads.
+template <int N, int B, bool FASTN, class Op>
+__device__ __forceinline__ void tile_roundtrip(const Op& op, const StageView& sv, cd* xA, cd* xB, const cd* twAp,
+                                               const cd* twBp, const cd* ktp, const double* ktr, bool actA, bool actB,
+                                               cd* out, cd* series, long long ostep) {
+    constexpr int R1 = Fact<N>::R1, R2 = Fact<N>::R2;
+    constexpr int SK = R2 | 1;
+    constexpr int ESTEP = FASTN ? R2 : R2 * B;
+    cd x[R1];
+    if (actA) {
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) x[n1] = op.pro(sv.c16(SLOT_IN, n1 * ESTEP), sv, n1 * ESTEP);
+        Dft<R1, -1>::run(x);
+        xA[0] = x[0];
+#pragma unroll
+        for (int j = 1; j < R1; ++j) xA[j * SK] = cmul(x[j], twAp[j * R2]);
+    }
+    __syncthreads();
+    if (actB) {
+        cd y[R2];
+#pragma unroll
+        for (int m = 0; m < R2; ++m) y[m] = xB[m];
+        Dft<R2, -1>::run(y);
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) {
+            if (Op::CPLX_MULT) y[k2] = cmul(y[k2], ktp[R1 * k2]);
+            else y[k2] = cscale(y[k2], ktr[R1 * k2]);
+        }
+        Dft<R2, +1>::run(y);
+        xB[0] = y[0];
+#pragma unroll
+        for (int m = 1; m < R2; ++m) xB[m] = cmulc(y[m], twBp[m * R1]);
+    }
+    __syncthreads();
+    if (actA) {
+#pragma unroll
+        for (int j = 0; j < R1; ++j) x[j] = xA[j * SK];
+        Dft<R1, +1>::run(x);
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) op.epi(x[n1], sv, n1 * ESTEP, out, series, n1 * ostep);
+    }
+}
+
 template <int N, int B, bool FASTN, class Op>
 __global__ void __launch_bounds__(PipeCfg<N, B>::T) pipe_kernel(PassGeom gm, PipeArgs pa, const cd* __restrict__ twN, Op op) {
     using Cfg = PipeCfg<N, B>;
@@ -196,41 +240,8 @@ __global__ void __launch_bounds__(PipeCfg<N, B>::T) pipe_kernel(PassGeom gm, Pip
 #pragma unroll
         for (int s = 0; s < NSLOT; ++s) sv.slot[s] = st + pa.src[s].slot_off + eA * pa.src[s].esz;
 
-        cd x[R1];
-        if (actA) {
-#pragma unroll
-            for (int n1 = 0; n1 < R1; ++n1) x[n1] = op.pro(sv.c16(SLOT_IN, n1 * ESTEP), sv, n1 * ESTEP);
-            Dft<R1, -1>::run(x);
-            xA[0] = x[0];
-#pragma unroll
-            for (int j = 1; j < R1; ++j) xA[j * SK] = cmul(x[j], twAp[j * R2]);
-        }
-        __syncthreads();
-        if (actB) {
-            cd y[R2];
-#pragma unroll
-            for (int m = 0; m < R2; ++m) y[m] = xB[m];
-            Dft<R2, -1>::run(y);
-#pragma unroll
-            for (int k2 = 0; k2 < R2; ++k2) {
-                if (Op::CPLX_MULT) y[k2] = cmul(y[k2], ktp[R1 * k2]);
-                else y[k2] = cscale(y[k2], ktr[R1 * k2]);
-            }
-            Dft<R2, +1>::run(y);
-            xB[0] = y[0];
-#pragma unroll
-            for (int m = 1; m < R2; ++m) xB[m] = cmulc(y[m], twBp[m * R1]);
-        }
-        __syncthreads();
-        if (actA) {
-#pragma unroll
-            for (int j = 0; j < R1; ++j) x[j] = xA[j * SK];
-            Dft<R1, +1>::run(x);
-            cd* out = op.p.out + base + oA;
-            cd* series = op.p.series + base + oA;
-#pragma unroll
-            for (int n1 = 0; n1 < R1; ++n1) op.epi(x[n1], sv, n1 * ESTEP, out, series, n1 * ostep);
-        }
+        tile_roundtrip<N, B, FASTN, Op>(op, sv, xA, xB, twAp, twBp, ktp, ktr, actA, actB, op.p.out + base + oA,
+                                        op.p.series + base + oA, ostep);
     }
 }
 

@@ -126,10 +126,15 @@ extern "C" int sgw_apply_H(sgw_ctx* c, int nvec, const void* d_in, void* d_out) 
         cd* o0 = out + (long long)v0 * c->ng;
         OpParams p = zero_params();
         p.out = o0;
-        p.mul_re = c->kin[0];
-        SGW_TRY(run_pass(c, 0, K_RT_STORE, nv, i0, p));
-        p.mul_re = c->kin[1]; p.acc = o0;
-        SGW_TRY(run_pass(c, 1, K_RT_ACC, nv, i0, p));
+        int rp = run_plane(c, PL_SUM, nv, i0, o0, nullptr, false);
+        if (rp < 0) return rp;
+        if (rp == 1) {
+            p.mul_re = c->kin[0];
+            SGW_TRY(run_pass(c, 0, K_RT_STORE, nv, i0, p));
+            p.mul_re = c->kin[1]; p.acc = o0;
+            SGW_TRY(run_pass(c, 1, K_RT_ACC, nv, i0, p));
+        }
+        p.acc = o0;
         SGW_TRY(kb_apply(c, nv, i0, o0, 0, 1.0));
         p.mul_re = c->kin[2]; p.vtab = c->vloc;
         SGW_TRY(run_pass(c, 2, K_RT_HFIN, nv, i0, p));
@@ -180,10 +185,16 @@ extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* 
                 const int nc = (nv - cv < chunk) ? nv - cv : chunk;
                 const long long co = (long long)cv * ng;
                 OpParams p = zero_params();
-                p.out = W; p.mul_re = c->cheb_kin[0];
-                SGW_TRY(run_pass(c, 0, K_RT_STORE, nc, cur + co, p));
-                p.mul_re = c->cheb_kin[1]; p.acc = W;
-                SGW_TRY(run_pass(c, 1, K_RT_ACC, nc, cur + co, p));
+                p.out = W;
+                int rp = run_plane(c, PL_SUM, nc, cur + co, W, nullptr, true);
+                if (rp < 0) return rp;
+                if (rp == 1) {
+                    p.mul_re = c->cheb_kin[0];
+                    SGW_TRY(run_pass(c, 0, K_RT_STORE, nc, cur + co, p));
+                    p.mul_re = c->cheb_kin[1]; p.acc = W;
+                    SGW_TRY(run_pass(c, 1, K_RT_ACC, nc, cur + co, p));
+                }
+                p.acc = W;
                 SGW_TRY(kb_apply(c, nc, cur + co, W, 0, s));
                 p.mul_re = c->cheb_kin[2]; p.vtab = c->vtab;
                 p.out = other + co; p.prev = other + co; p.use_prev = (n >= 2);
@@ -243,10 +254,15 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             } else {
                 p.pro_phase = c->phase;
             }
-            p.mul_c = c->td_kin[0];
-            SGW_TRY(run_pass(c, 0, K_RT_TD, nc, ps, p));
-            p.pro_phase = nullptr; p.mul_c = c->td_kin[1];
-            SGW_TRY(run_pass(c, 1, K_RT_TD, nc, ps, p));
+            int rp = run_plane(c, PL_TD, nc, ps, ps, p.pro_phase, false);
+            if (rp < 0) return rp;
+            if (rp == 1) {
+                p.mul_c = c->td_kin[0];
+                SGW_TRY(run_pass(c, 0, K_RT_TD, nc, ps, p));
+                p.pro_phase = nullptr; p.mul_c = c->td_kin[1];
+                SGW_TRY(run_pass(c, 1, K_RT_TD, nc, ps, p));
+            }
+            p.pro_phase = nullptr;
             p.mul_c = c->td_kin[2];
             if (!kb) p.epi_phase = c->phase;
             SGW_TRY(run_pass(c, 2, K_RT_TD, nc, ps, p));

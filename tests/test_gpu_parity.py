@@ -267,3 +267,31 @@ def test_norms_and_error_codes(api, torch_cuda):
     assert e.value.code == -1
     assert ctx.sgw_launch_count() > 0
     ctx.close()
+
+
+# ------------------------------------------------------------------ fused xy-plane pass (nx == ny)
+@pytest.mark.parametrize("n,nz,nvec,G", [(32, 16, 3, None), (96, 8, 2, None), (64, 12, 3, "3"), (128, 8, 2, "3"),
+                                          (48, 8, 1, "5"), (32, 8, 2, "1")])
+def test_plane_pass_H_cheb_td(api, torch_cuda, oracle, monkeypatch, n, nz, nvec, G):
+    """Square planes take the fused plane kernel; G (planes per group) is varied to hit ragged groups
+    and the single-plane path."""
+    torch = torch_cuda
+    if G is not None:
+        monkeypatch.setenv("SGW_PLANE_G", G)
+    g, vloc, kb, rng = problem(n, n, nz, seed=n + nz)
+    psi = rvec(rng, g, nvec)
+    ctx = make_ctx(api, torch, g, vloc, kb, nvec)
+    got = ctx.sgw_apply_H(torch.from_numpy(psi).cuda()).cpu().numpy()
+    assert relerr(got, oracle.apply_H(g, vloc, kb, psi, ld=True)) < TOL_H
+    emin, emax = W.spectral_bounds(g, vloc, True)
+    coeffs = rng.standard_normal(9)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+    assert relerr(t.cpu().numpy(), oracle.cheb_filter(g, vloc, kb, psi, coeffs, emin, emax, ld=True)) < TOL_FULL
+    ctx.sgw_set_nonlocal(None, None, None, None)
+    rs = 2.0 / (nvec * g.dV) * 0.01
+    ctx.sgw_set_td(1, rs)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_td_propagate(t, 0.05, 4)
+    assert relerr(t.cpu().numpy(), oracle.td_propagate(g, vloc, None, psi, 0.05, 4, 1, rs, ld=True)) < TOL_FULL
+    ctx.close()
