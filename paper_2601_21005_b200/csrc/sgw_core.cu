@@ -8,7 +8,8 @@
 
 #define SGW_DECL(N)                                             \
     extern "C" int sgw_pass_launch_##N(const sgw::PassCall*);   \
-    extern "C" int sgw_plane_launch_##N(const sgw::PlaneCall*);
+    extern "C" int sgw_plane_launch_##N(const sgw::PlaneCall*); \
+    extern "C" int sgw_eng_launch_##N(const sgw::EngCall*, int);
 SGW_DECL(8) SGW_DECL(12) SGW_DECL(16) SGW_DECL(24) SGW_DECL(32) SGW_DECL(48) SGW_DECL(64) SGW_DECL(96)
 SGW_DECL(128) SGW_DECL(192) SGW_DECL(256) SGW_DECL(384)
 #undef SGW_DECL
@@ -40,6 +41,16 @@ static pass_launch_fn launcher_for(int n) {
 static plane_launch_fn plane_launcher_for(int n) {
     switch (n) {
 #define SGW_CASE(N) case N: return sgw_plane_launch_##N;
+        SGW_CASE(8) SGW_CASE(12) SGW_CASE(16) SGW_CASE(24) SGW_CASE(32) SGW_CASE(48) SGW_CASE(64) SGW_CASE(96)
+        SGW_CASE(128) SGW_CASE(192) SGW_CASE(256) SGW_CASE(384)
+#undef SGW_CASE
+        default: return nullptr;
+    }
+}
+
+static eng_launch_fn eng_launcher_for(int n) {
+    switch (n) {
+#define SGW_CASE(N) case N: return sgw_eng_launch_##N;
         SGW_CASE(8) SGW_CASE(12) SGW_CASE(16) SGW_CASE(24) SGW_CASE(32) SGW_CASE(48) SGW_CASE(64) SGW_CASE(96)
         SGW_CASE(128) SGW_CASE(192) SGW_CASE(256) SGW_CASE(384)
 #undef SGW_CASE
@@ -213,7 +224,7 @@ extern "C" int sgw_destroy(sgw_ctx* c) {
     }
     cudaFree(c->vloc); cudaFree(c->vtab); cudaFree(c->vk3d); cudaFree(c->sph_ptr); cudaFree(c->sph_idx);
     cudaFree(c->beta); cudaFree(c->D); cudaFree(c->kbc); cudaFree(c->pois); cudaFree(c->rho); cudaFree(c->vh);
-    cudaFree(c->phase);
+    cudaFree(c->phase); cudaFree(c->d_segs); cudaFree(c->d_cnt); cudaFree(c->d_err);
     delete c;
     return SGW_OK;
 }
@@ -275,6 +286,14 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     if (nx == ny && nx % 8 == 0 && !(getenv("SGW_NOPLANE") && atoi(getenv("SGW_NOPLANE")))) c->plane = plane_launcher_for(nx);
     { const char* e = getenv("SGW_PLANE_G"); if (e && atoi(e) > 0) c->plane_G = atoi(e); }
     { const char* e = getenv("SGW_PLANE_CTAS"); if (e) c->plane_ctas = atoi(e); }
+    for (int a = 0; a < 3; ++a) { c->eng[a] = eng_launcher_for(dims[a]); c->engB[a] = (nx % 8 == 0 && ny % 8 == 0) ? 8 : 4; }
+    c->use_engine = 1; c->eng_max_ctas = 0; c->eng_resident = -1; c->eng_pc = 0;
+    c->d_segs = nullptr; c->segs_cap = 0; c->d_cnt = nullptr; c->cnt_cap = 0; c->d_err = nullptr;
+    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, 0);
+    { const char* e = getenv("SGW_ENGINE"); if (e) c->use_engine = atoi(e); }
+    { const char* e = getenv("SGW_ENG_CTAS"); if (e) c->eng_max_ctas = atoi(e); }
+    { const char* e = getenv("SGW_ENG_RESIDENT"); if (e) c->eng_resident = atoi(e); }
+    { const char* e = getenv("SGW_ENG_PC"); if (e) c->eng_pc = atoi(e); }
     for (int i = 0; i < 3 * K_NKINDS; ++i) { c->prof_ms[i] = 0; c->prof_n[i] = 0; }
     if (!rc) rc = dev_alloc(&c->vtab, c->ng);
     if (!rc) rc = dev_alloc(&c->vk3d, c->ng);

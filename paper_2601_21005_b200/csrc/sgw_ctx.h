@@ -8,6 +8,7 @@
 
 #include "../../include/sgw.h"
 #include "sgw_plane.cuh"
+#include "sgw_engine.cuh"
 
 struct sgw_ctx {
     int nx, ny, nz;
@@ -49,6 +50,19 @@ struct sgw_ctx {
     int hartree_mode;
     double rho_scale;
     int64_t launches;
+    // pass engine (sgw_engine.cuh)
+    sgw::eng_launch_fn eng[3];               // per-axis launcher
+    int engB[3];                             // pencils per tile per axis
+    int use_engine;                          // 0: v2 kernels (plane/pipe), 1: engine
+    int eng_max_ctas;                        // 0 = fill the device
+    int eng_resident;                        // -1 auto, 0 stream all vectors per term, 1 force L2-resident groups
+    int eng_pc;                              // planes per x/y group (0 = auto)
+    int num_sms;
+    sgw::Seg* d_segs;
+    size_t segs_cap;
+    unsigned* d_cnt;
+    size_t cnt_cap;
+    int* d_err;
     int l2_chunk;                            // vectors per L2-resident chunk (0 = whole batch)
     // optional per-pass device timing (sgw_profile_*): event pairs around pass launches
     bool prof_on;
@@ -66,4 +80,11 @@ PassGeom geom_for_axis(const sgw_ctx* c, int axis, int nvec, long long* ntiles);
 int run_pass(sgw_ctx* c, int axis, int kind, int nvec, const cd* in, const OpParams& p);
 // fused x+y pass; returns 1 when unavailable for this grid (caller runs the two passes instead)
 int run_plane(sgw_ctx* c, int mode, int nvec, const cd* in, cd* out, const cd* phase, bool cheb_tables);
+// engine-based implementations (sgw_program.cu)
+int eng_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out);
+int eng_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* h_coeffs, double s, int nterms);
+int eng_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb);
+int eng_check_error(sgw_ctx* c);
+int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau);
+int ensure_ws(sgw_ctx* c, int n);
 }  // namespace sgw

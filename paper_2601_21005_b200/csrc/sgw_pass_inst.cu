@@ -3,6 +3,7 @@
 #include <cstdlib>
 
 #include "sgw_plane.cuh"
+#include "sgw_engine.cuh"
 
 #ifndef SGW_N
 #error "compile with -DSGW_N=<axis length>"
@@ -137,6 +138,43 @@ static int launch_plane(const PlaneCall* c) {
     return cudaGetLastError() == cudaSuccess ? 0 : -4;
 }
 
+
+// ---- pass engine (sgw_engine.cuh) -----------------------------------------------------------------
+template <int B, bool CPLX>
+static int launch_engine_b(const EngCall* c) {
+    constexpr int N = SGW_N;
+    using Cfg = EngCfg<N, B>;
+    auto kern = engine_kernel<N, B, CPLX>;
+    const size_t smem = CPLX ? Cfg::SMEM_CPLX : Cfg::SMEM_REAL;
+    static int per_sm = 0, num_sms = 0;
+    if (!per_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaError_t e = smem > 48 * 1024 ? cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) : cudaSuccess;
+        if (e != cudaSuccess) return -(1000 + (int)e);
+        int n = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, Cfg::T, smem);
+        if (e != cudaSuccess) return -(2000 + (int)e);
+        if (n < 1) return -2999;
+        per_sm = n;
+    }
+    long long grid = (long long)per_sm * num_sms;
+    if (c->max_ctas > 0 && c->max_ctas < grid) grid = c->max_ctas;
+    if (grid > (long long)c->args.nitems) grid = c->args.nitems;
+    if (grid <= 0) return 0;
+    if (c->args.use_deps) {
+        EngArgs args = c->args;
+        void* params[] = {(void*)&args};
+        cudaError_t e = cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)grid), dim3(Cfg::T), params, smem,
+                                                    c->stream);
+        return e == cudaSuccess ? 0 : -(3000 + (int)e);
+    }
+    kern<<<(unsigned)grid, Cfg::T, smem, c->stream>>>(c->args);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? 0 : -(4000 + (int)e);
+}
+
 }  // namespace sgw
 
 #define SGW_CAT_(a, b) a##b
@@ -165,4 +203,12 @@ extern "C" int SGW_CAT(sgw_plane_launch_, SGW_N)(const sgw::PlaneCall* c) {
     (void)c;
     return 1;
 #endif
+}
+
+// Pass engine: B = pencils per tile (4 or 8).
+extern "C" int SGW_CAT(sgw_eng_launch_, SGW_N)(const sgw::EngCall* c, int B) {
+    using namespace sgw;
+    if (B == 8) return c->cplx ? launch_engine_b<8, true>(c) : launch_engine_b<8, false>(c);
+    if (B == 4) return c->cplx ? launch_engine_b<4, true>(c) : launch_engine_b<4, false>(c);
+    return 1;
 }

@@ -24,13 +24,15 @@ int launched(sgw_ctx* c, const char* what) {
     return check_cuda(cudaGetLastError(), what);
 }
 
-int ensure_ws(sgw_ctx* c, int n) {
+}  // namespace
+int sgw::ensure_ws(sgw_ctx* c, int n) {
     for (int a = 0; a < n; ++a)
         if (!c->ws[a])
             SGW_TRY(check_cuda(cudaMalloc((void**)&c->ws[a], (size_t)c->max_nvec * c->ng * sizeof(cd)), "workspace"));
     return 0;
 }
 
+namespace {
 int ensure_kbc(sgw_ctx* c, int nvec) {
     const long long need = (long long)nvec * c->nsphere * c->nproj;
     if (need <= c->kbc_cap) return 0;
@@ -54,7 +56,8 @@ int kb_apply_np(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double s
 }
 
 // dst += sum beta f <beta|src>, all projections taken from src before any scatter (R-11)
-int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau) {
+}  // namespace
+int sgw::kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau) {
     if (c->nsphere == 0) return 0;
     SGW_TRY(ensure_kbc(c, nvec));
     switch (c->nproj) {
@@ -70,6 +73,7 @@ int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scal
     return set_error(SGW_EINVAL, "bad nproj");
 }
 
+namespace {
 OpParams zero_params() {
     OpParams p;
     memset(&p, 0, sizeof(p));
@@ -124,6 +128,11 @@ extern "C" int sgw_apply_H(sgw_ctx* c, int nvec, const void* d_in, void* d_out) 
         const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
         const cd* i0 = in + (long long)v0 * c->ng;
         cd* o0 = out + (long long)v0 * c->ng;
+        if (c->use_engine) {
+            SGW_TRY(eng_apply_H(c, nv, i0, o0));
+            SGW_TRY(kb_apply(c, nv, i0, o0, 0, 1.0));
+            continue;
+        }
         OpParams p = zero_params();
         p.out = o0;
         int rp = run_plane(c, PL_SUM, nv, i0, o0, nullptr, false);
@@ -159,7 +168,7 @@ extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* 
         scale_kernel<<<blocks_for(ng * nvec, 256), 256, 0, c->stream>>>((cd*)d_psi, h_coeffs[0], ng * nvec);
         return launched(c, "scale");
     }
-    SGW_TRY(ensure_ws(c, 3));
+    SGW_TRY(ensure_ws(c, c->use_engine ? 2 : 3));
     // tables scaled by s = 2/dE so that one pass yields 2*Ht*phi directly (R-1; Eq. 3 mapping to [-1,1])
     for (int a = 0; a < 3; ++a) {
         scale_table_kernel<<<blocks_for(c->dims[a], 128), 128, 0, c->stream>>>(c->kin[a], s, c->cheb_kin[a], c->dims[a]);
@@ -170,6 +179,10 @@ extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* 
     for (int v0 = 0; v0 < nvec; v0 += c->max_nvec) {
         const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
         cd* X0 = (cd*)d_psi + (long long)v0 * ng;
+        if (c->use_engine) {
+            SGW_TRY(eng_cheb_filter(c, nv, X0, h_coeffs, s, nterms));
+            continue;
+        }
         cd *P1 = c->ws[0], *W = c->ws[1], *O = c->ws[2];
         cd* cur = X0;
         cd* other = P1;              // receives phi_n; holds phi_{n-2} for n >= 2
@@ -254,7 +267,13 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             } else {
                 p.pro_phase = c->phase;
             }
-            int rp = run_plane(c, PL_TD, nc, ps, ps, p.pro_phase, false);
+            int rp = 1;
+            if (c->use_engine) {
+                SGW_TRY(eng_td_step(c, nc, ps, kb));
+                rp = 2;
+            } else {
+                rp = run_plane(c, PL_TD, nc, ps, ps, p.pro_phase, false);
+            }
             if (rp < 0) return rp;
             if (rp == 1) {
                 p.mul_c = c->td_kin[0];
@@ -265,7 +284,7 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             p.pro_phase = nullptr;
             p.mul_c = c->td_kin[2];
             if (!kb) p.epi_phase = c->phase;
-            SGW_TRY(run_pass(c, 2, K_RT_TD, nc, ps, p));
+            if (rp != 2) SGW_TRY(run_pass(c, 2, K_RT_TD, nc, ps, p));
             if (kb) {
                 SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt));
                 dim3 g2(blocks_for(ng, 256), nc);
