@@ -287,13 +287,16 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     { const char* e = getenv("SGW_PLANE_G"); if (e && atoi(e) > 0) c->plane_G = atoi(e); }
     { const char* e = getenv("SGW_PLANE_CTAS"); if (e) c->plane_ctas = atoi(e); }
     for (int a = 0; a < 3; ++a) { c->eng[a] = eng_launcher_for(dims[a]); c->engB[a] = (nx % 8 == 0 && ny % 8 == 0) ? 8 : 4; }
-    c->use_engine = 1; c->eng_max_ctas = 0; c->eng_resident = -1; c->eng_pc = 0;
+    c->use_engine = 0; c->eng_max_ctas = 0; c->eng_resident = -1; c->eng_pc = 0;
     c->d_segs = nullptr; c->segs_cap = 0; c->d_cnt = nullptr; c->cnt_cap = 0; c->d_err = nullptr;
     cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, 0);
     { const char* e = getenv("SGW_ENGINE"); if (e) c->use_engine = atoi(e); }
     { const char* e = getenv("SGW_ENG_CTAS"); if (e) c->eng_max_ctas = atoi(e); }
     { const char* e = getenv("SGW_ENG_RESIDENT"); if (e) c->eng_resident = atoi(e); }
     { const char* e = getenv("SGW_ENG_PC"); if (e) c->eng_pc = atoi(e); }
+    c->eng_l2_prefetch = 0;
+    { const char* e = getenv("SGW_ENG_L2PF"); if (e) c->eng_l2_prefetch = atoi(e); }
+    { const char* e = getenv("SGW_ENG_B"); if (e && (atoi(e) == 4 || (atoi(e) == 8 && c->engB[0] == 8))) for (int a = 0; a < 3; ++a) c->engB[a] = atoi(e); }
     for (int i = 0; i < 3 * K_NKINDS; ++i) { c->prof_ms[i] = 0; c->prof_n[i] = 0; }
     if (!rc) rc = dev_alloc(&c->vtab, c->ng);
     if (!rc) rc = dev_alloc(&c->vk3d, c->ng);

@@ -56,6 +56,7 @@ struct sgw_ctx {
     int use_engine;                          // 0: v2 kernels (plane/pipe), 1: engine
     int eng_max_ctas;                        // 0 = fill the device
     int eng_resident;                        // -1 auto, 0 stream all vectors per term, 1 force L2-resident groups
+    int eng_l2_prefetch;                     // 1: prefetch the next item's operands into L2
     int eng_pc;                              // planes per x/y group (0 = auto)
     int num_sms;
     sgw::Seg* d_segs;

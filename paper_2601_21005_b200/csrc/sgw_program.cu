@@ -1,5 +1,6 @@
 // sgw_program.cu -- host side of the pass engine: builds programs of segments (sgw_engine.cuh) for
 // H apply, the Chebyshev filter and the split-operator step, and launches them.
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -37,7 +38,12 @@ int pick_pc(const sgw_ctx* c, int nplanes, int tpp) {
         while (nplanes % pc) --pc;
         return pc;
     }
-    int target = (6 * c->num_sms) / (2 * tpp);
+    // a group's y tiles follow its x tiles by one slot: make a slot about a wave of tiles (measured best on
+    // cfg1: 64 planes of 12 tiles), but keep the planes in flight (two slots, cur and acc) inside L2
+    int target = (5 * c->num_sms) / tpp;
+    const double plane_bytes = 16.0 * c->nx * c->ny;
+    const int cap = (int)(40.0e6 / (4.0 * plane_bytes));
+    if (target > cap) target = cap;
     if (target < 1) target = 1;
     if (target > nplanes) target = nplanes;
     while (nplanes % target) --target;
@@ -126,6 +132,7 @@ int launch_segments(sgw_ctx* c, const Program& P, int s0, int s1, unsigned nitem
     }
     a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
     a.use_deps = deps ? 1 : 0;
+    a.l2_prefetch = c->eng_l2_prefetch;
     call.cplx = t.cplx ? 1 : 0;
     call.max_ctas = c->eng_max_ctas;
     call.stream = c->stream;
@@ -248,8 +255,7 @@ int eng_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* a, double s, in
     // vectors per launch group: L2-resident groups when at least two vectors (3 arrays each) fit
     const double bytes_vec = 16.0 * (double)ng, l2_budget = 96.0e6;
     int fit = (int)(l2_budget / (3.0 * bytes_vec));
-    bool resident = cubic(c) && !kb && fit >= 2;
-    if (c->eng_resident == 0) resident = false;
+    bool resident = false;      // measured slower than streaming all vectors per term (launches too small): opt-in
     if (c->eng_resident > 0 && cubic(c) && !kb) { resident = true; if (fit < c->eng_resident) fit = c->eng_resident; }
     int group = nvec;
     if (resident) { group = fit < nvec ? fit : nvec; if (group > 2) group &= ~1; }
