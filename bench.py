@@ -22,8 +22,12 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2601_21005_b200 import workloads as W  # noqa: E402
+from paper_2601_21005_b200 import shard, workloads as W  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (z round trip + recurrence on
+# cfg1), from the ncu --set full capture summarised in profiles/r01_v2_cfg1.md: 3.69 GB without and 5.52 GB with
+# the series flush (every third term) -> average per launch
+NCU_TRAFFIC_BYTES = {"z_cheb": (2 * 3.69e9 + 5.52e9) / 3.0, "y_acc": 2.18e9}
 METRIC = "grid-pt*vector H-applies/s (Chebyshev filter)"
 UNIT = "grid-pt*vec*H-applies/s"
 WORKLOAD = "cfg1"
@@ -145,7 +149,7 @@ def run_gpu(args):
     units_rank = g.ng * nvec * napply
     stream = torch.cuda.current_stream(dev)
     ctx = api.context_for(w, max_nvec=nvec, stream=stream, device=f"cuda:{local}")
-    psi0 = ctx.sgw_random_vectors(W.SEED_VEC, rank * nvec, nvec)     # each rank filters its own vectors
+    psi0 = ctx.sgw_random_vectors(W.SEED_VEC, shard.first_vector(rank, nvec), nvec)   # each rank filters its own vectors
     psi = torch.empty_like(psi0)
 
     def barrier():
@@ -179,11 +183,8 @@ def run_gpu(args):
     clocks = sampler.stop() if rank == 0 else None
     prof = {(a, k): ctx.sgw_profile_get(a, k) for a in range(3) for k in range(8)}
     ctx.sgw_profile_enable(0)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = units_rank * world * args.steps / (ms * 1e-3)
+    ms = shard.max_over_ranks(ms, dev)
+    value = shard.whole_job_rate(units_rank, world, args.steps, ms)
 
     # ---- end to end: host buffers, H2D of the inputs and D2H of the result inside the timed region
     h_in = psi0.cpu().pin_memory()
@@ -203,12 +204,13 @@ def run_gpu(args):
     e1.record(stream)
     barrier()
     ms_e2e = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
-    e2e_value = units_rank * world * args.steps / (ms_e2e * 1e-3)
+    ms_e2e = shard.max_over_ranks(ms_e2e, dev)
+    e2e_value = shard.whole_job_rate(units_rank, world, args.steps, ms_e2e)
     checksum = float(torch.view_as_real(h_out).abs().sum())
+
+    td = None
+    if world == 1 and not args.no_td:
+        td = run_td(torch, api, dev, stream, args)
 
     if rank == 0:
         peak, peak_src = measured_peaks()
@@ -226,7 +228,7 @@ def run_gpu(args):
         strict_bytes = 80.0 + 8.0 / nvec                            # compulsory bytes per term
         term_gbs = strict_bytes * units_rank * args.steps / (ms * 1e-3) / 1e9
         moved = sum(bytes_per_unit.get(k_, 32.0) * units_launch * v_["launches"] for k_, v_ in passes.items())
-        cpu_val, cpu_dt, cpu_nv, cpu_cores = oracle_sample(w, os.cpu_count() or 1, 16)
+        cpu_val, cpu_dt, cpu_nv, cpu_cores = oracle_sample(w, os.cpu_count() or 1, 32)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -239,18 +241,55 @@ def run_gpu(args):
                     "ms_per_step": ms_e2e / args.steps, "checksum": checksum},
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "kernel": f"pass_kernel<96,RT,{dn}>", "achieved": ach, "peak": peak,
-                         "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                         "unit": "GB/s", "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(dn),
+                         "traffic_source": "profiles/r01_v2_cfg1.md (ncu --set full, bytes per launch)",
+                         "algorithmic_bytes_per_launch": bytes_per_unit.get(dn, 32.0) * units_launch, "peak_source": peak_src,
                          "avg_launch_ms": avg_ms, "bytes_per_unit": bytes_per_unit.get(dn, 32.0),
                          "kernel_share_of_step": dv["ms_total"] / ms,
                          "term_strict": {"bytes_per_unit": strict_bytes, "achieved": term_gbs, "frac": term_gbs / peak},
                          "term_moved": {"achieved": moved / (ms * 1e-3) / 1e9, "frac": moved / (ms * 1e-3) / 1e9 / peak},
                          "passes": passes},
+            "td": td,
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",
-                             "sample": f"{cpu_nv} vectors x 16 H applies of the same filter, {WORKLOAD} grid ({cpu_dt:.1f} s)"},
+                             "sample": f"{cpu_nv} vectors x 32 H applies of the same filter, {WORKLOAD} grid ({cpu_dt:.1f} s)"},
         }
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_td(torch, api, dev, stream, args):
+    """Second stage of the metric: split-operator steps with the per-step Hartree rebuild on BASELINE.json
+    configs[2] (128^3, Si87H76-shaped, 16 filtered vectors, dt = 0.05); a 100-step sample of the 2000."""
+    w = W.make_workload("cfg2", nterms=33)
+    ctx = api.context_for(w, max_nvec=w.nvec, stream=stream, device=str(dev))
+    psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
+    ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)            # filtered start vectors (untimed)
+    ctx.sgw_set_td(1, w.rho_scale)
+    nsteps = 100
+    ctx.sgw_td_propagate(psi, w.dt, 10)                            # warm-up
+    norms0 = ctx.sgw_norms(psi).cpu().numpy()
+    torch.cuda.synchronize(dev)
+    l0 = ctx.sgw_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    ctx.sgw_td_propagate(psi, w.dt, nsteps)
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    ms = e0.elapsed_time(e1)
+    norms = ctx.sgw_norms(psi).cpu().numpy()
+    units = w.grid.ng * w.nvec * nsteps
+    peak, _ = measured_peaks()
+    strict = 32.0 + 40.0 / w.nvec                                  # SURVEY 8(d): compulsory bytes per grid-pt*vector*step
+    gbs = strict * units / (ms * 1e-3) / 1e9
+    out = {"metric": "grid-pt*vector H-applies/s (TD step)", "value": units / (ms * 1e-3), "unit": UNIT,
+           "workload": f"cfg2: 128^3 grid h=0.5, {w.atoms}-shaped V_loc, {w.nvec} filtered vectors, dt=0.05, Hartree "
+                       f"rebuilt every step; {nsteps} of the 2000 steps timed",
+           "ms_per_step": ms / nsteps, "gpu_launches": int(ctx.sgw_launch_count() - l0),
+           "strict": {"bytes_per_unit": strict, "achieved": gbs, "frac": gbs / peak},
+           "norm_drift": float(np.max(np.abs(norms / norms0 - 1.0)))}
+    ctx.close()
+    return out
 
 
 def main():
@@ -261,6 +300,7 @@ def main():
     ap.add_argument("--impl", default="sgw", choices=["sgw", "reference"])
     ap.add_argument("--nterms", type=int, default=None,
                     help="shorten the filter (profiling runs under ncu only; the default is the config's 512)")
+    ap.add_argument("--no-td", action="store_true", help="skip the TD-step sample (cfg2 shape)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

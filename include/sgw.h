@@ -22,6 +22,10 @@
  *  - The library owns only its context (tables, workspace for max_nvec vectors).  Calls with
  *    nvec > max_nvec are processed in sub-batches of max_nvec (vectors are independent in the
  *    filter; in the TD step the density is accumulated over all sub-batches first).
+ *  - Two implementations of the fused passes are built in: the default one (one kernel for the x and y
+ *    round trips of whole planes, one persistent cp.async-pipelined kernel for z) and a pass engine
+ *    (one persistent kernel executing a program of passes with dependency counters), selected with the
+ *    environment variable SGW_ENGINE=1 when the context is created.  Both compute the same results.
  *  - There is no CPU fallback: without a CUDA device sgw_init_grid fails with SGW_ECUDA.
  */
 #ifndef SGW_H
@@ -116,6 +120,11 @@ int64_t sgw_launch_count(const sgw_ctx* ctx);
 int sgw_profile_enable(sgw_ctx* ctx, int on);
 int sgw_profile_reset(sgw_ctx* ctx);
 int sgw_profile_get(sgw_ctx* ctx, int axis, int kind, int64_t* count, double* total_ms);
+
+/* Synchronises the context's stream and reports asynchronous failures: SGW_ECUDA if a kernel faulted or
+ * if a dependency wait inside the pass engine gave up (the engine never hangs: a bounded spin sets a
+ * flag instead); SGW_OK otherwise.  The only call besides setup that blocks the host. */
+int sgw_sync_check(sgw_ctx* ctx);
 
 /* Message for the last error on the calling thread ("" if none). */
 const char* sgw_last_error(void);

@@ -13,13 +13,13 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsgw.so")
+LIB_PATH = os.environ.get("SGW_LIB", os.path.join(_HERE, "libsgw.so"))
 _lib = None
 
 ERRORS = {-1: "SGW_EINVAL", -2: "SGW_ESIZE", -3: "SGW_ENOMEM", -4: "SGW_ECUDA"}
 EXPORTS = ["sgw_init_grid", "sgw_destroy", "sgw_set_vloc", "sgw_set_nonlocal", "sgw_random_vectors",
            "sgw_apply_H", "sgw_cheb_filter", "sgw_hartree", "sgw_set_td", "sgw_td_propagate", "sgw_norms",
-           "sgw_launch_count", "sgw_last_error", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get"]
+           "sgw_launch_count", "sgw_last_error", "sgw_sync_check", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get"]
 
 
 class SGWError(RuntimeError):
@@ -48,6 +48,7 @@ def load():
         lib.sgw_td_propagate.argtypes = [vp, i, vp, d, i]
         lib.sgw_norms.argtypes = [vp, i, vp, vp]
         lib.sgw_launch_count.argtypes = [vp]
+        lib.sgw_sync_check.argtypes = [vp]
         lib.sgw_launch_count.restype = i64
         lib.sgw_last_error.restype = C.c_char_p
         lib.sgw_profile_enable.argtypes = [vp, i]
@@ -172,6 +173,10 @@ class Context:
         n, ms = C.c_int64(), C.c_double()
         _check(self.lib.sgw_profile_get(self._h, axis, kind, C.byref(n), C.byref(ms)))
         return n.value, ms.value
+
+    def sgw_sync_check(self):
+        _check(self.lib.sgw_sync_check(self._h))
+        return 0
 
     def sgw_launch_count(self):
         return int(self.lib.sgw_launch_count(self._h))

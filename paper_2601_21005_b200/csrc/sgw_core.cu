@@ -215,6 +215,13 @@ extern "C" int sgw_profile_get(sgw_ctx* c, int axis, int kind, int64_t* count, d
     return SGW_OK;
 }
 
+extern "C" int sgw_sync_check(sgw_ctx* c) {
+    if (!c) return set_error(SGW_EINVAL, "sgw_sync_check: null context");
+    int rc = check_cuda(cudaStreamSynchronize(c->stream), "sgw_sync_check");
+    if (rc) return rc;
+    return sgw::eng_check_error(c);
+}
+
 extern "C" int sgw_destroy(sgw_ctx* c) {
     if (!c) return SGW_OK;
     cudaStreamSynchronize(c->stream);

@@ -106,8 +106,11 @@ static int launch_rt(const PassCall* c) {
 
 // rows/columns per plane tile: wide tiles keep one CTA (8-9 warps) on few planes so the x->y
 // transpose stays L2-resident
+#ifndef SGW_PLANE_B96
+#define SGW_PLANE_B96 24
+#endif
 constexpr int plane_B(int n) {
-    return n == 32 ? 32 : n == 48 ? 24 : n == 64 ? 32 : n == 96 ? 24 : n == 128 ? 16 : 8;
+    return n == 32 ? 32 : n == 48 ? 24 : n == 64 ? 32 : n == 96 ? SGW_PLANE_B96 : n == 128 ? 16 : 8;
 }
 
 template <int MODE>

@@ -1,0 +1,164 @@
+"""GPU parity at the sizes of BASELINE.json's configs, in the launch configuration bench.py times, and
+for the opt-in pass engine (SGW_ENGINE=1).
+
+Full-size oracle runs are only feasible for a few applications, so ("Oracle cost and
+parity coverage"): every config shape gets a single H apply compared element by element on a declared
+subset of vectors; cfg1 (the bench workload) also gets a filter prefix on two vectors taken from the
+64-vector batch that bench.py filters; cfg2 gets a TD-Hartree prefix on all 16 vectors (the Hartree
+term couples them).  What was compared at full length and what at a prefix is stated in each test.
+"""
+import numpy as np
+import pytest
+
+from paper_2601_21005_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_H = 1e-11
+TOL_FULL = 1e-8
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def api(torch_cuda):
+    from paper_2601_21005_b200 import api as a
+    a.load()
+    return a
+
+
+def relerr(got, want):
+    got = got.reshape(got.shape[0], -1)
+    want = want.reshape(want.shape[0], -1)
+    return float(np.max(np.linalg.norm(got - want, axis=1) / np.linalg.norm(want, axis=1)))
+
+
+@pytest.mark.parametrize("engine", ["0", "1"])
+def test_cfg1_bench_configuration_sampled_vectors(api, torch_cuda, oracle, monkeypatch, engine):
+    """cfg1 exactly as bench.py runs it (96^3, 64 vectors in one call, max_nvec = 64): the first 33 terms of
+    the 512-term coefficient list.  Vectors 0, 37 and 63 of the batch are compared with the oracle."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_ENGINE", engine)
+    w = W.make_workload("cfg1")
+    coeffs = w.coeffs[:33]
+    ctx = api.context_for(w)
+    psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
+    ref0 = oracle.random_vectors(w.grid, W.SEED_VEC, 0, w.nvec)
+    assert np.array_equal(psi.cpu().numpy().view(np.uint64), ref0.view(np.uint64))
+    h = ctx.sgw_apply_H(psi)
+    pick = [0, 37, 63]
+    assert relerr(h[pick].cpu().numpy(), oracle.apply_H(w.grid, w.vloc, None, ref0[pick], ld=True)) < TOL_H
+    ctx.sgw_cheb_filter(psi, coeffs, w.emin, w.emax)
+    want = oracle.cheb_filter(w.grid, w.vloc, None, ref0[pick], coeffs, w.emin, w.emax, ld=True)
+    assert relerr(psi[pick].cpu().numpy(), want) < TOL_FULL
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
+
+
+@pytest.mark.parametrize("engine", ["0", "1"])
+def test_cfg2_td_hartree_prefix_all_vectors(api, torch_cuda, oracle, monkeypatch, engine):
+    """cfg2 (128^3, 16 vectors): a 9-term filter, then 3 split-operator steps with the Hartree potential
+    rebuilt every step from all 16 vectors (prefix of the 2000 steps), every vector compared."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_ENGINE", engine)
+    w = W.make_workload("cfg2", nterms=9)
+    ctx = api.context_for(w)
+    psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
+    ref = oracle.random_vectors(w.grid, W.SEED_VEC, 0, w.nvec)
+    ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
+    ref = oracle.cheb_filter(w.grid, w.vloc, None, ref, w.coeffs, w.emin, w.emax, ld=True)
+    assert relerr(psi.cpu().numpy(), ref) < TOL_FULL
+    ctx.sgw_set_td(1, w.rho_scale)
+    n0 = ctx.sgw_norms(psi).cpu().numpy()
+    ctx.sgw_td_propagate(psi, w.dt, 3)
+    ref = oracle.td_propagate(w.grid, w.vloc, None, ref, w.dt, 3, 1, w.rho_scale, ld=True)
+    assert relerr(psi.cpu().numpy(), ref) < TOL_FULL
+    # local-only propagation is unitary: norms conserved (property that holds at any length)
+    n1 = ctx.sgw_norms(psi).cpu().numpy()
+    assert np.max(np.abs(n1 / n0 - 1.0)) < 1e-12
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
+
+
+@pytest.mark.parametrize("engine", ["0", "1"])
+def test_cfg3_shape_apply_H_and_terms_with_kb(api, torch_cuda, oracle, monkeypatch, engine):
+    """cfg3 shape (256^3, Si705H300 local + KB projectors): 2 vectors out of the 256; one H apply and a
+    4-term filter (3 applications) compared element by element."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_ENGINE", engine)
+    w = W.make_workload("cfg3", nvec=2, nterms=4)
+    assert w.atoms == "Si705H300" and w.kb.nsphere == 705
+    ctx = api.context_for(w)
+    psi = ctx.sgw_random_vectors(W.SEED_VEC, 100, 2)          # vectors 100, 101 of the batch
+    ref = oracle.random_vectors(w.grid, W.SEED_VEC, 100, 2)
+    h = ctx.sgw_apply_H(psi)
+    assert relerr(h.cpu().numpy(), oracle.apply_H(w.grid, w.vloc, w.kb, ref, ld=True)) < TOL_H
+    ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
+    want = oracle.cheb_filter(w.grid, w.vloc, w.kb, ref, w.coeffs, w.emin, w.emax, ld=True)
+    assert relerr(psi.cpu().numpy(), want) < TOL_FULL
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
+
+
+@pytest.mark.slow
+def test_cfg4_shape_apply_H_and_td_step_with_kb(api, torch_cuda, oracle):
+    """cfg4 shape (384^3, Si8381H1620 = 10001 atoms, local + KB): one vector; one H apply and one
+    TD-Hartree step compared element by element (the largest supported axis length, radix-3 factor)."""
+    torch = torch_cuda
+    w = W.make_workload("cfg4", nvec=1, nterms=2)
+    assert w.atoms == "Si8381H1620"
+    ctx = api.context_for(w)
+    psi = ctx.sgw_random_vectors(W.SEED_VEC, 31, 1)
+    ref = oracle.random_vectors(w.grid, W.SEED_VEC, 31, 1)
+    h = ctx.sgw_apply_H(psi)
+    assert relerr(h.cpu().numpy(), oracle.apply_H(w.grid, w.vloc, w.kb, ref, ld=True)) < TOL_H
+    del h
+    ctx.sgw_set_td(1, w.rho_scale)
+    ctx.sgw_td_propagate(psi, w.dt, 1)
+    want = oracle.td_propagate(w.grid, w.vloc, w.kb, ref, w.dt, 1, 1, w.rho_scale, ld=True)
+    assert relerr(psi.cpu().numpy(), want) < TOL_FULL
+    ctx.close()
+
+
+@pytest.mark.parametrize("n,nz,nvec,use_kb", [(32, 32, 4, False), (48, 48, 3, True), (64, 24, 2, True), (24, 12, 5, True),
+                                              (12, 12, 2, False)])
+def test_engine_path_small_grids(api, torch_cuda, oracle, monkeypatch, n, nz, nvec, use_kb):
+    """The pass engine (SGW_ENGINE=1) on cubic grids (one dependent launch), non-cubic grids (one launch per
+    pass) and an axis length that is not a multiple of 8 (4 pencils per tile): H apply, odd and even term
+    counts, TD with and without the Hartree rebuild."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_ENGINE", "1")
+    g = W.Grid(n, n, nz, 0.5, 0.5, 0.55)
+    rng = np.random.default_rng(7 * n + nz)
+    L = np.array(g.box)
+    centers = rng.uniform(0, 1, size=(3, 3)) * L
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    kb = W.kb_projectors(g, centers[:2], radius=min(1.8, 0.45 * L.min()), sigma=0.7) if use_kb else W.KB.empty()
+    psi = rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    if kb.nsphere:
+        ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                             torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+    kbo = kb if kb.nsphere else None
+    got = ctx.sgw_apply_H(torch.from_numpy(psi).cuda()).cpu().numpy()
+    assert relerr(got, oracle.apply_H(g, vloc, kbo, psi, ld=True)) < TOL_H
+    emin, emax = W.spectral_bounds(g, vloc, True)
+    for nterms in (2, 3, 8, 9):
+        coeffs = rng.standard_normal(nterms)
+        t = torch.from_numpy(psi).cuda()
+        ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+        assert relerr(t.cpu().numpy(), oracle.cheb_filter(g, vloc, kbo, psi, coeffs, emin, emax, ld=True)) < TOL_FULL
+    rs = 2.0 / (nvec * g.dV) * 0.01
+    for mode in (0, 1):
+        ctx.sgw_set_td(mode, rs)
+        t = torch.from_numpy(psi).cuda()
+        ctx.sgw_td_propagate(t, 0.05, 3)
+        assert relerr(t.cpu().numpy(), oracle.td_propagate(g, vloc, kbo, psi, 0.05, 3, mode, rs, ld=True)) < TOL_FULL
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
