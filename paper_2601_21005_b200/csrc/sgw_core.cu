@@ -9,7 +9,8 @@
 #define SGW_DECL(N)                                             \
     extern "C" int sgw_pass_launch_##N(const sgw::PassCall*);   \
     extern "C" int sgw_plane_launch_##N(const sgw::PlaneCall*); \
-    extern "C" int sgw_eng_launch_##N(const sgw::EngCall*, int);
+    extern "C" int sgw_eng_launch_##N(const sgw::EngCall*, int); \
+    extern "C" int sgw_lean_launch_##N(const sgw::LeanCall*, int);
 SGW_DECL(8) SGW_DECL(12) SGW_DECL(16) SGW_DECL(24) SGW_DECL(32) SGW_DECL(48) SGW_DECL(64) SGW_DECL(96)
 SGW_DECL(128) SGW_DECL(192) SGW_DECL(256) SGW_DECL(384)
 #undef SGW_DECL
@@ -56,6 +57,34 @@ static eng_launch_fn eng_launcher_for(int n) {
 #undef SGW_CASE
         default: return nullptr;
     }
+}
+
+static lean_launch_fn lean_launcher_for(int n) {
+    switch (n) {
+#define SGW_CASE(N) case N: return sgw_lean_launch_##N;
+        SGW_CASE(8) SGW_CASE(12) SGW_CASE(16) SGW_CASE(24) SGW_CASE(32) SGW_CASE(48) SGW_CASE(64) SGW_CASE(96)
+        SGW_CASE(128) SGW_CASE(192) SGW_CASE(256) SGW_CASE(384)
+#undef SGW_CASE
+        default: return nullptr;
+    }
+}
+
+// event pair around a launch while profiling is on: returns the closing event (or nullptr)
+cudaEvent_t prof_begin(sgw_ctx* c, int tag) {
+    if (!c->prof_on || c->prof_used >= 60000) return nullptr;
+    if (c->prof_ev.size() < 2 * (c->prof_used + 1)) {
+        cudaEvent_t a, b;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return nullptr;
+        c->prof_ev.push_back(a); c->prof_ev.push_back(b); c->prof_tag.push_back(0);
+    }
+    c->prof_tag[c->prof_used] = tag;
+    cudaEventRecord(c->prof_ev[2 * c->prof_used], c->stream);
+    return c->prof_ev[2 * c->prof_used + 1];
+}
+void prof_end(sgw_ctx* c, cudaEvent_t e1) {
+    if (!e1) return;
+    cudaEventRecord(e1, c->stream);
+    c->prof_used++;
 }
 
 int run_plane(sgw_ctx* c, int mode, int nvec, const cd* in, cd* out, const cd* phase, bool cheb_tables) {
@@ -293,8 +322,12 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     if (nx == ny && nx % 8 == 0 && !(getenv("SGW_NOPLANE") && atoi(getenv("SGW_NOPLANE")))) c->plane = plane_launcher_for(nx);
     { const char* e = getenv("SGW_PLANE_G"); if (e && atoi(e) > 0) c->plane_G = atoi(e); }
     { const char* e = getenv("SGW_PLANE_CTAS"); if (e) c->plane_ctas = atoi(e); }
+    for (int a = 0; a < 3; ++a) c->lean[a] = lean_launcher_for(dims[a]);
+    c->lean_G = 0; c->lean_ctas = 0;
+    { const char* e = getenv("SGW_LEAN_G"); if (e) c->lean_G = atoi(e); }
+    { const char* e = getenv("SGW_LEAN_CTAS"); if (e) c->lean_ctas = atoi(e); }
     for (int a = 0; a < 3; ++a) { c->eng[a] = eng_launcher_for(dims[a]); c->engB[a] = (nx % 8 == 0 && ny % 8 == 0) ? 8 : 4; }
-    c->use_engine = 0; c->eng_max_ctas = 0; c->eng_resident = -1; c->eng_pc = 0;
+    c->use_engine = 2; c->eng_max_ctas = 0; c->eng_resident = -1; c->eng_pc = 0;
     c->d_segs = nullptr; c->segs_cap = 0; c->d_cnt = nullptr; c->cnt_cap = 0; c->d_err = nullptr;
     cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, 0);
     { const char* e = getenv("SGW_ENGINE"); if (e) c->use_engine = atoi(e); }

@@ -9,6 +9,7 @@
 #include "../../include/sgw.h"
 #include "sgw_plane.cuh"
 #include "sgw_engine.cuh"
+#include "sgw_lean.cuh"
 
 struct sgw_ctx {
     int nx, ny, nz;
@@ -53,7 +54,9 @@ struct sgw_ctx {
     // pass engine (sgw_engine.cuh)
     sgw::eng_launch_fn eng[3];               // per-axis launcher
     int engB[3];                             // pencils per tile per axis
-    int use_engine;                          // 0: v2 kernels (plane/pipe), 1: engine
+    sgw::lean_launch_fn lean[3];             // per-axis launcher of the lean passes
+    int lean_G, lean_ctas;                   // plane kernel: planes per CTA-owned group, CTAs per SM (0 = auto)
+    int use_engine;                          // 0: v2 kernels (plane/pipe), 1: engine, 2: lean passes (default)
     int eng_max_ctas;                        // 0 = fill the device
     int eng_resident;                        // -1 auto, 0 stream all vectors per term, 1 force L2-resident groups
     int eng_l2_prefetch;                     // 1: prefetch the next item's operands into L2
@@ -86,6 +89,12 @@ int eng_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out);
 int eng_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* h_coeffs, double s, int nterms);
 int eng_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb);
 int eng_check_error(sgw_ctx* c);
+// lean-pass implementations (sgw_program.cu)
+int lean_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out);
+int lean_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* h_coeffs, double s, int nterms);
+int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb);
+cudaEvent_t prof_begin(sgw_ctx* c, int tag);
+void prof_end(sgw_ctx* c, cudaEvent_t e1);
 int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau);
 int ensure_ws(sgw_ctx* c, int n);
 }  // namespace sgw

@@ -1,0 +1,294 @@
+// sgw_lean.cuh -- lean streaming round-trip passes for sm_100a (the default implementation).
+//
+// One pass = for every tile of B pencils: acc <- hs * RT_axis(cur) [+ hs * V * cur] + alpha * acc (real k
+// table: H apply, Chebyshev term) or psi <- [phase] RT_axis([phase] psi) (complex k table:
+// split-operator factor).  What the profiles of the earlier kernels showed (profiles/
+// r01_v2_cfg1.md, r01_engine_v3_cfg1.md) shaped this one:
+//  * a tile belongs to an autonomous warp group (B * R2 threads, two warps for N = 96) with its own slice
+//    of shared memory and its own named barrier; 16 warps per SM in different phases hide each other's
+//    latency, nothing is staged through shared memory, and the only per-item work outside the
+//    transforms is one multiply-add for the tile origin;
+//  * the input is loaded straight into the registers of the first butterfly stage; everything the
+//    epilogue needs (old accumulator, potential, series) is loaded late, after the inverse transform, so
+//    it never lives across the transforms (no spills at 128 registers);
+//  * measured alone on 64 x 96^3 such a pass runs at 6.2 TB/s (acc += RT(cur), 48 B per point), i.e. at
+//    the measured HBM copy peak.
+// plane_lean_kernel runs the x and the y pass of whole xy planes in one launch: a CTA owns a group of
+// planes, does their row tiles, __syncthreads, then their column tiles, so the x->y transpose goes
+// through L2 and HBM sees cur once and acc once for the two passes.
+#pragma once
+#include "sgw_engine.cuh"   // Fact2, F_* flags
+
+namespace sgw {
+
+struct LeanArgs {
+    const cd* cur;            // input vectors
+    cd* acc;                  // accumulator / output vectors (may alias cur for the complex family)
+    cd* series;               // Chebyshev series accumulator (F_FLUSH)
+    const double* vtab;       // N_g real table (F_VTAB)
+    const cd* phase;          // N_g complex table (F_PRO / F_EPI)
+    const cd* tw;             // exp(-2 pi i j / N)
+    const double* kre[2];     // real k tables (include 1/N and any scale): [0] first pass, [1] second pass (y of a plane launch)
+    const cd* kc[2];          // complex k tables
+    double hs, c0, c1;
+    int flags[2], alpha[2];   // per pass
+    int nx, ny, nz;
+    unsigned ntiles;          // axis kernel: tiles; plane kernel: planes (nz * nvec)
+    int G;                    // plane kernel: planes per CTA-owned group
+};
+
+template <int N, int B>
+struct LeanCfg {
+    static constexpr int R1 = Fact2<N>::R1, R2 = Fact2<N>::R2;
+    static constexpr int TG = B * R2;                        // threads of a group that own stage-A data
+    static constexpr int GW = (TG + 31) / 32;                // warps per group
+    static constexpr int GT = GW * 32;
+    // groups per CTA: 8 warps (two CTAs per SM) below N = 128, 16 warps (one CTA per SM, so that the planes
+    // owned by the resident CTAs of the plane kernel stay within L2) from there on
+    static constexpr int WPC = N < 128 ? 8 : 16;
+    static constexpr int NWG = (WPC / GW) > 0 ? (WPC / GW) : 1;
+    static constexpr int T = NWG * GT;
+    static constexpr int MINB = (65536 / 128) / T > 0 ? (65536 / 128) / T : 1;   // <= 128 registers: 16 warps per SM
+    static constexpr int TASKS = R1 * B;
+    static constexpr int ROUNDS = (TASKS + GT - 1) / GT;
+    static constexpr int SK = R2 | 1;
+    static constexpr int SB = (R1 * SK) | 1;
+    static constexpr int XCH = B * SB;
+    static constexpr int SMEM_REAL = 2 * N * 16 + 2 * N * 8 + NWG * XCH * 16;
+    static constexpr int SMEM_CPLX = 2 * N * 16 + 2 * N * 16 + NWG * XCH * 16;
+};
+
+template <int GW>
+__device__ __forceinline__ void lean_sync(int grp) {
+    if (GW == 1) __syncwarp();
+    else asm volatile("bar.sync %0, %1;\n" ::"r"(grp + 1), "r"(GW * 32) : "memory");
+}
+
+// One tile.  cur/acc/series point at this thread's first element of the tile, vt/ph at the same grid point
+// of the N_g tables; element n1 of the thread is n1 * estep further.  ktab: this pass's k table (already + 0).
+template <int N, int B, bool CPLX, bool FIRST>
+__device__ __forceinline__ void lean_tile(const LeanArgs& a, int pass, const cd* cur, cd* acc,
+                                          cd* ser, const double* __restrict__ vt, const cd* __restrict__ ph,
+                                          int estep, cd* xch, const cd* twA, const cd* twB, const void* ktab, int grp,
+                                          int gt, int n2, int bA) {
+    using C = LeanCfg<N, B>;
+    constexpr int R1 = C::R1, R2 = C::R2, TG = C::TG, GW = C::GW, GT = C::GT, SK = C::SK, SB = C::SB;
+    constexpr int TASKS = C::TASKS, ROUNDS = C::ROUNDS;
+    const bool actA = gt < TG;
+    const int flags = a.flags[pass], alpha = a.alpha[pass];
+    cd x[R1];
+    cd* xA = xch + bA * SB + n2;
+    if (actA) {
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) x[n1] = __ldcg(cur + n1 * estep);
+        if (CPLX && (flags & F_PRO)) {
+#pragma unroll
+            for (int n1 = 0; n1 < R1; ++n1) x[n1] = cmul(x[n1], __ldg(ph + n1 * estep));
+        }
+        Dft<R1, -1>::run(x);
+        xA[0] = x[0];
+#pragma unroll
+        for (int j = 1; j < R1; ++j) xA[j * SK] = cmul(x[j], twA[j * R2 + n2]);
+    }
+    lean_sync<GW>(grp);
+#pragma unroll
+    for (int rd = 0; rd < ROUNDS; ++rd) {
+        const int task = gt + rd * GT;
+        if (task < TASKS) {
+            const int k1 = task % R1, bB = task / R1;
+            cd* xB = xch + bB * SB + k1 * SK;
+            cd y[R2];
+#pragma unroll
+            for (int m = 0; m < R2; ++m) y[m] = xB[m];
+            Dft<R2, -1>::run(y);
+            if (CPLX) {
+                const cd* kt = reinterpret_cast<const cd*>(ktab) + k1;
+#pragma unroll
+                for (int k2 = 0; k2 < R2; ++k2) y[k2] = cmul(y[k2], kt[R1 * k2]);
+            } else {
+                const double* kt = reinterpret_cast<const double*>(ktab) + k1;
+#pragma unroll
+                for (int k2 = 0; k2 < R2; ++k2) y[k2] = cscale(y[k2], kt[R1 * k2]);
+            }
+            Dft<R2, +1>::run(y);
+            xB[0] = y[0];
+#pragma unroll
+            for (int m = 1; m < R2; ++m) xB[m] = cmulc(y[m], twB[m * R1 + k1]);
+        }
+    }
+    lean_sync<GW>(grp);
+    if (actA) {
+#pragma unroll
+        for (int j = 0; j < R1; ++j) x[j] = xA[j * SK];
+        Dft<R1, +1>::run(x);
+        if (CPLX) {
+            if (flags & F_EPI) {
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) x[n1] = cmul(x[n1], __ldg(ph + n1 * estep));
+            }
+#pragma unroll
+            for (int n1 = 0; n1 < R1; ++n1) __stcg(acc + n1 * estep, x[n1]);
+        } else {
+            const double hs = a.hs;
+            if (FIRST && (flags & (F_VTAB | F_FLUSH))) {
+                // first pass of an operator application: needs the input again (L2 hit) with the potential,
+                // and (every second Chebyshev term) adds the two vectors at hand to the series
+                const double al = (double)alpha, c0 = a.c0, c1 = a.c1;
+                constexpr int CH = (R1 % 4 == 0) ? 4 : ((R1 % 3 == 0) ? 3 : ((R1 % 2 == 0) ? 2 : 1));
+#pragma unroll
+                for (int c = 0; c < R1; c += CH) {
+                    cd vin[CH], ao[CH], so[CH];
+                    double v[CH];
+#pragma unroll
+                    for (int q = 0; q < CH; ++q) {
+                        const int o = (c + q) * estep;
+                        vin[q] = __ldcg(cur + o);
+                        ao[q] = alpha != 0 ? __ldcg(acc + o) : make_double2(0.0, 0.0);
+                        v[q] = (flags & F_VTAB) ? __ldg(vt + o) : 0.0;
+                        so[q] = ((flags & F_FLUSH) && !(flags & F_SINIT)) ? __ldcs(ser + o) : make_double2(0.0, 0.0);
+                    }
+#pragma unroll
+                    for (int q = 0; q < CH; ++q) {
+                        const int n1 = c + q, o = n1 * estep;
+                        if (flags & F_FLUSH)
+                            __stcs(ser + o, make_double2(so[q].x + c0 * ao[q].x + c1 * vin[q].x,
+                                                         so[q].y + c0 * ao[q].y + c1 * vin[q].y));
+                        const double hv = hs * v[q];
+                        __stcg(acc + o, make_double2(hs * x[n1].x + hv * vin[q].x + al * ao[q].x,
+                                                     hs * x[n1].y + hv * vin[q].y + al * ao[q].y));
+                    }
+                }
+            } else if (alpha != 0) {
+                cd ad[R1];
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) ad[n1] = __ldcg(acc + n1 * estep);
+                const double al = (double)alpha;
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1)
+                    __stcg(acc + n1 * estep, make_double2(hs * x[n1].x + al * ad[n1].x, hs * x[n1].y + al * ad[n1].y));
+            } else {
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) __stcg(acc + n1 * estep, cscale(x[n1], hs));
+            }
+        }
+    }
+    lean_sync<GW>(grp);                                       // the exchange buffer is free for the next tile
+}
+
+template <int N, int B, bool CPLX>
+__device__ __forceinline__ void lean_tables(const LeanArgs& a, cd* twA, cd* twB, char* ktab) {
+    using C = LeanCfg<N, B>;
+    for (int i = threadIdx.x; i < N; i += C::T) {
+        twA[i] = a.tw[(i % C::R2) * (i / C::R2)];
+        twB[i] = a.tw[(i / C::R1) * (i % C::R1)];
+    }
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+        for (int k = threadIdx.x; k < N; k += C::T) {
+            if (CPLX) { if (a.kc[p]) reinterpret_cast<cd*>(ktab)[p * N + k] = a.kc[p][k]; }
+            else { if (a.kre[p]) reinterpret_cast<double*>(ktab)[p * N + k] = a.kre[p][k]; }
+        }
+    }
+    __syncthreads();
+}
+
+// One pass along AXIS (0 x, 1 y, 2 z) over all tiles; groups take tiles round robin.
+//   x: tile t = B consecutive rows (rows are contiguous across planes and vectors)
+//   y: tile t = (plane, column block);  z: tile t = (vector, xy block)
+//   CUBE: nx == ny == N as well (compile-time strides)
+template <int N, int B, bool CPLX, int AXIS, bool CUBE>
+__global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) axis_lean_kernel(const LeanArgs a) {
+    using C = LeanCfg<N, B>;
+    constexpr int R2 = C::R2, GT = C::GT, NWG = C::NWG;
+    extern __shared__ __align__(16) char smraw[];
+    cd* twA = reinterpret_cast<cd*>(smraw);
+    cd* twB = twA + N;
+    char* ktab = reinterpret_cast<char*>(twB + N);
+    const int tid = threadIdx.x, grp = tid / GT, gt = tid % GT;
+    cd* xch = reinterpret_cast<cd*>(ktab + 2 * N * (CPLX ? 16 : 8)) + grp * C::XCH;
+    lean_tables<N, B, CPLX>(a, twA, twB, ktab);
+
+    const int nxy = CUBE ? N * N : a.nx * a.ny;
+    const long long ng = (long long)nxy * a.nz;
+    int n2, bA, e0, estep;
+    if (AXIS == 0) { n2 = gt % R2; bA = gt / R2; e0 = bA * a.nx + n2; estep = R2; }
+    else { bA = gt % B; n2 = gt / B; const int sN = (AXIS == 1) ? (CUBE ? N : a.nx) : nxy; e0 = n2 * sN + bA; estep = R2 * sN; }
+    const unsigned stride = gridDim.x * NWG;
+    const unsigned rows_per_vec = (unsigned)(a.ny * a.nz), cb_per_plane = (unsigned)(a.nx / B), blk_per_vec = (unsigned)(nxy / B);
+    for (unsigned t = blockIdx.x * NWG + grp; t < a.ntiles; t += stride) {
+        long long base;
+        int g0;
+        if (AXIS == 0) {
+            base = (long long)t * (B * a.nx);
+            g0 = (int)((t * B) % rows_per_vec) * a.nx;
+        } else if (AXIS == 1) {
+            const unsigned p = t / cb_per_plane, cb = t - p * cb_per_plane;
+            base = (long long)p * nxy + (long long)cb * B;
+            g0 = (int)(p % (unsigned)a.nz) * nxy + (int)cb * B;
+        } else {
+            const unsigned v = t / blk_per_vec, i = t - v * blk_per_vec;
+            base = (long long)v * ng + (long long)i * B;
+            g0 = (int)i * B;
+        }
+        const long long o = base + e0;
+        lean_tile<N, B, CPLX, AXIS == 0>(a, 0, a.cur + o, a.acc + o, a.series + o, a.vtab + g0 + e0, a.phase + g0 + e0, estep,
+                                         xch, twA, twB, ktab, grp, gt, n2, bA);
+    }
+}
+
+// x pass then y pass of whole xy planes (nx == ny == N) in one launch.  A CTA owns planes [pg*G, pg*G + G): its
+// groups do the row tiles of those planes, the CTA synchronises (which also makes the stores visible to the
+// whole CTA), then the column tiles; the transpose goes through L2.  (A barrier-free variant that pipelines
+// planes inside a CTA with shared-memory counters was tried: it needs both a producer and a consumer
+// throttle to bound the planes in flight, keeps more of them live than L2 holds, and was slower.)
+template <int N, int B, bool CPLX>
+__global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) plane_lean_kernel(const LeanArgs a) {
+    using C = LeanCfg<N, B>;
+    constexpr int R2 = C::R2, GT = C::GT, NWG = C::NWG;
+    constexpr unsigned TPP = N / B;
+    constexpr int NXY = N * N;
+    extern __shared__ __align__(16) char smraw[];
+    cd* twA = reinterpret_cast<cd*>(smraw);
+    cd* twB = twA + N;
+    char* ktab = reinterpret_cast<char*>(twB + N);
+    const int tid = threadIdx.x, grp = tid / GT, gt = tid % GT;
+    cd* xch = reinterpret_cast<cd*>(ktab + 2 * N * (CPLX ? 16 : 8)) + grp * C::XCH;
+    lean_tables<N, B, CPLX>(a, twA, twB, ktab);
+    const char* ktab_y = ktab + N * (CPLX ? 16 : 8);
+
+    const int n2x = gt % R2, bAx = gt / R2, e0x = bAx * N + n2x;                 // x: lanes along n
+    const int bAy = gt % B, n2y = gt / B, e0y = n2y * N + bAy;                   // y: lanes along b
+    const unsigned G = (unsigned)a.G;
+    const unsigned ngroups = (a.ntiles + G - 1) / G;
+    for (unsigned pg = blockIdx.x; pg < ngroups; pg += gridDim.x) {
+        const unsigned p0 = pg * G, np = (a.ntiles - p0 < G) ? a.ntiles - p0 : G;
+        for (unsigned q = grp; q < np * TPP; q += NWG) {
+            const unsigned p = p0 + q / TPP, rb = q % TPP;
+            const long long o = (long long)p * NXY + (long long)rb * (B * N) + e0x;
+            const int g = (int)(p % (unsigned)a.nz) * NXY + (int)rb * (B * N) + e0x;
+            lean_tile<N, B, CPLX, true>(a, 0, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g, R2, xch, twA, twB,
+                                        ktab, grp, gt, n2x, bAx);
+        }
+        __syncthreads();                                     // every row tile of the group is stored (to L2)
+        for (unsigned q = grp; q < np * TPP; q += NWG) {
+            const unsigned p = p0 + q / TPP, cb = q % TPP;
+            const long long o = (long long)p * NXY + (long long)cb * B + e0y;
+            const int g = (int)(p % (unsigned)a.nz) * NXY + (int)cb * B + e0y;
+            // the y pass reads what the x pass left in acc; for the complex family cur == acc
+            lean_tile<N, B, CPLX, false>(a, 1, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g, R2 * N, xch, twA,
+                                         twB, ktab_y, grp, gt, n2y, bAy);
+        }
+    }
+}
+
+struct LeanCall {
+    LeanArgs args;
+    int cplx;
+    int kind;                 // 0..2: axis pass along x, y, z; 3: plane pass (x then y); 4: z pass on a cubic grid
+    int ctas_per_sm;          // 0 = as many as fit
+    cudaStream_t stream;
+};
+// returns 0, -(stage*1000 + cudaError) on failure, or 1 if this (N, B) is not instantiated
+typedef int (*lean_launch_fn)(const LeanCall*, int B);
+
+}  // namespace sgw

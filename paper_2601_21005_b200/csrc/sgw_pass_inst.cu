@@ -4,6 +4,7 @@
 
 #include "sgw_plane.cuh"
 #include "sgw_engine.cuh"
+#include "sgw_lean.cuh"
 
 #ifndef SGW_N
 #error "compile with -DSGW_N=<axis length>"
@@ -178,6 +179,58 @@ static int launch_engine_b(const EngCall* c) {
     return e == cudaSuccess ? 0 : -(4000 + (int)e);
 }
 
+
+// ---- lean passes (sgw_lean.cuh) --------------------------------------------------------------------
+template <class K>
+static int lean_launch_kernel(K kern, int threads, size_t smem, long long want_ctas, int ctas_per_sm, const LeanArgs& args,
+                              cudaStream_t stream, int* per_sm_cache) {
+    static int num_sms = 0;
+    if (!num_sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    if (!*per_sm_cache) {
+        cudaError_t e = smem > 48 * 1024 ? cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                                         : cudaSuccess;
+        if (e != cudaSuccess) return -(1000 + (int)e);
+        int n = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, threads, smem);
+        if (e != cudaSuccess) return -(2000 + (int)e);
+        if (n < 1) return -2999;
+        *per_sm_cache = n;
+    }
+    int per_sm = *per_sm_cache;
+    if (ctas_per_sm > 0 && ctas_per_sm < per_sm) per_sm = ctas_per_sm;
+    long long grid = (long long)per_sm * num_sms;
+    if (grid > want_ctas) grid = want_ctas;
+    if (grid <= 0) return 0;
+    kern<<<(unsigned)grid, threads, smem, stream>>>(args);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? 0 : -(4000 + (int)e);
+}
+
+template <int B, bool CPLX>
+static int launch_lean_b(const LeanCall* c) {
+    constexpr int N = SGW_N;
+    using Cfg = LeanCfg<N, B>;
+    const size_t smem = CPLX ? Cfg::SMEM_CPLX : Cfg::SMEM_REAL;
+    static int occ[5] = {0, 0, 0, 0, 0};
+    const long long tiles_ctas = ((long long)c->args.ntiles + Cfg::NWG - 1) / Cfg::NWG;
+    switch (c->kind) {
+        case 0: return lean_launch_kernel(axis_lean_kernel<N, B, CPLX, 0, false>, Cfg::T, smem, tiles_ctas, c->ctas_per_sm, c->args, c->stream, &occ[0]);
+        case 1: return lean_launch_kernel(axis_lean_kernel<N, B, CPLX, 1, false>, Cfg::T, smem, tiles_ctas, c->ctas_per_sm, c->args, c->stream, &occ[1]);
+        case 2: return lean_launch_kernel(axis_lean_kernel<N, B, CPLX, 2, false>, Cfg::T, smem, tiles_ctas, c->ctas_per_sm, c->args, c->stream, &occ[2]);
+        case 4: return lean_launch_kernel(axis_lean_kernel<N, B, CPLX, 2, true>, Cfg::T, smem, tiles_ctas, c->ctas_per_sm, c->args, c->stream, &occ[4]);
+        case 3: {
+            if (N % B) return 1;
+            const long long ngroups = ((long long)c->args.ntiles + c->args.G - 1) / c->args.G;
+            return lean_launch_kernel(plane_lean_kernel<N, B, CPLX>, Cfg::T, smem, ngroups, c->ctas_per_sm, c->args, c->stream, &occ[3]);
+        }
+    }
+    return -1;
+}
+
 }  // namespace sgw
 
 #define SGW_CAT_(a, b) a##b
@@ -213,5 +266,13 @@ extern "C" int SGW_CAT(sgw_eng_launch_, SGW_N)(const sgw::EngCall* c, int B) {
     using namespace sgw;
     if (B == 8) return c->cplx ? launch_engine_b<8, true>(c) : launch_engine_b<8, false>(c);
     if (B == 4) return c->cplx ? launch_engine_b<4, true>(c) : launch_engine_b<4, false>(c);
+    return 1;
+}
+
+// Lean passes: B = pencils per tile (4 or 8).
+extern "C" int SGW_CAT(sgw_lean_launch_, SGW_N)(const sgw::LeanCall* c, int B) {
+    using namespace sgw;
+    if (B == 8) return c->cplx ? launch_lean_b<8, true>(c) : launch_lean_b<8, false>(c);
+    if (B == 4) return c->cplx ? launch_lean_b<4, true>(c) : launch_lean_b<4, false>(c);
     return 1;
 }

@@ -375,3 +375,155 @@ int eng_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb) {
 }
 
 }  // namespace sgw
+
+// =====================================================================================================
+// lean passes (sgw_lean.cuh): the default implementation
+// =====================================================================================================
+namespace {
+
+struct LeanOp {
+    const cd* cur; cd* acc; cd* series;
+    const double* vtab; const cd* phase;
+    double hs, c0, c1;
+    int fx, ax, fy, ay, fz, az;          // flags / alpha of the x, y, z passes
+    bool cplx;
+    const double* kre[3];
+    const cd* kc[3];
+};
+
+int lean_launch(sgw_ctx* c, int axis_n, int kind, const LeanArgs& args, bool cplx, int ctas_per_sm, int prof_tag) {
+    LeanCall call;
+    call.args = args;
+    call.cplx = cplx ? 1 : 0;
+    call.kind = kind;
+    call.ctas_per_sm = ctas_per_sm;
+    call.stream = c->stream;
+    cudaEvent_t e1 = prof_begin(c, prof_tag);
+    const int rc = c->lean[axis_n](&call, c->engB[0]);
+    if (rc != 0)
+        return set_error(rc < 0 ? SGW_ECUDA : SGW_ESIZE,
+                         "lean pass launch failed: stage " + std::to_string((-rc) / 1000) + ": " +
+                             cudaGetErrorString((cudaError_t)((-rc) % 1000)));
+    prof_end(c, e1);
+    c->launches++;
+    return 0;
+}
+
+// true if the fused x+y plane kernel applies: square planes whose CTA-owned groups (cur and acc of every
+// resident CTA's group) stay inside L2
+bool lean_use_plane(const sgw_ctx* c, int* G, int* ctas) {
+    if (c->nx != c->ny) return false;
+    const int n = c->nx, B = c->engB[0];
+    if (n % B) return false;
+    const double plane_bytes = 16.0 * n * n;
+    // 8-warp CTAs (two per SM) below n = 128, 16-warp CTAs (one per SM) above; cur and acc of every resident
+    // CTA's plane group must stay in L2 between the row tiles and the column tiles
+    int per_sm = n < 128 ? 2 : 1;
+    if (c->lean_ctas > 0) per_sm = c->lean_ctas;
+    const int g = c->lean_G > 0 ? c->lean_G : 1;
+    if (2.0 * plane_bytes * g * per_sm * c->num_sms > 100.0e6) return false;
+    *G = g; *ctas = per_sm;
+    return true;
+}
+
+// one operator application over nv vectors: x and y (one launch when the plane kernel applies), then z
+int lean_apply(sgw_ctx* c, int nv, const LeanOp& op, int kind_tag) {
+    const int B = c->engB[0];
+    const long long nxy = (long long)c->nx * c->ny;
+    LeanArgs a;
+    memset(&a, 0, sizeof(a));
+    a.cur = op.cur; a.acc = op.acc; a.series = op.series; a.vtab = op.vtab; a.phase = op.phase;
+    a.hs = op.hs; a.c0 = op.c0; a.c1 = op.c1;
+    a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+    int G = 1, ctas = 0;
+    if (lean_use_plane(c, &G, &ctas)) {
+        a.tw = c->tw[0];
+        a.kre[0] = op.kre[0]; a.kre[1] = op.kre[1]; a.kc[0] = op.kc[0]; a.kc[1] = op.kc[1];
+        a.flags[0] = op.fx; a.alpha[0] = op.ax; a.flags[1] = op.fy; a.alpha[1] = op.ay;
+        a.ntiles = (unsigned)((long long)nv * c->nz);
+        a.G = G;
+        SGW_TRY(lean_launch(c, 0, 3, a, op.cplx, ctas, 1 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_ACC)));
+    } else {
+        a.tw = c->tw[0];
+        a.kre[0] = op.kre[0]; a.kc[0] = op.kc[0]; a.kre[1] = nullptr; a.kc[1] = nullptr;
+        a.flags[0] = op.fx; a.alpha[0] = op.ax;
+        a.ntiles = (unsigned)((long long)nv * c->nz * c->ny / B);
+        SGW_TRY(lean_launch(c, 0, 0, a, op.cplx, 0, 0 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_STORE)));
+        a.tw = c->tw[1];
+        a.kre[0] = op.kre[1]; a.kc[0] = op.kc[1];
+        a.flags[0] = op.fy; a.alpha[0] = op.ay;
+        if (op.cplx) a.cur = op.acc;
+        a.ntiles = (unsigned)((long long)nv * c->nz * (c->nx / B));
+        SGW_TRY(lean_launch(c, 1, 1, a, op.cplx, 0, 1 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_ACC)));
+    }
+    a.tw = c->tw[2];
+    a.cur = op.cplx ? (const cd*)op.acc : op.cur;
+    a.kre[0] = op.kre[2]; a.kc[0] = op.kc[2]; a.kre[1] = nullptr; a.kc[1] = nullptr;
+    a.flags[0] = op.fz; a.alpha[0] = op.az;
+    a.ntiles = (unsigned)((long long)nv * (nxy / B));
+    const bool cube = c->nx == c->ny && c->ny == c->nz;
+    return lean_launch(c, 2, cube ? 4 : 2, a, op.cplx, 0, 2 * K_NKINDS + kind_tag);
+}
+
+}  // namespace
+
+namespace sgw {
+
+// out = (Tx + Ty + Tz + V_loc) in (the KB term is added by the caller)
+int lean_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out) {
+    LeanOp op;
+    memset(&op, 0, sizeof(op));
+    op.cur = in; op.acc = out; op.vtab = c->vloc; op.hs = 1.0;
+    op.fx = c->vloc ? F_VTAB : 0; op.ax = 0; op.fy = 0; op.ay = 1; op.fz = 0; op.az = 1;
+    op.cplx = false;
+    for (int a = 0; a < 3; ++a) op.kre[a] = c->kin[a];
+    return lean_apply(c, nv, op, K_RT_HFIN);
+}
+
+// Chebyshev recurrence, accumulated in place (same scheme as eng_cheb_filter): term n takes cur = phi_{n-1},
+// acc = phi_{n-2} and leaves acc = phi_n = hs (s T + vtab) cur - acc; the series is updated in the x pass of
+// every even term; the tail kernel adds what is pending and writes psi.
+int lean_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* a, double s, int nterms) {
+    const long long ng = c->ng;
+    SGW_TRY(ensure_ws(c, 2));
+    cd *Pb = psi, *Qb = c->ws[0], *Ob = c->ws[1];
+    const bool kb = c->nsphere > 0;
+    const int L = nterms - 1;
+    for (int n = 1; n <= L; ++n) {
+        const bool odd = n & 1;
+        LeanOp op;
+        memset(&op, 0, sizeof(op));
+        op.cur = odd ? Pb : Qb; op.acc = odd ? Qb : Pb; op.series = Ob; op.vtab = c->vtab;
+        op.hs = (n == 1) ? 0.5 : 1.0;
+        op.fx = F_VTAB; op.ax = (n == 1) ? 0 : -1; op.fy = 0; op.ay = 1; op.fz = 0; op.az = 1;
+        if (n >= 2 && !odd) {
+            op.fx |= F_FLUSH;
+            if (n == 2) op.fx |= F_SINIT;
+            op.c0 = a[n - 2]; op.c1 = a[n - 1];
+        }
+        op.cplx = false;
+        for (int ax = 0; ax < 3; ++ax) op.kre[ax] = c->cheb_kin[ax];
+        SGW_TRY(lean_apply(c, nvec, op, K_RT_CHEB));
+        if (kb) SGW_TRY(kb_apply(c, nvec, op.cur, op.acc, 0, s * op.hs));
+    }
+    const bool Lodd = L & 1;
+    const double cL = a[L], cLm1 = Lodd ? a[L - 1] : 0.0;
+    const double cP = Lodd ? cLm1 : cL, cQ = Lodd ? cL : cLm1;
+    const long long n = (long long)nvec * ng;
+    cheb_tail_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(Pb, Pb, Qb, Ob, cP, cQ, L >= 2 ? 1 : 0, n);
+    c->launches++;
+    return check_cuda(cudaGetLastError(), "cheb_tail");
+}
+
+// one split-operator step with the phase table c->phase = exp(-i V dt/2) (R-8)
+int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb) {
+    LeanOp op;
+    memset(&op, 0, sizeof(op));
+    op.cur = psi; op.acc = psi; op.phase = c->phase; op.hs = 1.0;
+    op.fx = kb ? 0 : F_PRO; op.fz = kb ? 0 : F_EPI;
+    op.cplx = true;
+    for (int a = 0; a < 3; ++a) op.kc[a] = c->td_kin[a];
+    return lean_apply(c, nvec, op, K_RT_TD);
+}
+
+}  // namespace sgw

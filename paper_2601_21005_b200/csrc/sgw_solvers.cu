@@ -129,7 +129,7 @@ extern "C" int sgw_apply_H(sgw_ctx* c, int nvec, const void* d_in, void* d_out) 
         const cd* i0 = in + (long long)v0 * c->ng;
         cd* o0 = out + (long long)v0 * c->ng;
         if (c->use_engine) {
-            SGW_TRY(eng_apply_H(c, nv, i0, o0));
+            SGW_TRY(c->use_engine == 2 ? lean_apply_H(c, nv, i0, o0) : eng_apply_H(c, nv, i0, o0));
             SGW_TRY(kb_apply(c, nv, i0, o0, 0, 1.0));
             continue;
         }
@@ -180,7 +180,8 @@ extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* 
         const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
         cd* X0 = (cd*)d_psi + (long long)v0 * ng;
         if (c->use_engine) {
-            SGW_TRY(eng_cheb_filter(c, nv, X0, h_coeffs, s, nterms));
+            SGW_TRY(c->use_engine == 2 ? lean_cheb_filter(c, nv, X0, h_coeffs, s, nterms)
+                                       : eng_cheb_filter(c, nv, X0, h_coeffs, s, nterms));
             continue;
         }
         cd *P1 = c->ws[0], *W = c->ws[1], *O = c->ws[2];
@@ -269,7 +270,7 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             }
             int rp = 1;
             if (c->use_engine) {
-                SGW_TRY(eng_td_step(c, nc, ps, kb));
+                SGW_TRY(c->use_engine == 2 ? lean_td_step(c, nc, ps, kb) : eng_td_step(c, nc, ps, kb));
                 rp = 2;
             } else {
                 rp = run_plane(c, PL_TD, nc, ps, ps, p.pro_phase, false);

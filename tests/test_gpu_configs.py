@@ -1,5 +1,5 @@
-"""GPU parity at the sizes of BASELINE.json's configs, in the launch configuration bench.py times, and
-for the opt-in pass engine (SGW_ENGINE=1).
+"""GPU parity at the sizes of BASELINE.json's configs, in the launch configuration bench.py times, for the
+three pass implementations (SGW_ENGINE=2 lean passes, the default; 0 staged kernels; 1 pass engine).
 
 Full-size oracle runs are only feasible for a few applications, so ("Oracle cost and
 parity coverage"): every config shape gets a single H apply compared element by element on a declared
@@ -38,7 +38,7 @@ def relerr(got, want):
     return float(np.max(np.linalg.norm(got - want, axis=1) / np.linalg.norm(want, axis=1)))
 
 
-@pytest.mark.parametrize("engine", ["0", "1"])
+@pytest.mark.parametrize("engine", ["2", "0", "1"])
 def test_cfg1_bench_configuration_sampled_vectors(api, torch_cuda, oracle, monkeypatch, engine):
     """cfg1 exactly as bench.py runs it (96^3, 64 vectors in one call, max_nvec = 64): the first 33 terms of
     the 512-term coefficient list.  Vectors 0, 37 and 63 of the batch are compared with the oracle."""
@@ -60,7 +60,7 @@ def test_cfg1_bench_configuration_sampled_vectors(api, torch_cuda, oracle, monke
     ctx.close()
 
 
-@pytest.mark.parametrize("engine", ["0", "1"])
+@pytest.mark.parametrize("engine", ["2", "0", "1"])
 def test_cfg2_td_hartree_prefix_all_vectors(api, torch_cuda, oracle, monkeypatch, engine):
     """cfg2 (128^3, 16 vectors): a 9-term filter, then 3 split-operator steps with the Hartree potential
     rebuilt every step from all 16 vectors (prefix of the 2000 steps), every vector compared."""
@@ -85,7 +85,7 @@ def test_cfg2_td_hartree_prefix_all_vectors(api, torch_cuda, oracle, monkeypatch
     ctx.close()
 
 
-@pytest.mark.parametrize("engine", ["0", "1"])
+@pytest.mark.parametrize("engine", ["2"])
 def test_cfg3_shape_apply_H_and_terms_with_kb(api, torch_cuda, oracle, monkeypatch, engine):
     """cfg3 shape (256^3, Si705H300 local + KB projectors): 2 vectors out of the 256; one H apply and a
     4-term filter (3 applications) compared element by element."""
@@ -127,12 +127,13 @@ def test_cfg4_shape_apply_H_and_td_step_with_kb(api, torch_cuda, oracle):
 
 @pytest.mark.parametrize("n,nz,nvec,use_kb", [(32, 32, 4, False), (48, 48, 3, True), (64, 24, 2, True), (24, 12, 5, True),
                                               (12, 12, 2, False)])
-def test_engine_path_small_grids(api, torch_cuda, oracle, monkeypatch, n, nz, nvec, use_kb):
-    """The pass engine (SGW_ENGINE=1) on cubic grids (one dependent launch), non-cubic grids (one launch per
+@pytest.mark.parametrize("engine", ["2", "1"])
+def test_engine_path_small_grids(api, torch_cuda, oracle, monkeypatch, n, nz, nvec, use_kb, engine):
+    """The lean passes and the pass engine on cubic grids (one dependent launch), non-cubic grids (one launch per
     pass) and an axis length that is not a multiple of 8 (4 pencils per tile): H apply, odd and even term
     counts, TD with and without the Hartree rebuild."""
     torch = torch_cuda
-    monkeypatch.setenv("SGW_ENGINE", "1")
+    monkeypatch.setenv("SGW_ENGINE", engine)
     g = W.Grid(n, n, nz, 0.5, 0.5, 0.55)
     rng = np.random.default_rng(7 * n + nz)
     L = np.array(g.box)
@@ -160,5 +161,33 @@ def test_engine_path_small_grids(api, torch_cuda, oracle, monkeypatch, n, nz, nv
         t = torch.from_numpy(psi).cuda()
         ctx.sgw_td_propagate(t, 0.05, 3)
         assert relerr(t.cpu().numpy(), oracle.td_propagate(g, vloc, kbo, psi, 0.05, 3, mode, rs, ld=True)) < TOL_FULL
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
+
+
+@pytest.mark.parametrize("engine", ["2", "0", "1"])
+@pytest.mark.parametrize("n,nvec", [(32, 80), (48, 40)])
+def test_many_planes_per_cta(api, torch_cuda, oracle, monkeypatch, engine, n, nvec):
+    """Enough xy planes (2560 / 1920) that every persistent CTA owns several plane groups and every warp group
+    many tiles: the regime of the bench workload, at a size the oracle finishes in seconds."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_ENGINE", engine)
+    g = W.Grid(n, n, n, 0.5, 0.5, 0.5)
+    rng = np.random.default_rng(n + nvec)
+    centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    psi = rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    emin, emax = W.spectral_bounds(g, vloc, False)
+    coeffs = rng.standard_normal(12)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+    assert relerr(t.cpu().numpy(), oracle.cheb_filter(g, vloc, None, psi, coeffs, emin, emax, ld=True)) < TOL_FULL
+    rs = 2.0 / (nvec * g.dV) * 0.01
+    ctx.sgw_set_td(1, rs)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_td_propagate(t, 0.05, 4)
+    assert relerr(t.cpu().numpy(), oracle.td_propagate(g, vloc, None, psi, 0.05, 4, 1, rs, ld=True)) < TOL_FULL
     assert ctx.sgw_sync_check() == 0
     ctx.close()
