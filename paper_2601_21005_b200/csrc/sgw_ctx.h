@@ -92,7 +92,7 @@ int eng_check_error(sgw_ctx* c);
 // lean-pass implementations (sgw_program.cu)
 int lean_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out);
 int lean_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* h_coeffs, double s, int nterms);
-int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb);
+int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb, bool accumulate_density);
 cudaEvent_t prof_begin(sgw_ctx* c, int tag);
 void prof_end(sgw_ctx* c, cudaEvent_t e1);
 int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau);

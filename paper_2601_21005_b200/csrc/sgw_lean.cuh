@@ -27,6 +27,8 @@ struct LeanArgs {
     cd* series;               // Chebyshev series accumulator (F_FLUSH)
     const double* vtab;       // N_g real table (F_VTAB)
     const cd* phase;          // N_g complex table (F_PRO / F_EPI)
+    double* rho;              // N_g doubles: density accumulator (F_DENS)
+    double dens_scale;
     const cd* tw;             // exp(-2 pi i j / N)
     const double* kre[2];     // real k tables (include 1/N and any scale): [0] first pass, [1] second pass (y of a plane launch)
     const cd* kc[2];          // complex k tables
@@ -37,18 +39,22 @@ struct LeanArgs {
     int G;                    // plane kernel: planes per CTA-owned group
 };
 
-template <int N, int B>
+// warps per CTA of the plane kernel: its resident CTAs own one plane group each, and cur + acc of all of them
+// must stay in L2 between the row tiles and the column tiles (measured: ~87 MB of live planes already
+// misses 38 % of the re-reads; one 12- or 16-warp CTA per SM at N = 96 halves the live planes but was
+// slower: 37.1 / 35.7 against 38.3 G units/s), so from N = 128 on there is one 16-warp CTA per SM
+template <int N> struct PlaneWarps { static constexpr int W = N < 128 ? 8 : 16; };
+
+template <int N, int B, int WPC_ = 8>
 struct LeanCfg {
     static constexpr int R1 = Fact2<N>::R1, R2 = Fact2<N>::R2;
     static constexpr int TG = B * R2;                        // threads of a group that own stage-A data
     static constexpr int GW = (TG + 31) / 32;                // warps per group
     static constexpr int GT = GW * 32;
-    // groups per CTA: 8 warps (two CTAs per SM) below N = 128, 16 warps (one CTA per SM, so that the planes
-    // owned by the resident CTAs of the plane kernel stay within L2) from there on
-    static constexpr int WPC = N < 128 ? 8 : 16;
+    static constexpr int WPC = WPC_;                         // warps per CTA (axis kernels: 8, two CTAs per SM)
     static constexpr int NWG = (WPC / GW) > 0 ? (WPC / GW) : 1;
     static constexpr int T = NWG * GT;
-    static constexpr int MINB = (65536 / 128) / T > 0 ? (65536 / 128) / T : 1;   // <= 128 registers: 16 warps per SM
+    static constexpr int MINB = (65536 / 128) / T > 0 ? (65536 / 128) / T : 1;   // <= 128 registers when two CTAs fit
     static constexpr int TASKS = R1 * B;
     static constexpr int ROUNDS = (TASKS + GT - 1) / GT;
     static constexpr int SK = R2 | 1;
@@ -58,6 +64,27 @@ struct LeanCfg {
     static constexpr int SMEM_CPLX = 2 * N * 16 + 2 * N * 16 + NWG * XCH * 16;
 };
 
+// L2 residency hints.  The plane kernel re-reads in its y pass what its x pass touched a few microseconds
+// earlier, while 2 x 148 planes of two arrays (~87 MB on cfg1) are in flight: x-pass traffic is marked
+// evict_last, everything that will not be touched again before it leaves L2 anyway evict_first.
+enum { H_STREAM = 0, H_KEEP = 1 };
+template <int H>
+__device__ __forceinline__ unsigned long long l2_policy() {
+    unsigned long long pol;
+    if (H == H_KEEP) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(pol));
+    else asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ cd ld_hint(const cd* p, unsigned long long pol) {
+    cd v;
+    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;\n"
+                 : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_hint(cd* p, cd v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;\n" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+
 template <int GW>
 __device__ __forceinline__ void lean_sync(int grp) {
     if (GW == 1) __syncwarp();
@@ -66,21 +93,22 @@ __device__ __forceinline__ void lean_sync(int grp) {
 
 // One tile.  cur/acc/series point at this thread's first element of the tile, vt/ph at the same grid point
 // of the N_g tables; element n1 of the thread is n1 * estep further.  ktab: this pass's k table (already + 0).
-template <int N, int B, bool CPLX, bool FIRST>
+template <int N, int B, int WPC, bool CPLX, bool FIRST, int HIN, int HOUT>
 __device__ __forceinline__ void lean_tile(const LeanArgs& a, int pass, const cd* cur, cd* acc,
                                           cd* ser, const double* __restrict__ vt, const cd* __restrict__ ph,
                                           int estep, cd* xch, const cd* twA, const cd* twB, const void* ktab, int grp,
                                           int gt, int n2, int bA) {
-    using C = LeanCfg<N, B>;
+    using C = LeanCfg<N, B, WPC>;
     constexpr int R1 = C::R1, R2 = C::R2, TG = C::TG, GW = C::GW, GT = C::GT, SK = C::SK, SB = C::SB;
     constexpr int TASKS = C::TASKS, ROUNDS = C::ROUNDS;
     const bool actA = gt < TG;
     const int flags = a.flags[pass], alpha = a.alpha[pass];
+    const unsigned long long pin = l2_policy<HIN>(), pout = l2_policy<HOUT>(), pstream = l2_policy<H_STREAM>();
     cd x[R1];
     cd* xA = xch + bA * SB + n2;
     if (actA) {
 #pragma unroll
-        for (int n1 = 0; n1 < R1; ++n1) x[n1] = __ldcg(cur + n1 * estep);
+        for (int n1 = 0; n1 < R1; ++n1) x[n1] = ld_hint(cur + n1 * estep, pin);
         if (CPLX && (flags & F_PRO)) {
 #pragma unroll
             for (int n1 = 0; n1 < R1; ++n1) x[n1] = cmul(x[n1], __ldg(ph + n1 * estep));
@@ -126,8 +154,16 @@ __device__ __forceinline__ void lean_tile(const LeanArgs& a, int pass, const cd*
 #pragma unroll
                 for (int n1 = 0; n1 < R1; ++n1) x[n1] = cmul(x[n1], __ldg(ph + n1 * estep));
             }
+            if (flags & F_DENS) {
+                // rho += rho_scale |psi|^2 of the finished step, so the next step's Hartree rebuild does
+                // not have to read the vectors again; one FP64 reduction per point and vector
+                double* rp = a.rho + (ph - a.phase);
+                const double ds = a.dens_scale;
 #pragma unroll
-            for (int n1 = 0; n1 < R1; ++n1) __stcg(acc + n1 * estep, x[n1]);
+                for (int n1 = 0; n1 < R1; ++n1) atomicAdd(rp + n1 * estep, ds * (x[n1].x * x[n1].x + x[n1].y * x[n1].y));
+            }
+#pragma unroll
+            for (int n1 = 0; n1 < R1; ++n1) st_hint(acc + n1 * estep, x[n1], pout);
         } else {
             const double hs = a.hs;
             if (FIRST && (flags & (F_VTAB | F_FLUSH))) {
@@ -142,8 +178,8 @@ __device__ __forceinline__ void lean_tile(const LeanArgs& a, int pass, const cd*
 #pragma unroll
                     for (int q = 0; q < CH; ++q) {
                         const int o = (c + q) * estep;
-                        vin[q] = __ldcg(cur + o);
-                        ao[q] = alpha != 0 ? __ldcg(acc + o) : make_double2(0.0, 0.0);
+                        vin[q] = ld_hint(cur + o, pin);
+                        ao[q] = alpha != 0 ? ld_hint(acc + o, pstream) : make_double2(0.0, 0.0);
                         v[q] = (flags & F_VTAB) ? __ldg(vt + o) : 0.0;
                         so[q] = ((flags & F_FLUSH) && !(flags & F_SINIT)) ? __ldcs(ser + o) : make_double2(0.0, 0.0);
                     }
@@ -154,30 +190,30 @@ __device__ __forceinline__ void lean_tile(const LeanArgs& a, int pass, const cd*
                             __stcs(ser + o, make_double2(so[q].x + c0 * ao[q].x + c1 * vin[q].x,
                                                          so[q].y + c0 * ao[q].y + c1 * vin[q].y));
                         const double hv = hs * v[q];
-                        __stcg(acc + o, make_double2(hs * x[n1].x + hv * vin[q].x + al * ao[q].x,
-                                                     hs * x[n1].y + hv * vin[q].y + al * ao[q].y));
+                        st_hint(acc + o, make_double2(hs * x[n1].x + hv * vin[q].x + al * ao[q].x,
+                                                            hs * x[n1].y + hv * vin[q].y + al * ao[q].y), pout);
                     }
                 }
             } else if (alpha != 0) {
                 cd ad[R1];
 #pragma unroll
-                for (int n1 = 0; n1 < R1; ++n1) ad[n1] = __ldcg(acc + n1 * estep);
+                for (int n1 = 0; n1 < R1; ++n1) ad[n1] = ld_hint(acc + n1 * estep, pstream);
                 const double al = (double)alpha;
 #pragma unroll
                 for (int n1 = 0; n1 < R1; ++n1)
-                    __stcg(acc + n1 * estep, make_double2(hs * x[n1].x + al * ad[n1].x, hs * x[n1].y + al * ad[n1].y));
+                    st_hint(acc + n1 * estep, make_double2(hs * x[n1].x + al * ad[n1].x, hs * x[n1].y + al * ad[n1].y), pout);
             } else {
 #pragma unroll
-                for (int n1 = 0; n1 < R1; ++n1) __stcg(acc + n1 * estep, cscale(x[n1], hs));
+                for (int n1 = 0; n1 < R1; ++n1) st_hint(acc + n1 * estep, cscale(x[n1], hs), pout);
             }
         }
     }
     lean_sync<GW>(grp);                                       // the exchange buffer is free for the next tile
 }
 
-template <int N, int B, bool CPLX>
+template <int N, int B, int WPC, bool CPLX>
 __device__ __forceinline__ void lean_tables(const LeanArgs& a, cd* twA, cd* twB, char* ktab) {
-    using C = LeanCfg<N, B>;
+    using C = LeanCfg<N, B, WPC>;
     for (int i = threadIdx.x; i < N; i += C::T) {
         twA[i] = a.tw[(i % C::R2) * (i / C::R2)];
         twB[i] = a.tw[(i / C::R1) * (i % C::R1)];
@@ -206,7 +242,7 @@ __global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) axis_le
     char* ktab = reinterpret_cast<char*>(twB + N);
     const int tid = threadIdx.x, grp = tid / GT, gt = tid % GT;
     cd* xch = reinterpret_cast<cd*>(ktab + 2 * N * (CPLX ? 16 : 8)) + grp * C::XCH;
-    lean_tables<N, B, CPLX>(a, twA, twB, ktab);
+    lean_tables<N, B, 8, CPLX>(a, twA, twB, ktab);
 
     const int nxy = CUBE ? N * N : a.nx * a.ny;
     const long long ng = (long long)nxy * a.nz;
@@ -231,7 +267,7 @@ __global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) axis_le
             g0 = (int)i * B;
         }
         const long long o = base + e0;
-        lean_tile<N, B, CPLX, AXIS == 0>(a, 0, a.cur + o, a.acc + o, a.series + o, a.vtab + g0 + e0, a.phase + g0 + e0, estep,
+        lean_tile<N, B, 8, CPLX, AXIS == 0, H_STREAM, H_STREAM>(a, 0, a.cur + o, a.acc + o, a.series + o, a.vtab + g0 + e0, a.phase + g0 + e0, estep,
                                          xch, twA, twB, ktab, grp, gt, n2, bA);
     }
 }
@@ -242,8 +278,10 @@ __global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) axis_le
 // planes inside a CTA with shared-memory counters was tried: it needs both a producer and a consumer
 // throttle to bound the planes in flight, keeps more of them live than L2 holds, and was slower.)
 template <int N, int B, bool CPLX>
-__global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) plane_lean_kernel(const LeanArgs a) {
-    using C = LeanCfg<N, B>;
+__global__ void __launch_bounds__(LeanCfg<N, B, PlaneWarps<N>::W>::T, LeanCfg<N, B, PlaneWarps<N>::W>::MINB)
+plane_lean_kernel(const LeanArgs a) {
+    constexpr int WPC = PlaneWarps<N>::W;
+    using C = LeanCfg<N, B, WPC>;
     constexpr int R2 = C::R2, GT = C::GT, NWG = C::NWG;
     constexpr unsigned TPP = N / B;
     constexpr int NXY = N * N;
@@ -253,7 +291,7 @@ __global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) plane_l
     char* ktab = reinterpret_cast<char*>(twB + N);
     const int tid = threadIdx.x, grp = tid / GT, gt = tid % GT;
     cd* xch = reinterpret_cast<cd*>(ktab + 2 * N * (CPLX ? 16 : 8)) + grp * C::XCH;
-    lean_tables<N, B, CPLX>(a, twA, twB, ktab);
+    lean_tables<N, B, WPC, CPLX>(a, twA, twB, ktab);
     const char* ktab_y = ktab + N * (CPLX ? 16 : 8);
 
     const int n2x = gt % R2, bAx = gt / R2, e0x = bAx * N + n2x;                 // x: lanes along n
@@ -266,7 +304,7 @@ __global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) plane_l
             const unsigned p = p0 + q / TPP, rb = q % TPP;
             const long long o = (long long)p * NXY + (long long)rb * (B * N) + e0x;
             const int g = (int)(p % (unsigned)a.nz) * NXY + (int)rb * (B * N) + e0x;
-            lean_tile<N, B, CPLX, true>(a, 0, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g, R2, xch, twA, twB,
+            lean_tile<N, B, WPC, CPLX, true, H_KEEP, H_KEEP>(a, 0, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g, R2, xch, twA, twB,
                                         ktab, grp, gt, n2x, bAx);
         }
         __syncthreads();                                     // every row tile of the group is stored (to L2)
@@ -275,7 +313,7 @@ __global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) plane_l
             const long long o = (long long)p * NXY + (long long)cb * B + e0y;
             const int g = (int)(p % (unsigned)a.nz) * NXY + (int)cb * B + e0y;
             // the y pass reads what the x pass left in acc; for the complex family cur == acc
-            lean_tile<N, B, CPLX, false>(a, 1, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g, R2 * N, xch, twA,
+            lean_tile<N, B, WPC, CPLX, false, H_STREAM, H_STREAM>(a, 1, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g, R2 * N, xch, twA,
                                          twB, ktab_y, grp, gt, n2y, bAy);
         }
     }
@@ -284,7 +322,7 @@ __global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) plane_l
 struct LeanCall {
     LeanArgs args;
     int cplx;
-    int kind;                 // 0..2: axis pass along x, y, z; 3: plane pass (x then y); 4: z pass on a cubic grid
+    int kind;                 // 0..2: axis pass along x, y, z; 3: plane pass (x then y); 4 / 5: z / y pass on a cubic grid
     int ctas_per_sm;          // 0 = as many as fit
     cudaStream_t stream;
 };

@@ -384,6 +384,7 @@ namespace {
 struct LeanOp {
     const cd* cur; cd* acc; cd* series;
     const double* vtab; const cd* phase;
+    double* rho; double dens_scale;
     double hs, c0, c1;
     int fx, ax, fy, ay, fz, az;          // flags / alpha of the x, y, z passes
     bool cplx;
@@ -418,7 +419,7 @@ bool lean_use_plane(const sgw_ctx* c, int* G, int* ctas) {
     const double plane_bytes = 16.0 * n * n;
     // 8-warp CTAs (two per SM) below n = 128, 16-warp CTAs (one per SM) above; cur and acc of every resident
     // CTA's plane group must stay in L2 between the row tiles and the column tiles
-    int per_sm = n < 128 ? 2 : 1;
+    int per_sm = n < 128 ? 2 : 1;    // PlaneWarps: 8-warp CTAs below 128, one 16-warp CTA per SM above
     if (c->lean_ctas > 0) per_sm = c->lean_ctas;
     const int g = c->lean_G > 0 ? c->lean_G : 1;
     if (2.0 * plane_bytes * g * per_sm * c->num_sms > 100.0e6) return false;
@@ -427,16 +428,17 @@ bool lean_use_plane(const sgw_ctx* c, int* G, int* ctas) {
 }
 
 // one operator application over nv vectors: x and y (one launch when the plane kernel applies), then z
-int lean_apply(sgw_ctx* c, int nv, const LeanOp& op, int kind_tag) {
+int lean_apply(sgw_ctx* c, int nv, const LeanOp& op, int kind_tag, bool allow_plane = true) {
     const int B = c->engB[0];
     const long long nxy = (long long)c->nx * c->ny;
     LeanArgs a;
     memset(&a, 0, sizeof(a));
     a.cur = op.cur; a.acc = op.acc; a.series = op.series; a.vtab = op.vtab; a.phase = op.phase;
+    a.rho = op.rho; a.dens_scale = op.dens_scale;
     a.hs = op.hs; a.c0 = op.c0; a.c1 = op.c1;
     a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
     int G = 1, ctas = 0;
-    if (lean_use_plane(c, &G, &ctas)) {
+    if (allow_plane && lean_use_plane(c, &G, &ctas)) {
         a.tw = c->tw[0];
         a.kre[0] = op.kre[0]; a.kre[1] = op.kre[1]; a.kc[0] = op.kc[0]; a.kc[1] = op.kc[1];
         a.flags[0] = op.fx; a.alpha[0] = op.ax; a.flags[1] = op.fy; a.alpha[1] = op.ay;
@@ -454,7 +456,8 @@ int lean_apply(sgw_ctx* c, int nv, const LeanOp& op, int kind_tag) {
         a.flags[0] = op.fy; a.alpha[0] = op.ay;
         if (op.cplx) a.cur = op.acc;
         a.ntiles = (unsigned)((long long)nv * c->nz * (c->nx / B));
-        SGW_TRY(lean_launch(c, 1, 1, a, op.cplx, 0, 1 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_ACC)));
+        SGW_TRY(lean_launch(c, 1, (c->nx == c->ny && c->ny == c->nz) ? 5 : 1, a, op.cplx, 0,
+                            1 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_ACC)));
     }
     a.tw = c->tw[2];
     a.cur = op.cplx ? (const cd*)op.acc : op.cur;
@@ -489,22 +492,30 @@ int lean_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* a, double s, i
     cd *Pb = psi, *Qb = c->ws[0], *Ob = c->ws[1];
     const bool kb = c->nsphere > 0;
     const int L = nterms - 1;
-    for (int n = 1; n <= L; ++n) {
-        const bool odd = n & 1;
-        LeanOp op;
-        memset(&op, 0, sizeof(op));
-        op.cur = odd ? Pb : Qb; op.acc = odd ? Qb : Pb; op.series = Ob; op.vtab = c->vtab;
-        op.hs = (n == 1) ? 0.5 : 1.0;
-        op.fx = F_VTAB; op.ax = (n == 1) ? 0 : -1; op.fy = 0; op.ay = 1; op.fz = 0; op.az = 1;
-        if (n >= 2 && !odd) {
-            op.fx |= F_FLUSH;
-            if (n == 2) op.fx |= F_SINIT;
-            op.c0 = a[n - 2]; op.c1 = a[n - 1];
+    // vectors per chunk: 0 = all vectors per term (streaming); c > 0 = run c vectors through all terms before the
+    // next c, with separate x, y, z passes, so that cur and acc of the chunk stay in L2 (SGW_LEAN_CHUNK)
+    int chunk = nvec;
+    { const char* e = getenv("SGW_LEAN_CHUNK"); if (e && atoi(e) > 0 && !kb) chunk = atoi(e) < nvec ? atoi(e) : nvec; }
+    for (int v0 = 0; v0 < nvec; v0 += chunk) {
+        const int nvc = (nvec - v0 < chunk) ? nvec - v0 : chunk;
+        const long long voff = (long long)v0 * ng;
+        for (int n = 1; n <= L; ++n) {
+            const bool odd = n & 1;
+            LeanOp op;
+            memset(&op, 0, sizeof(op));
+            op.cur = (odd ? Pb : Qb) + voff; op.acc = (odd ? Qb : Pb) + voff; op.series = Ob + voff; op.vtab = c->vtab;
+            op.hs = (n == 1) ? 0.5 : 1.0;
+            op.fx = F_VTAB; op.ax = (n == 1) ? 0 : -1; op.fy = 0; op.ay = 1; op.fz = 0; op.az = 1;
+            if (n >= 2 && !odd) {
+                op.fx |= F_FLUSH;
+                if (n == 2) op.fx |= F_SINIT;
+                op.c0 = a[n - 2]; op.c1 = a[n - 1];
+            }
+            op.cplx = false;
+            for (int ax = 0; ax < 3; ++ax) op.kre[ax] = c->cheb_kin[ax];
+            SGW_TRY(lean_apply(c, nvc, op, K_RT_CHEB, chunk == nvec));
+            if (kb) SGW_TRY(kb_apply(c, nvc, op.cur, op.acc, 0, s * op.hs));
         }
-        op.cplx = false;
-        for (int ax = 0; ax < 3; ++ax) op.kre[ax] = c->cheb_kin[ax];
-        SGW_TRY(lean_apply(c, nvec, op, K_RT_CHEB));
-        if (kb) SGW_TRY(kb_apply(c, nvec, op.cur, op.acc, 0, s * op.hs));
     }
     const bool Lodd = L & 1;
     const double cL = a[L], cLm1 = Lodd ? a[L - 1] : 0.0;
@@ -516,11 +527,12 @@ int lean_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* a, double s, i
 }
 
 // one split-operator step with the phase table c->phase = exp(-i V dt/2) (R-8)
-int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb) {
+int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb, bool accumulate_density) {
     LeanOp op;
     memset(&op, 0, sizeof(op));
     op.cur = psi; op.acc = psi; op.phase = c->phase; op.hs = 1.0;
     op.fx = kb ? 0 : F_PRO; op.fz = kb ? 0 : F_EPI;
+    if (accumulate_density && !kb) { op.fz |= F_DENS; op.rho = c->rho; op.dens_scale = c->rho_scale; }
     op.cplx = true;
     for (int a = 0; a < 3; ++a) op.kc[a] = c->td_kin[a];
     return lean_apply(c, nvec, op, K_RT_TD);

@@ -81,10 +81,12 @@ OpParams zero_params() {
 }
 
 // rho = scale * sum |psi|^2 ; V_H by the cut-Coulomb Poisson solve (R-10).  Results in c->vh (and rho/rho2).
-int hartree_into(sgw_ctx* c, int nvec, const cd* psi, double rho_scale, double* rho2) {
+int hartree_into(sgw_ctx* c, int nvec, const cd* psi, double rho_scale, double* rho2, bool rho_ready = false) {
     const long long ng = c->ng;
-    density_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(psi, nvec, ng, rho_scale, c->rho, rho2);
-    SGW_TRY(launched(c, "density"));
+    if (!rho_ready) {          // otherwise c->rho was accumulated by the last pass of the previous step
+        density_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(psi, nvec, ng, rho_scale, c->rho, rho2);
+        SGW_TRY(launched(c, "density"));
+    }
     real_to_complex_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->rho, c->pois, ng);
     SGW_TRY(launched(c, "r2c"));
     OpParams p = zero_params();
@@ -247,10 +249,18 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
         c->td_dt = dt; c->td_kin_valid = true;
     }
     const bool kb = c->nsphere > 0;
+    // lean passes without KB: the last pass of a step accumulates the density of its result (atomics), so only
+    // the first step of a call reads the vectors for the density
+    const bool fuse_density = c->hartree_mode && c->use_engine == 2 && !kb;
     for (int step = 0; step < nsteps; ++step) {
         if (c->hartree_mode || step == 0) {
             const double* vh = nullptr;
-            if (c->hartree_mode) { SGW_TRY(hartree_into(c, nvec, psi, c->rho_scale, nullptr)); vh = c->vh; }
+            if (c->hartree_mode) {
+                SGW_TRY(hartree_into(c, nvec, psi, c->rho_scale, nullptr, fuse_density && step > 0));
+                vh = c->vh;
+                if (fuse_density && step + 1 < nsteps)
+                    SGW_TRY(check_cuda(cudaMemsetAsync(c->rho, 0, ng * sizeof(double), c->stream), "rho reset"));
+            }
             phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, vh, 0.5 * dt, c->phase, ng);
             SGW_TRY(launched(c, "phase"));
         }
@@ -270,7 +280,7 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             }
             int rp = 1;
             if (c->use_engine) {
-                SGW_TRY(c->use_engine == 2 ? lean_td_step(c, nc, ps, kb) : eng_td_step(c, nc, ps, kb));
+                SGW_TRY(c->use_engine == 2 ? lean_td_step(c, nc, ps, kb, fuse_density && step + 1 < nsteps) : eng_td_step(c, nc, ps, kb));
                 rp = 2;
             } else {
                 rp = run_plane(c, PL_TD, nc, ps, ps, p.pro_phase, false);
