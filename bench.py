@@ -27,7 +27,17 @@ from paper_2601_21005_b200 import shard, workloads as W  # noqa: E402
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (z round trip + recurrence on
 # cfg1), from the ncu --set full capture summarised in profiles/r01_v2_cfg1.md: 3.69 GB without and 5.52 GB with
 # the series flush (every third term) -> average per launch
-NCU_TRAFFIC_BYTES = {"z_cheb": (2 * 3.69e9 + 5.52e9) / 3.0, "y_acc": 2.18e9}
+# lean passes (default): x+y plane pass 3.06 GB without and 5.50 GB with the series flush (every second term),
+# z pass 2.67 GB, from profiles/r01_lean_cfg1.md
+NCU_TRAFFIC_BYTES = {"lean": {"y_acc": (3.06e9 + 5.50e9) / 2.0, "z_cheb": 2.67e9},
+                     "v2": {"z_cheb": (2 * 3.69e9 + 5.52e9) / 3.0, "y_acc": 2.18e9}, "engine": {}}
+TRAFFIC_SOURCE = {"lean": "profiles/r01_lean_cfg1.md", "v2": "profiles/r01_v2_cfg1.md", "engine": "profiles/r01_engine_v3_cfg1.md"}
+KERNEL_NAMES = {"lean": {"y_acc": "plane_lean_kernel<96,8,real,8> (x and y round trips of whole planes, recurrence on store)",
+                         "z_cheb": "axis_lean_kernel<96,8,real,z,cube> (z round trip, accumulate)",
+                         "x_store": "axis_lean_kernel<96,8,real,x>"},
+                "v2": {"y_acc": "plane_kernel<96,24> (x+y round trips)",
+                       "z_cheb": "pipe_kernel<96,8,POpCheb> (z round trip + recurrence)"},
+                "engine": {"engine": "engine_kernel<96,8> (all passes)"}}
 METRIC = "grid-pt*vector H-applies/s (Chebyshev filter)"
 UNIT = "grid-pt*vec*H-applies/s"
 WORKLOAD = "cfg1"
@@ -217,8 +227,8 @@ def run_gpu(args):
         names = {0: "x", 1: "y", 2: "z"}
         kinds = ["store", "acc", "hfin", "cheb", "td", "mul3d", "fwd", "inv"]
         passes = {f"{names[a]}_{kinds[k]}": {"launches": n, "ms_total": t_} for (a, k), (n, t_) in prof.items() if n}
-        engine = os.environ.get("SGW_ENGINE", "0") not in ("", "0")
-        if engine or not passes:
+        impl = {"0": "v2", "1": "engine"}.get(os.environ.get("SGW_ENGINE", "2"), "lean")
+        if impl == "engine" or not passes:
             # pass engine: one persistent kernel runs all passes of up to 256 terms; its launch time is the step's
             passes = {"engine": {"launches": max(1, int(launches) // 2), "ms_total": ms}}
         dom = max(passes.items(), key=lambda kv: kv[1]["ms_total"])
@@ -226,6 +236,10 @@ def run_gpu(args):
         series_share = 32.0 / 3.0                                   # series r/w every third term
         bytes_per_unit = {"x_store": 32.0, "y_acc": 48.0, "z_cheb": 64.0 + series_share + 8.0 / nvec,
                           "engine": (96.0 + 16.0 + 8.0 / nvec)}          # engine: per term, all three passes
+        if impl == "lean":
+            # x+y plane pass: read cur and acc, write acc (the x->y transpose goes through L2), series r/w every
+            # second term, potential table; z pass: read cur and acc, write acc
+            bytes_per_unit = {"y_acc": 48.0 + 16.0 + 8.0 / nvec, "z_cheb": 48.0, "x_store": 48.0}
         dn, dv = dom
         units_launch = g.ng * nvec
         if dn == "engine":
@@ -242,16 +256,16 @@ def run_gpu(args):
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{WORKLOAD}: 96^3 grid h=0.45, {w.atoms}-shaped V_loc, {nvec} +-1 vectors per GPU, "
                                    f"{w.nterms}-term sqrt-Fermi-Dirac Chebyshev filter ({napply} H applies)",
-                       "l2": "inputs larger than L2 (each array 906 MB per GPU)", "passes_per_term": 3},
+                       "l2": "inputs larger than L2 (each array 906 MB per GPU)", "passes_per_term": 3,
+                       "launches_per_term": 2 if impl != "engine" else 0},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                     "ms_per_step": ms_e2e / args.steps, "checksum": checksum},
             "gpu_launches": int(launches),
-            "roofline": {"bound": "hbm", "kernel": ("engine_kernel<96,8> (all passes)" if dn == "engine" else
-                                                   {"y_acc": "plane_kernel<96,24> (x+y round trips)",
-                                                    "z_cheb": "pipe_kernel<96,8,POpCheb> (z round trip + recurrence)"}.get(dn, dn)), "achieved": ach, "peak": peak,
-                         "unit": "GB/s", "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(dn),
-                         "traffic_source": "profiles/r01_v2_cfg1.md (ncu --set full, bytes per launch)",
+            "roofline": {"bound": "hbm", "implementation": impl, "kernel": KERNEL_NAMES[impl].get(dn, dn),
+                         "achieved": ach, "peak": peak,
+                         "unit": "GB/s", "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES[impl].get(dn),
+                         "traffic_source": TRAFFIC_SOURCE[impl] + " (ncu --set full, dram bytes per launch)",
                          "algorithmic_bytes_per_launch": bytes_per_unit.get(dn, 32.0) * units_launch, "peak_source": peak_src,
                          "avg_launch_ms": avg_ms, "bytes_per_unit": bytes_per_unit.get(dn, 32.0),
                          "kernel_share_of_step": dv["ms_total"] / ms,

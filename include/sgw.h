@@ -22,10 +22,11 @@
  *  - The library owns only its context (tables, workspace for max_nvec vectors).  Calls with
  *    nvec > max_nvec are processed in sub-batches of max_nvec (vectors are independent in the
  *    filter; in the TD step the density is accumulated over all sub-batches first).
- *  - Two implementations of the fused passes are built in: the default one (one kernel for the x and y
- *    round trips of whole planes, one persistent cp.async-pipelined kernel for z) and a pass engine
- *    (one persistent kernel executing a program of passes with dependency counters), selected with the
- *    environment variable SGW_ENGINE=1 when the context is created.  Both compute the same results.
+ *  - Three implementations of the fused passes are built in and selected by the environment variable
+ *    SGW_ENGINE when the context is created: 2 (default) lean streaming passes (autonomous warp groups,
+ *    register operands, a plane kernel for x+y); 0 staged kernels (cp.async-pipelined operands in shared
+ *    memory); 1 pass engine (one persistent kernel executing a program of passes with dependency counters).
+ *    All compute the same results.
  *  - There is no CPU fallback: without a CUDA device sgw_init_grid fails with SGW_ECUDA.
  */
 #ifndef SGW_H
@@ -47,7 +48,7 @@ typedef struct sgw_ctx sgw_ctx;
 
 /* Create a context for an nx*ny*nz periodic grid with spacings hx,hy,hz (bohr) (N_g =
  * N_x N_y N_z).  k_i = 2 pi m/(N_i h_i), m in [-N_i/2, N_i/2) (R: SURVEY 8(a) a3).  max_nvec
- * sizes the internal workspace (3 complex arrays of max_nvec*N_g, allocated lazily by the first
+ * sizes the internal workspace (2 or 3 complex arrays of max_nvec*N_g, allocated lazily by the first
  * call that needs them).  cuda_stream is a cudaStream_t owned by the caller (NULL = default
  * stream).  *ctx is written on success only. */
 int sgw_init_grid(sgw_ctx** ctx, int nx, int ny, int nz, double hx, double hy, double hz,

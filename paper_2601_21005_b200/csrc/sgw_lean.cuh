@@ -39,12 +39,6 @@ struct LeanArgs {
     int G;                    // plane kernel: planes per CTA-owned group
 };
 
-// warps per CTA of the plane kernel: its resident CTAs own one plane group each, and cur + acc of all of them
-// must stay in L2 between the row tiles and the column tiles (measured: ~87 MB of live planes already
-// misses 38 % of the re-reads; one 12- or 16-warp CTA per SM at N = 96 halves the live planes but was
-// slower: 37.1 / 35.7 against 38.3 G units/s), so from N = 128 on there is one 16-warp CTA per SM
-template <int N> struct PlaneWarps { static constexpr int W = N < 128 ? 8 : 16; };
-
 template <int N, int B, int WPC_ = 8>
 struct LeanCfg {
     static constexpr int R1 = Fact2<N>::R1, R2 = Fact2<N>::R2;
@@ -277,10 +271,8 @@ __global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) axis_le
 // whole CTA), then the column tiles; the transpose goes through L2.  (A barrier-free variant that pipelines
 // planes inside a CTA with shared-memory counters was tried: it needs both a producer and a consumer
 // throttle to bound the planes in flight, keeps more of them live than L2 holds, and was slower.)
-template <int N, int B, bool CPLX>
-__global__ void __launch_bounds__(LeanCfg<N, B, PlaneWarps<N>::W>::T, LeanCfg<N, B, PlaneWarps<N>::W>::MINB)
-plane_lean_kernel(const LeanArgs a) {
-    constexpr int WPC = PlaneWarps<N>::W;
+template <int N, int B, bool CPLX, int WPC>
+__global__ void __launch_bounds__(LeanCfg<N, B, WPC>::T, LeanCfg<N, B, WPC>::MINB) plane_lean_kernel(const LeanArgs a) {
     using C = LeanCfg<N, B, WPC>;
     constexpr int R2 = C::R2, GT = C::GT, NWG = C::NWG;
     constexpr unsigned TPP = N / B;
@@ -324,6 +316,7 @@ struct LeanCall {
     int cplx;
     int kind;                 // 0..2: axis pass along x, y, z; 3: plane pass (x then y); 4 / 5: z / y pass on a cubic grid
     int ctas_per_sm;          // 0 = as many as fit
+    int wpc;                  // plane kernel: warps per CTA, 8 (two CTAs per SM) or 16 (one)
     cudaStream_t stream;
 };
 // returns 0, -(stage*1000 + cudaError) on failure, or 1 if this (N, B) is not instantiated

@@ -215,7 +215,7 @@ static int launch_lean_b(const LeanCall* c) {
     constexpr int N = SGW_N;
     using Cfg = LeanCfg<N, B>;
     const size_t smem = CPLX ? Cfg::SMEM_CPLX : Cfg::SMEM_REAL;
-    static int occ[6] = {0, 0, 0, 0, 0, 0};
+    static int occ[7] = {0, 0, 0, 0, 0, 0, 0};
     const long long tiles_ctas = ((long long)c->args.ntiles + Cfg::NWG - 1) / Cfg::NWG;
     switch (c->kind) {
         case 0: return lean_launch_kernel(axis_lean_kernel<N, B, CPLX, 0, false>, Cfg::T, smem, tiles_ctas, c->ctas_per_sm, c->args, c->stream, &occ[0]);
@@ -225,10 +225,16 @@ static int launch_lean_b(const LeanCall* c) {
         case 4: return lean_launch_kernel(axis_lean_kernel<N, B, CPLX, 2, true>, Cfg::T, smem, tiles_ctas, c->ctas_per_sm, c->args, c->stream, &occ[4]);
         case 3: {
             if (N % B) return 1;
-            using PCfg = LeanCfg<N, B, PlaneWarps<N>::W>;
-            const size_t psmem = CPLX ? PCfg::SMEM_CPLX : PCfg::SMEM_REAL;
             const long long ngroups = ((long long)c->args.ntiles + c->args.G - 1) / c->args.G;
-            return lean_launch_kernel(plane_lean_kernel<N, B, CPLX>, PCfg::T, psmem, ngroups, c->ctas_per_sm, c->args, c->stream, &occ[3]);
+            if (c->wpc == 16) {
+                using PCfg = LeanCfg<N, B, 16>;
+                if (PCfg::T > 1024) return 1;
+                return lean_launch_kernel(plane_lean_kernel<N, B, CPLX, 16>, PCfg::T, CPLX ? PCfg::SMEM_CPLX : PCfg::SMEM_REAL, ngroups,
+                                          c->ctas_per_sm, c->args, c->stream, &occ[6]);
+            }
+            using PCfg = LeanCfg<N, B, 8>;
+            return lean_launch_kernel(plane_lean_kernel<N, B, CPLX, 8>, PCfg::T, CPLX ? PCfg::SMEM_CPLX : PCfg::SMEM_REAL, ngroups,
+                                      c->ctas_per_sm, c->args, c->stream, &occ[3]);
         }
     }
     return -1;

@@ -392,8 +392,9 @@ struct LeanOp {
     const cd* kc[3];
 };
 
-int lean_launch(sgw_ctx* c, int axis_n, int kind, const LeanArgs& args, bool cplx, int ctas_per_sm, int prof_tag) {
+int lean_launch(sgw_ctx* c, int axis_n, int kind, const LeanArgs& args, bool cplx, int ctas_per_sm, int prof_tag, int wpc = 8) {
     LeanCall call;
+    call.wpc = wpc;
     call.args = args;
     call.cplx = cplx ? 1 : 0;
     call.kind = kind;
@@ -412,18 +413,22 @@ int lean_launch(sgw_ctx* c, int axis_n, int kind, const LeanArgs& args, bool cpl
 
 // true if the fused x+y plane kernel applies: square planes whose CTA-owned groups (cur and acc of every
 // resident CTA's group) stay inside L2
-bool lean_use_plane(const sgw_ctx* c, int* G, int* ctas) {
+bool lean_use_plane(const sgw_ctx* c, bool cplx, int* G, int* ctas, int* wpc) {
     if (c->nx != c->ny) return false;
     const int n = c->nx, B = c->engB[0];
     if (n % B) return false;
-    const double plane_bytes = 16.0 * n * n;
-    // 8-warp CTAs (two per SM) below n = 128, 16-warp CTAs (one per SM) above; cur and acc of every resident
-    // CTA's plane group must stay in L2 between the row tiles and the column tiles
-    int per_sm = n < 128 ? 2 : 1;    // PlaneWarps: 8-warp CTAs below 128, one 16-warp CTA per SM above
-    if (c->lean_ctas > 0) per_sm = c->lean_ctas;
+    // bytes the resident CTAs keep live in L2 between their row tiles and their column tiles: cur and acc of
+    // one plane group per CTA (one array for the complex family, which works in place).  Two 8-warp CTAs per SM
+    // overlap each other's barriers and are preferred while that stays under ~90 MB (measured on cfg1: 87 MB
+    // live misses 38 % of the re-reads and is still faster than one CTA per SM); then one 16-warp CTA per SM.
+    const double plane_bytes = 16.0 * n * n * (cplx ? 1.0 : 2.0);
     const int g = c->lean_G > 0 ? c->lean_G : 1;
-    if (2.0 * plane_bytes * g * per_sm * c->num_sms > 100.0e6) return false;
-    *G = g; *ctas = per_sm;
+    int w = 8, per_sm = 2;
+    if (plane_bytes * g * 2 * c->num_sms > 90.0e6) { w = 16; per_sm = 1; }
+    if (c->lean_ctas == 1) { w = 16; per_sm = 1; }
+    if (c->lean_ctas == 2) { w = 8; per_sm = 2; }
+    if (plane_bytes * g * per_sm * c->num_sms > 100.0e6) return false;
+    *G = g; *ctas = per_sm; *wpc = w;
     return true;
 }
 
@@ -437,14 +442,14 @@ int lean_apply(sgw_ctx* c, int nv, const LeanOp& op, int kind_tag, bool allow_pl
     a.rho = op.rho; a.dens_scale = op.dens_scale;
     a.hs = op.hs; a.c0 = op.c0; a.c1 = op.c1;
     a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
-    int G = 1, ctas = 0;
-    if (allow_plane && lean_use_plane(c, &G, &ctas)) {
+    int G = 1, ctas = 0, wpc = 8;
+    if (allow_plane && lean_use_plane(c, op.cplx, &G, &ctas, &wpc)) {
         a.tw = c->tw[0];
         a.kre[0] = op.kre[0]; a.kre[1] = op.kre[1]; a.kc[0] = op.kc[0]; a.kc[1] = op.kc[1];
         a.flags[0] = op.fx; a.alpha[0] = op.ax; a.flags[1] = op.fy; a.alpha[1] = op.ay;
         a.ntiles = (unsigned)((long long)nv * c->nz);
         a.G = G;
-        SGW_TRY(lean_launch(c, 0, 3, a, op.cplx, ctas, 1 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_ACC)));
+        SGW_TRY(lean_launch(c, 0, 3, a, op.cplx, ctas, 1 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_ACC), wpc));
     } else {
         a.tw = c->tw[0];
         a.kre[0] = op.kre[0]; a.kc[0] = op.kc[0]; a.kre[1] = nullptr; a.kc[1] = nullptr;
