@@ -95,6 +95,7 @@ __device__ __forceinline__ void lean_tile(const LeanArgs& a, int pass, const cd*
     using C = LeanCfg<N, B, WPC>;
     constexpr int R1 = C::R1, R2 = C::R2, TG = C::TG, GW = C::GW, GT = C::GT, SK = C::SK, SB = C::SB;
     constexpr int TASKS = C::TASKS, ROUNDS = C::ROUNDS;
+    constexpr bool WCACHE = R2 <= 8;     // stage B keeps its twiddles in registers and applies both directions
     const bool actA = gt < TG;
     const int flags = a.flags[pass], alpha = a.alpha[pass];
     const unsigned long long pin = l2_policy<HIN>(), pout = l2_policy<HOUT>(), pstream = l2_policy<H_STREAM>();
@@ -108,9 +109,14 @@ __device__ __forceinline__ void lean_tile(const LeanArgs& a, int pass, const cd*
             for (int n1 = 0; n1 < R1; ++n1) x[n1] = cmul(x[n1], __ldg(ph + n1 * estep));
         }
         Dft<R1, -1>::run(x);
-        xA[0] = x[0];
+        if (WCACHE) {
 #pragma unroll
-        for (int j = 1; j < R1; ++j) xA[j * SK] = cmul(x[j], twA[j * R2 + n2]);
+            for (int j = 0; j < R1; ++j) xA[j * SK] = x[j];  // the twiddle W^(n2 k1) is applied by stage B
+        } else {
+            xA[0] = x[0];
+#pragma unroll
+            for (int j = 1; j < R1; ++j) xA[j * SK] = cmul(x[j], twA[j * R2 + n2]);
+        }
     }
     lean_sync<GW>(grp);
 #pragma unroll
@@ -119,9 +125,17 @@ __device__ __forceinline__ void lean_tile(const LeanArgs& a, int pass, const cd*
         if (task < TASKS) {
             const int k1 = task % R1, bB = task / R1;
             cd* xB = xch + bB * SB + k1 * SK;
-            cd y[R2];
+            // one twiddle table read serves both directions: forward y[m] *= W^(m k1), inverse y[m] *= conj(W^(m k1))
+            // (small R2 only: for R2 >= 12 the cached twiddles would not fit the register budget)
+            cd y[R2], w[WCACHE ? R2 : 1];
+            y[0] = xB[0];
+            if (WCACHE) {
 #pragma unroll
-            for (int m = 0; m < R2; ++m) y[m] = xB[m];
+                for (int m = 1; m < R2; ++m) { w[m] = twB[m * R1 + k1]; y[m] = cmul(xB[m], w[m]); }
+            } else {
+#pragma unroll
+                for (int m = 1; m < R2; ++m) y[m] = xB[m];
+            }
             Dft<R2, -1>::run(y);
             if (CPLX) {
                 const cd* kt = reinterpret_cast<const cd*>(ktab) + k1;
@@ -135,7 +149,7 @@ __device__ __forceinline__ void lean_tile(const LeanArgs& a, int pass, const cd*
             Dft<R2, +1>::run(y);
             xB[0] = y[0];
 #pragma unroll
-            for (int m = 1; m < R2; ++m) xB[m] = cmulc(y[m], twB[m * R1 + k1]);
+            for (int m = 1; m < R2; ++m) xB[m] = cmulc(y[m], WCACHE ? w[m] : twB[m * R1 + k1]);
         }
     }
     lean_sync<GW>(grp);
