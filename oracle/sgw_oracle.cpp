@@ -21,7 +21,7 @@
 //
 // Pins (tests/test_oracle_*.py): splitmix64 published stream; FFT vs O(N^2) DFT and numpy.fft;
 // plane-wave eigenvalues; dense-H built independently with numpy; eigh brute force; Hartree erf
-// closed form; TD closed forms and order-2 convergence.  "parity unpinned": the TD-Hartree
+// closed form; TD closed forms and order-2 convergence; power-iteration bounds vs dense eigenvalues.  "parity unpinned": the TD-Hartree
 // trajectory and the KB factor NL(tau) inside the propagator beyond unitarity/limit checks
 // (they are defined by the algorithm below, R-8, R-9, R-11).
 #include <cmath>
@@ -325,6 +325,47 @@ void td_batch(const Grid& g, const double* vloc, const KBList& kb, int nvec, dou
 // =============================================================================================
 // C entry points (ctypes).  use_ld != 0 selects the long double instantiation.
 // =============================================================================================
+// ---------------------------------------------------------------------------------------------
+// Spectral bounds by shifted power iteration ("the upper and lower spectral bounds of the
+// Kohn-Sham Hamiltonian ... a shifted power iteration"; R-20 in DESIGN.md fixes the details the
+// paper leaves open).  power(shift, x0): x = x0/|x0|; repeat niter times: y = H x - shift x;
+// lambda = Re<x|y> (Rayleigh quotient of H - shift, |x| = 1); x = y/|y|.  Returns lambda + shift.
+// Run 1 (shift 0, start vector `seed`,0) converges to the eigenvalue of largest magnitude la; run 2
+// (shift la, start vector `seed`,1) to the other end of the spectrum.  Plain sums over grid points.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+T power_iteration(const Grid& g, const double* vloc, const KBList& kb, T shift, int niter, uint64_t seed, uint64_t vec) {
+    const size_t ng = (size_t)g.nx * g.ny * g.nz;
+    std::vector<C<T>> x(ng), y(ng);
+    for (size_t i = 0; i < ng; ++i) x[i] = C<T>((keyed_hash(seed, vec, i) >> 63) ? (T)-1 : (T)1, (T)0);
+    T nrm = 0;
+    for (size_t i = 0; i < ng; ++i) nrm += std::norm(x[i]);
+    nrm = std::sqrt(nrm);
+    for (size_t i = 0; i < ng; ++i) x[i] /= nrm;
+    T lambda = 0;
+    for (int it = 0; it < niter; ++it) {
+        apply_H_one<T>(g, vloc, kb, x.data(), y.data());
+        T a = 0, b = 0;
+        for (size_t i = 0; i < ng; ++i) {
+            y[i] -= shift * x[i];
+            a += x[i].real() * y[i].real() + x[i].imag() * y[i].imag();
+            b += std::norm(y[i]);
+        }
+        lambda = a;
+        const T inv = (T)1 / std::sqrt(b);
+        for (size_t i = 0; i < ng; ++i) x[i] = y[i] * inv;
+    }
+    return lambda + shift;
+}
+
+template <class T>
+void spectral_bounds(const Grid& g, const double* vloc, const KBList& kb, int niter, uint64_t seed, double* emin, double* emax) {
+    const T la = power_iteration<T>(g, vloc, kb, (T)0, niter, seed, 0);
+    const T lb = power_iteration<T>(g, vloc, kb, la, niter, seed, 1);
+    *emin = (double)(la < lb ? la : lb);
+    *emax = (double)(la < lb ? lb : la);
+}
+
 extern "C" {
 
 uint64_t sgwo_splitmix64_next(uint64_t* state) {   // the standard generator: state += gamma; mix
@@ -420,6 +461,13 @@ void sgwo_td_propagate(GRID_ARGS, const double* vloc, KB_ARGS, int nvec, double*
     MK
     if (use_ld) td_batch<long double>(g, vloc, kb, nvec, psi, dt, nsteps, hartree_mode, rho_scale);
     else td_batch<double>(g, vloc, kb, nvec, psi, dt, nsteps, hartree_mode, rho_scale);
+}
+
+void sgwo_spectral_bounds(GRID_ARGS, const double* vloc, KB_ARGS, int niter, uint64_t seed, double* emin, double* emax,
+                          int use_ld) {
+    MK
+    if (use_ld) spectral_bounds<long double>(g, vloc, kb, niter, seed, emin, emax);
+    else spectral_bounds<double>(g, vloc, kb, niter, seed, emin, emax);
 }
 
 void sgwo_norms(int64_t ng, int nvec, const double* psi, double* out) {   // sum_g |psi|^2 (no dV)

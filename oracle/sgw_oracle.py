@@ -142,6 +142,16 @@ def td_propagate(grid, vloc, kb, psi, dt, nsteps, hartree_mode=0, rho_scale=0.0,
     return psi
 
 
+def spectral_bounds(grid, vloc, kb, niter, seed, ld: bool = False):
+    """Shifted power iteration (R-20): returns (E_min, E_max) estimates."""
+    kba, keep = _kb_args(kb)
+    v = None if vloc is None else np.ascontiguousarray(vloc, np.float64)
+    emin, emax = C.c_double(), C.c_double()
+    lib().sgwo_spectral_bounds(*_grid_args(grid), _p(v), *kba, C.c_int(niter), C.c_uint64(seed), C.byref(emin),
+                               C.byref(emax), C.c_int(int(ld)))
+    return emin.value, emax.value
+
+
 def norms(psi):
     psi = _vec(psi)
     out = np.empty(psi.shape[0], np.float64)

@@ -263,3 +263,36 @@ def test_td_hartree_mode_uses_start_of_step_density(oracle):
     # and it stays unitary over several steps (V real at every step)
     c = oracle.td_propagate(g, vloc, None, psi, 0.05, 6, hartree_mode=1, rho_scale=rs)
     assert np.abs(oracle.norms(c) / oracle.norms(psi) - 1).max() < 1e-13
+
+
+# ------------------------------------------------------------------ spectral bounds (NEXT-1)
+def test_power_iteration_bounds_converge_to_dense_extreme_eigenvalues(oracle):
+    """Shifted power iteration (R-20) against numpy's eigvalsh of the independently built dense H:
+    Rayleigh quotients always lie inside the spectrum, tighten with the iteration count, and reach both ends
+    to ~1e-12 of the spectral range after 1600 iterations."""
+    for n, h, with_kb in [(8, 0.7, True), (10, 0.6, False)]:
+        g, vloc, kb, _ = small_problem(n, h, with_kb)
+        H = dense_H(g, vloc, kb)
+        ev = np.linalg.eigvalsh(0.5 * (H + H.conj().T))
+        rng_ = ev[-1] - ev[0]
+        prev = None
+        for niter in (20, 100, 400, 1600):
+            emin, emax = oracle.spectral_bounds(g, vloc, kb, niter, 1234)
+            assert ev[0] - 1e-10 * rng_ <= emin <= emax <= ev[-1] + 1e-10 * rng_
+            if prev is not None:
+                assert emin <= prev[0] + 1e-12 * rng_ and emax >= prev[1] - 1e-12 * rng_
+            prev = (emin, emax)
+        assert abs(prev[0] - ev[0]) < 1e-11 * rng_ and abs(prev[1] - ev[-1]) < 1e-11 * rng_
+        # the analytic bounds the configs use (R-3) enclose the true spectrum
+        lo, hi = W.spectral_bounds(g, vloc, with_kb)
+        assert lo <= ev[0] and ev[-1] <= hi
+    # V = 0: the top of the spectrum is the Nyquist corner, 1/2 sum (pi/h_i)^2, and the bottom is 0
+    g = W.Grid(8, 8, 8, 0.5, 0.6, 0.7)
+    emin, emax = oracle.spectral_bounds(g, np.zeros(g.shape), None, 300, 7)
+    top = 0.5 * sum((math.pi / hh) ** 2 for hh in (0.5, 0.6, 0.7))
+    assert abs(emax - top) < 1e-12 * top and -1e-12 * top <= emin < 1e-4 * top
+    # the long double instantiation agrees
+    g, vloc, kb, _ = small_problem(8, 0.7, True)
+    a = oracle.spectral_bounds(g, vloc, kb, 50, 99)
+    b = oracle.spectral_bounds(g, vloc, kb, 50, 99, ld=True)
+    assert np.allclose(a, b, rtol=1e-12, atol=1e-12)
