@@ -104,6 +104,15 @@ int sgw_set_td(sgw_ctx* ctx, int hartree_mode, double rho_scale);
  * dt may be negative (reverse-time propagation). */
 int sgw_td_propagate(sgw_ctx* ctx, int nvec, void* d_psi, double dt, int nsteps);
 
+/* Spectral bounds of H by shifted power iteration ("the upper and lower spectral bounds of the Kohn-Sham
+ * Hamiltonian ... a shifted power iteration"; R-20).  power(shift, x0): x = x0/|x0|; niter times: y = H x - shift x,
+ * lambda = Re<x|y>, x = y/|y|; result lambda + shift.  Run 1: shift 0 from white-noise vector (seed, 0) gives the
+ * eigenvalue of largest magnitude la; run 2: shift la from vector (seed, 1) gives the other end.  *h_emin / *h_emax
+ * (HOST doubles) receive min / max of the two.  Rayleigh quotients lie inside the spectrum, so the estimates
+ * approach the true bounds from inside; callers pad them.  Uses the V_loc / nonlocal terms currently set.  Reductions
+ * are segmented sums with one atomic per block.  Synchronises the stream (it returns host values). */
+int sgw_spectral_bounds(sgw_ctx* ctx, int niter, uint64_t seed, double* h_emin, double* h_emax);
+
 /* d_out[l] = sum_g |psi_l(g)|^2 (no dV factor), nvec doubles (normalisations as segmented
  * sums with one atomic add per segment).  Test helper. */
 int sgw_norms(sgw_ctx* ctx, int nvec, const void* d_psi, double* d_out);

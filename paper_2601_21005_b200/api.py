@@ -19,7 +19,7 @@ _lib = None
 ERRORS = {-1: "SGW_EINVAL", -2: "SGW_ESIZE", -3: "SGW_ENOMEM", -4: "SGW_ECUDA"}
 EXPORTS = ["sgw_init_grid", "sgw_destroy", "sgw_set_vloc", "sgw_set_nonlocal", "sgw_random_vectors",
            "sgw_apply_H", "sgw_cheb_filter", "sgw_hartree", "sgw_set_td", "sgw_td_propagate", "sgw_norms",
-           "sgw_launch_count", "sgw_last_error", "sgw_sync_check", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get"]
+           "sgw_launch_count", "sgw_last_error", "sgw_sync_check", "sgw_spectral_bounds", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get"]
 
 
 class SGWError(RuntimeError):
@@ -49,6 +49,7 @@ def load():
         lib.sgw_norms.argtypes = [vp, i, vp, vp]
         lib.sgw_launch_count.argtypes = [vp]
         lib.sgw_sync_check.argtypes = [vp]
+        lib.sgw_spectral_bounds.argtypes = [vp, i, u64, C.POINTER(d), C.POINTER(d)]
         lib.sgw_launch_count.restype = i64
         lib.sgw_last_error.restype = C.c_char_p
         lib.sgw_profile_enable.argtypes = [vp, i]
@@ -173,6 +174,11 @@ class Context:
         n, ms = C.c_int64(), C.c_double()
         _check(self.lib.sgw_profile_get(self._h, axis, kind, C.byref(n), C.byref(ms)))
         return n.value, ms.value
+
+    def sgw_spectral_bounds(self, niter, seed):
+        emin, emax = C.c_double(), C.c_double()
+        _check(self.lib.sgw_spectral_bounds(self._h, int(niter), int(seed), C.byref(emin), C.byref(emax)))
+        return emin.value, emax.value
 
     def sgw_sync_check(self):
         _check(self.lib.sgw_sync_check(self._h))

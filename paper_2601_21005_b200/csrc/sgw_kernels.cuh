@@ -111,6 +111,43 @@ static __global__ void norms_kernel(const cd* __restrict__ psi, long long ng, do
     }
 }
 
+// ---- spectral bounds by shifted power iteration (R-20) ------------------------------------
+// y -= shift * x;  red[0] += Re<x|y>,  red[1] += |y|^2   (segmented sums + one atomic per block)
+static __global__ void power_reduce_kernel(const cd* __restrict__ x, cd* __restrict__ y, double shift, long long n,
+                                           double* __restrict__ red) {
+    double a = 0.0, b = 0.0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const cd xv = x[i];
+        cd yv = y[i];
+        yv.x -= shift * xv.x; yv.y -= shift * xv.y;
+        y[i] = yv;
+        a += xv.x * yv.x + xv.y * yv.y;
+        b += yv.x * yv.x + yv.y * yv.y;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, o);
+        b += __shfl_down_sync(0xffffffffu, b, o);
+    }
+    __shared__ double pa[8], pb[8];
+    if ((threadIdx.x & 31) == 0) { pa[threadIdx.x >> 5] = a; pb[threadIdx.x >> 5] = b; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double ta = 0.0, tb = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { ta += pa[w]; tb += pb[w]; }
+        atomicAdd(red, ta);
+        atomicAdd(red + 1, tb);
+    }
+}
+// x = y / sqrt(red[1]);  lambda_out[0] = red[0] (Rayleigh quotient of the normalised x);  then red is cleared by the host
+static __global__ void power_scale_kernel(cd* __restrict__ x, const cd* __restrict__ y, const double* __restrict__ red,
+                                          long long n, double* __restrict__ lambda_out) {
+    const double inv = 1.0 / sqrt(red[1]);
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) lambda_out[0] = red[0];
+    if (i < n) x[i] = cscale(y[i], inv);
+}
+
 // ---- a6: Kleinman-Bylander gather-dot (R-12) --------------------------------------------
 // grid (nsphere, nvec), 128 threads: c[v][s][p] = dV * sum_j beta[j][p] * psi_v[idx[j]]
 template <int NP>

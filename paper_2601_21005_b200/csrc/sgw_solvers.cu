@@ -122,6 +122,44 @@ extern "C" int sgw_norms(sgw_ctx* c, int nvec, const void* d_psi, double* d_out)
     return launched(c, "norms_kernel");
 }
 
+static int power_iteration(sgw_ctx* c, double shift, int niter, uint64_t seed, int vec, double* d_red, double* lambda) {
+    const long long ng = c->ng;
+    cd *x = c->ws[0], *y = c->ws[1];
+    SGW_TRY(sgw_random_vectors(c, seed, vec, 1, x));
+    // |x0|^2 = N_g exactly for +-1 entries: normalise with that
+    scale_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(x, 1.0 / sqrt((double)ng), ng);
+    SGW_TRY(launched(c, "scale"));
+    const unsigned nb = (unsigned)((ng + 256LL * 16 - 1) / (256LL * 16));      // segments of 16 elements per thread
+    for (int it = 0; it < niter; ++it) {
+        SGW_TRY(sgw_apply_H(c, 1, x, y));
+        SGW_TRY(check_cuda(cudaMemsetAsync(d_red, 0, 2 * sizeof(double), c->stream), "memset"));
+        power_reduce_kernel<<<nb, 256, 0, c->stream>>>(x, y, shift, ng, d_red);
+        SGW_TRY(launched(c, "power_reduce"));
+        power_scale_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(x, y, d_red, ng, d_red + 2);
+        SGW_TRY(launched(c, "power_scale"));
+    }
+    double lam = 0.0;
+    SGW_TRY(check_cuda(cudaMemcpyAsync(&lam, d_red + 2, sizeof(double), cudaMemcpyDeviceToHost, c->stream), "read lambda"));
+    SGW_TRY(check_cuda(cudaStreamSynchronize(c->stream), "sync"));
+    *lambda = lam + shift;
+    return SGW_OK;
+}
+
+extern "C" int sgw_spectral_bounds(sgw_ctx* c, int niter, uint64_t seed, double* h_emin, double* h_emax) {
+    if (!c || niter < 1 || !h_emin || !h_emax) return set_error(SGW_EINVAL, "sgw_spectral_bounds: bad argument");
+    SGW_TRY(ensure_ws(c, 2));
+    double* d_red = nullptr;
+    SGW_TRY(check_cuda(cudaMalloc((void**)&d_red, 3 * sizeof(double)), "reduction buffer"));
+    double la = 0.0, lb = 0.0;
+    int rc = power_iteration(c, 0.0, niter, seed, 0, d_red, &la);
+    if (!rc) rc = power_iteration(c, la, niter, seed, 1, d_red, &lb);
+    cudaFree(d_red);
+    if (rc) return rc;
+    *h_emin = la < lb ? la : lb;
+    *h_emax = la < lb ? lb : la;
+    return SGW_OK;
+}
+
 extern "C" int sgw_apply_H(sgw_ctx* c, int nvec, const void* d_in, void* d_out) {
     if (!c || nvec < 0 || (nvec > 0 && (!d_in || !d_out)) || d_in == d_out) return set_error(SGW_EINVAL, "sgw_apply_H: bad argument");
     const cd* in = (const cd*)d_in;

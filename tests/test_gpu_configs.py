@@ -191,3 +191,28 @@ def test_many_planes_per_cta(api, torch_cuda, oracle, monkeypatch, engine, n, nv
     assert relerr(t.cpu().numpy(), oracle.td_propagate(g, vloc, None, psi, 0.05, 4, 1, rs, ld=True)) < TOL_FULL
     assert ctx.sgw_sync_check() == 0
     ctx.close()
+
+
+def test_spectral_bounds_vs_oracle_and_enclosure(api, torch_cuda, oracle):
+    """NEXT-1: shifted power iteration on the GPU against the oracle's (same algorithm, same start
+    vectors), with and without KB projectors, and the enclosure by the analytic bounds the configs use."""
+    torch = torch_cuda
+    for n, use_kb in [(24, True), (32, False)]:
+        g = W.Grid(n, n, n, 0.5, 0.5, 0.5)
+        rng = np.random.default_rng(n)
+        centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+        vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+        kb = W.kb_projectors(g, centers[:2], radius=1.8, sigma=0.7) if use_kb else W.KB.empty()
+        ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, 1)
+        ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+        if kb.nsphere:
+            ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                                 torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+        for niter in (5, 60):
+            emin, emax = ctx.sgw_spectral_bounds(niter, 4242)
+            omin, omax = oracle.spectral_bounds(g, vloc, kb if kb.nsphere else None, niter, 4242, ld=True)
+            span = omax - omin
+            assert abs(emin - omin) < 1e-9 * span and abs(emax - omax) < 1e-9 * span
+        lo, hi = W.spectral_bounds(g, vloc, bool(kb.nsphere))
+        assert lo <= emin <= emax <= hi
+        ctx.close()
