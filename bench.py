@@ -218,9 +218,10 @@ def run_gpu(args):
     e2e_value = shard.whole_job_rate(units_rank, world, args.steps, ms_e2e)
     checksum = float(torch.view_as_real(h_out).abs().sum())
 
-    td = None
+    td, samples = None, None
     if world == 1 and not args.no_td:
         td = run_td(torch, api, dev, stream, args)
+        samples = run_config_samples(torch, api, dev, stream)
 
     if rank == 0:
         peak, peak_src = measured_peaks()
@@ -273,6 +274,7 @@ def run_gpu(args):
                          "term_moved": {"achieved": moved / (ms * 1e-3) / 1e9, "frac": moved / (ms * 1e-3) / 1e9 / peak},
                          "passes": passes},
             "td": td,
+            "other_configs": samples,
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",
                              "sample": f"{cpu_nv} vectors x 32 H applies of the same filter, {WORKLOAD} grid ({cpu_dt:.1f} s)"},
         }
@@ -315,6 +317,48 @@ def run_td(torch, api, dev, stream, args):
     return out
 
 
+def run_config_samples(torch, api, dev, stream):
+    """Short samples of the other BASELINE.json configs (shapes and potentials as specified, fewer vectors / terms /
+    steps, stated per entry): evidence that every config runs on the same kernels, not headline numbers."""
+    out = {}
+    specs = [("cfg0", dict(), 128, 0, "32^3, 4 vectors, all 128 terms (launch-latency bound)"),
+             ("cfg3", dict(nvec=8, nterms=17), 17, 4, "256^3, Si705H300 + KB projectors, 8 of 256 vectors, 16 of 2047 applications, 4 TD-Hartree steps"),
+             ("cfg4", dict(nvec=2, nterms=9), 9, 2, "384^3, Si8381H1620 + KB projectors, 2 of 32 vectors, 8 of 2047 applications, 2 of 500 TD-Hartree steps")]
+    for name, kw, nterms, nsteps, what in specs:
+        w = W.make_workload(name, **kw)
+        ctx = api.context_for(w, max_nvec=w.nvec, stream=stream, device=str(dev))
+        psi0 = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
+        psi = psi0.clone()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        best = None
+        for _ in range(3):
+            psi.copy_(psi0)
+            torch.cuda.synchronize(dev)
+            e0.record(stream)
+            ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
+            e1.record(stream)
+            torch.cuda.synchronize(dev)
+            ms = e0.elapsed_time(e1)
+            best = ms if best is None or ms < best else best
+        entry = {"sample": what, "filter_units_per_s": w.grid.ng * w.nvec * (nterms - 1) / (best * 1e-3), "filter_ms": best}
+        if nsteps:
+            ctx.sgw_set_td(1, w.rho_scale)
+            ctx.sgw_td_propagate(psi, w.dt, 1)
+            torch.cuda.synchronize(dev)
+            e0.record(stream)
+            ctx.sgw_td_propagate(psi, w.dt, nsteps)
+            e1.record(stream)
+            torch.cuda.synchronize(dev)
+            ms = e0.elapsed_time(e1)
+            entry["td_units_per_s"] = w.grid.ng * w.nvec * nsteps / (ms * 1e-3)
+            entry["td_ms_per_step"] = ms / nsteps
+        out[name] = entry
+        ctx.close()
+        del psi, psi0
+        torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -323,7 +367,7 @@ def main():
     ap.add_argument("--impl", default="sgw", choices=["sgw", "reference"])
     ap.add_argument("--nterms", type=int, default=None,
                     help="shorten the filter (profiling runs under ncu only; the default is the config's 512)")
-    ap.add_argument("--no-td", action="store_true", help="skip the TD-step sample (cfg2 shape)")
+    ap.add_argument("--no-td", action="store_true", help="skip the TD-step sample (cfg2) and the short samples of cfg0/cfg3/cfg4")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
