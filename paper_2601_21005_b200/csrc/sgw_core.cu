@@ -260,7 +260,7 @@ extern "C" int sgw_destroy(sgw_ctx* c) {
     }
     cudaFree(c->vloc); cudaFree(c->vtab); cudaFree(c->vk3d); cudaFree(c->sph_ptr); cudaFree(c->sph_idx);
     cudaFree(c->beta); cudaFree(c->D); cudaFree(c->kbc); cudaFree(c->pois); cudaFree(c->rho); cudaFree(c->vh);
-    cudaFree(c->phase); cudaFree(c->d_segs); cudaFree(c->d_cnt); cudaFree(c->d_err);
+    cudaFree(c->phase); cudaFree(c->phase_last); cudaFree(c->vprev); cudaFree(c->d_segs); cudaFree(c->d_cnt); cudaFree(c->d_err);
     delete c;
     return SGW_OK;
 }
@@ -314,7 +314,7 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     c->vloc = nullptr; c->vtab = nullptr; c->vk3d = nullptr;
     c->nsphere = 0; c->nproj = 0; c->sph_ptr = nullptr; c->sph_idx = nullptr; c->beta = nullptr; c->D = nullptr;
     c->kbc = nullptr; c->kbc_cap = 0;
-    c->pois = nullptr; c->rho = nullptr; c->vh = nullptr; c->phase = nullptr;
+    c->pois = nullptr; c->rho = nullptr; c->vh = nullptr; c->phase = nullptr; c->phase_last = nullptr; c->vprev = nullptr;
     c->hartree_mode = 0; c->rho_scale = 0; c->launches = 0;
     c->prof_on = false; c->prof_used = 0;
     { const char* e = getenv("SGW_L2_CHUNK"); c->l2_chunk = e ? atoi(e) : 0; }

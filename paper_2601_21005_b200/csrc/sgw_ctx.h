@@ -47,7 +47,9 @@ struct sgw_ctx {
     sgw::cd* pois;                           // N_g complex scratch for the Poisson solve
     double* rho;
     double* vh;
-    sgw::cd* phase;                          // exp(-i V dt/2), N_g
+    sgw::cd* phase;                          // exp(-i V dt/2), N_g (merged table of two half steps in the lean TD path)
+    sgw::cd* phase_last;                     // closing exp(-i V dt/2) of the last step of a call (lean TD path, lazy)
+    double* vprev;                           // total potential of the previous step (lean TD path, lazy)
     int hartree_mode;
     double rho_scale;
     int64_t launches;
@@ -92,7 +94,7 @@ int eng_check_error(sgw_ctx* c);
 // lean-pass implementations (sgw_program.cu)
 int lean_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out);
 int lean_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* h_coeffs, double s, int nterms);
-int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb, bool accumulate_density);
+int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb, bool accumulate_density, bool merged, bool last);
 cudaEvent_t prof_begin(sgw_ctx* c, int tag);
 void prof_end(sgw_ctx* c, cudaEvent_t e1);
 int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau);

@@ -65,6 +65,26 @@ static __global__ void phase_kernel(const double* __restrict__ vloc, const doubl
     phase[i] = make_double2(c, -s);
 }
 
+// Merged half-step phases for consecutive split-operator steps (R-8): the closing factor exp(-i V_{n-1} dt/2) of
+// step n-1 and the opening factor exp(-i V_n dt/2) of step n are applied together on load in step n:
+//   table[g] = exp(-i (V_n + V_{n-1}) half_dt)   (first step of a call: exp(-i V_n half_dt));   vprev <- V_n
+//   last[g]  = exp(-i V_n half_dt)               (only for the last step of a call, applied on store)
+static __global__ void phase_merge_kernel(const double* __restrict__ vloc, const double* __restrict__ vh, double* __restrict__ vprev,
+                                          double half_dt, int first, cd* __restrict__ table, cd* __restrict__ last, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double v = vloc ? vloc[i] : 0.0;
+    if (vh) v += vh[i];
+    double s, c;
+    sincos((first ? v : v + vprev[i]) * half_dt, &s, &c);
+    table[i] = make_double2(c, -s);
+    vprev[i] = v;
+    if (last) {
+        sincos(v * half_dt, &s, &c);
+        last[i] = make_double2(c, -s);
+    }
+}
+
 // psi[v][g] *= phase[g]
 static __global__ void apply_phase_kernel(cd* __restrict__ psi, const cd* __restrict__ phase, long long ng) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;

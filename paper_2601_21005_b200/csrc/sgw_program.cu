@@ -383,7 +383,7 @@ namespace {
 
 struct LeanOp {
     const cd* cur; cd* acc; cd* series;
-    const double* vtab; const cd* phase;
+    const double* vtab; const cd* phase; const cd* phase_z;
     double* rho; double dens_scale;
     double hs, c0, c1;
     int fx, ax, fy, ay, fz, az;          // flags / alpha of the x, y, z passes
@@ -465,6 +465,7 @@ int lean_apply(sgw_ctx* c, int nv, const LeanOp& op, int kind_tag, bool allow_pl
                             1 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_ACC)));
     }
     a.tw = c->tw[2];
+    if (op.phase_z) a.phase = op.phase_z;
     a.cur = op.cplx ? (const cd*)op.acc : op.cur;
     a.kre[0] = op.kre[2]; a.kc[0] = op.kc[2]; a.kre[1] = nullptr; a.kc[1] = nullptr;
     a.flags[0] = op.fz; a.alpha[0] = op.az;
@@ -532,11 +533,17 @@ int lean_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* a, double s, i
 }
 
 // one split-operator step with the phase table c->phase = exp(-i V dt/2) (R-8)
-int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb, bool accumulate_density) {
+// merged: c->phase holds the product of the previous step's closing and this step's opening half-step factor, and
+// only the last step of a call applies a closing factor (c->phase_last) on store
+int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb, bool accumulate_density, bool merged, bool last) {
     LeanOp op;
     memset(&op, 0, sizeof(op));
     op.cur = psi; op.acc = psi; op.phase = c->phase; op.hs = 1.0;
     op.fx = kb ? 0 : F_PRO; op.fz = kb ? 0 : F_EPI;
+    if (merged && !kb) {
+        if (last) op.phase_z = c->phase_last;
+        else op.fz = 0;
+    }
     if (accumulate_density && !kb) { op.fz |= F_DENS; op.rho = c->rho; op.dens_scale = c->rho_scale; }
     op.cplx = true;
     for (int a = 0; a < 3; ++a) op.kc[a] = c->td_kin[a];

@@ -290,6 +290,12 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
     // lean passes without KB: the last pass of a step accumulates the density of its result (atomics), so only
     // the first step of a call reads the vectors for the density
     const bool fuse_density = c->hartree_mode && c->use_engine == 2 && !kb;
+    // lean passes without KB: consecutive half-step phases are merged into one table applied on load (R-8)
+    const bool merged = c->use_engine == 2 && !kb;
+    if (merged && !c->vprev) {
+        SGW_TRY(check_cuda(cudaMalloc((void**)&c->vprev, ng * sizeof(double)), "vprev"));
+        SGW_TRY(check_cuda(cudaMalloc((void**)&c->phase_last, ng * sizeof(cd)), "phase_last"));
+    }
     for (int step = 0; step < nsteps; ++step) {
         if (c->hartree_mode || step == 0) {
             const double* vh = nullptr;
@@ -299,8 +305,18 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
                 if (fuse_density && step + 1 < nsteps)
                     SGW_TRY(check_cuda(cudaMemsetAsync(c->rho, 0, ng * sizeof(double), c->stream), "rho reset"));
             }
-            phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, vh, 0.5 * dt, c->phase, ng);
-            SGW_TRY(launched(c, "phase"));
+            if (!merged) {
+                phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, vh, 0.5 * dt, c->phase, ng);
+                SGW_TRY(launched(c, "phase"));
+            }
+        }
+        const bool last = step + 1 == nsteps;
+        if (merged && (c->hartree_mode || step <= 1 || last)) {
+            // frozen V: the merged table is exp(-i V dt/2) in step 0 and exp(-i V dt) from step 1 on
+            phase_merge_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, c->hartree_mode ? c->vh : nullptr, c->vprev,
+                                                                            0.5 * dt, step == 0 ? 1 : 0, c->phase,
+                                                                            last ? c->phase_last : nullptr, ng);
+            SGW_TRY(launched(c, "phase_merge"));
         }
         const int chunk = (!kb && c->l2_chunk > 0 && c->l2_chunk < nvec) ? c->l2_chunk : nvec;
         for (int cv = 0; cv < nvec; cv += chunk) {            // chunks small enough to stay in L2 across the 3 passes
@@ -318,7 +334,7 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             }
             int rp = 1;
             if (c->use_engine) {
-                SGW_TRY(c->use_engine == 2 ? lean_td_step(c, nc, ps, kb, fuse_density && step + 1 < nsteps) : eng_td_step(c, nc, ps, kb));
+                SGW_TRY(c->use_engine == 2 ? lean_td_step(c, nc, ps, kb, fuse_density && step + 1 < nsteps, merged, last) : eng_td_step(c, nc, ps, kb));
                 rp = 2;
             } else {
                 rp = run_plane(c, PL_TD, nc, ps, ps, p.pro_phase, false);
