@@ -69,12 +69,13 @@ static __global__ void phase_kernel(const double* __restrict__ vloc, const doubl
 // step n-1 and the opening factor exp(-i V_n dt/2) of step n are applied together on load in step n:
 //   table[g] = exp(-i (V_n + V_{n-1}) half_dt)   (first step of a call: exp(-i V_n half_dt));   vprev <- V_n
 //   last[g]  = exp(-i V_n half_dt)               (only for the last step of a call, applied on store)
-static __global__ void phase_merge_kernel(const double* __restrict__ vloc, const double* __restrict__ vh, double* __restrict__ vprev,
+// vh_c: the Hartree potential as the real part of the Poisson solve's complex result (or NULL)
+static __global__ void phase_merge_kernel(const double* __restrict__ vloc, const cd* __restrict__ vh_c, double* __restrict__ vprev,
                                           double half_dt, int first, cd* __restrict__ table, cd* __restrict__ last, long long n) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double v = vloc ? vloc[i] : 0.0;
-    if (vh) v += vh[i];
+    if (vh_c) v += vh_c[i].x;
     double s, c;
     sincos((first ? v : v + vprev[i]) * half_dt, &s, &c);
     table[i] = make_double2(c, -s);

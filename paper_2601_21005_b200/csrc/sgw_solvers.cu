@@ -81,7 +81,8 @@ OpParams zero_params() {
 }
 
 // rho = scale * sum |psi|^2 ; V_H by the cut-Coulomb Poisson solve (R-10).  Results in c->vh (and rho/rho2).
-int hartree_into(sgw_ctx* c, int nvec, const cd* psi, double rho_scale, double* rho2, bool rho_ready = false) {
+int hartree_into(sgw_ctx* c, int nvec, const cd* psi, double rho_scale, double* rho2, bool rho_ready = false,
+                 bool keep_complex = false) {
     const long long ng = c->ng;
     if (!rho_ready) {          // otherwise c->rho was accumulated by the last pass of the previous step
         density_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(psi, nvec, ng, rho_scale, c->rho, rho2);
@@ -98,6 +99,7 @@ int hartree_into(sgw_ctx* c, int nvec, const cd* psi, double rho_scale, double* 
     p.mul3d = nullptr;
     SGW_TRY(run_pass(c, 1, K_INV, 1, c->pois, p));
     SGW_TRY(run_pass(c, 0, K_INV, 1, c->pois, p));
+    if (keep_complex) return 0;      // the caller reads V_H as the real part of c->pois
     complex_to_real_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->pois, c->vh, ng);
     return launched(c, "c2r");
 }
@@ -300,7 +302,7 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
         if (c->hartree_mode || step == 0) {
             const double* vh = nullptr;
             if (c->hartree_mode) {
-                SGW_TRY(hartree_into(c, nvec, psi, c->rho_scale, nullptr, fuse_density && step > 0));
+                SGW_TRY(hartree_into(c, nvec, psi, c->rho_scale, nullptr, fuse_density && step > 0, merged));
                 vh = c->vh;
                 if (fuse_density && step + 1 < nsteps)
                     SGW_TRY(check_cuda(cudaMemsetAsync(c->rho, 0, ng * sizeof(double), c->stream), "rho reset"));
@@ -313,7 +315,7 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
         const bool last = step + 1 == nsteps;
         if (merged && (c->hartree_mode || step <= 1 || last)) {
             // frozen V: the merged table is exp(-i V dt/2) in step 0 and exp(-i V dt) from step 1 on
-            phase_merge_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, c->hartree_mode ? c->vh : nullptr, c->vprev,
+            phase_merge_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, c->hartree_mode ? c->pois : nullptr, c->vprev,
                                                                             0.5 * dt, step == 0 ? 1 : 0, c->phase,
                                                                             last ? c->phase_last : nullptr, ng);
             SGW_TRY(launched(c, "phase_merge"));
