@@ -97,6 +97,7 @@ int lean_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* h_coeffs, doub
 int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb, bool accumulate_density, bool merged, bool last);
 cudaEvent_t prof_begin(sgw_ctx* c, int tag);
 void prof_end(sgw_ctx* c, cudaEvent_t e1);
-int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau);
+int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau, const cd* phase = nullptr,
+             int fold = 0);
 int ensure_ws(sgw_ctx* c, int n);
 }  // namespace sgw

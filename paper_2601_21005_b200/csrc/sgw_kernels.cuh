@@ -176,14 +176,19 @@ static __global__ void __launch_bounds__(128) kb_project_kernel(const cd* __rest
                                                                  const int64_t* __restrict__ ptr,
                                                                  const int32_t* __restrict__ idx,
                                                                  const double* __restrict__ beta, double dV,
-                                                                 cd* __restrict__ cout, int nsphere) {
+                                                                 cd* __restrict__ cout, int nsphere,
+                                                                 const cd* __restrict__ phase = nullptr, int phase_conj = 0) {
     const int s = blockIdx.x, v = blockIdx.y;
     const cd* p = psi + (long long)v * ng;
     double ar[NP], ai[NP];
 #pragma unroll
     for (int q = 0; q < NP; ++q) ar[q] = ai[q] = 0.0;
     for (int64_t j = ptr[s] + threadIdx.x; j < ptr[s + 1]; j += blockDim.x) {
-        const cd a = p[idx[j]];
+        cd a = p[idx[j]];
+        if (phase) {               // the projections are those of phase * psi (or conj(phase) * psi): see sgw_td_propagate
+            const cd ph = phase[idx[j]];
+            a = phase_conj ? cmulc(a, ph) : cmul(a, ph);
+        }
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
             const double b = beta[j * NP + q];
@@ -220,7 +225,8 @@ static __global__ void __launch_bounds__(128) kb_scatter_kernel(cd* __restrict__
                                                                  const double* __restrict__ beta,
                                                                  const double* __restrict__ D,
                                                                  const cd* __restrict__ cin, int nsphere, int mode,
-                                                                 double scale_or_tau) {
+                                                                 double scale_or_tau, const cd* __restrict__ phase = nullptr,
+                                                                 int phase_conj = 0) {
     const int s = blockIdx.x, v = blockIdx.y;
     __shared__ cd f[NP];
     if (threadIdx.x < NP) {
@@ -245,6 +251,11 @@ static __global__ void __launch_bounds__(128) kb_scatter_kernel(cd* __restrict__
             im += b * f[q].y;
         }
         const long long g = idx[j];
+        if (phase) {               // the contribution is added to phase^-1 * (...) or phase * (...): |phase| = 1
+            const cd ph = phase[g];
+            const cd t = phase_conj ? cmulc(make_double2(re, im), ph) : cmul(make_double2(re, im), ph);
+            re = t.x; im = t.y;
+        }
         atomicAdd(out + 2 * g, re);
         atomicAdd(out + 2 * g + 1, im);
     }

@@ -45,30 +45,33 @@ int ensure_kbc(sgw_ctx* c, int nvec) {
 }
 
 template <int NP>
-int kb_apply_np(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau) {
+int kb_apply_np(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau, const cd* phase, int fold) {
     dim3 grid(c->nsphere, nvec);
     const double dV = c->hx * c->hy * c->hz;
-    kb_project_kernel<NP><<<grid, 128, 0, c->stream>>>(src, c->ng, c->sph_ptr, c->sph_idx, c->beta, dV, c->kbc, c->nsphere);
+    // fold = +1: projections of phase*src, contribution times conj(phase)  (opening half step: the pass multiplies by phase on load)
+    // fold = -1: projections of conj(phase)*src, contribution times phase  (closing half step: the pass multiplied by phase on store)
+    kb_project_kernel<NP><<<grid, 128, 0, c->stream>>>(src, c->ng, c->sph_ptr, c->sph_idx, c->beta, dV, c->kbc, c->nsphere,
+                                                       fold ? phase : nullptr, fold < 0 ? 1 : 0);
     SGW_TRY(launched(c, "kb_project"));
     kb_scatter_kernel<NP><<<grid, 128, 0, c->stream>>>(dst, c->ng, c->sph_ptr, c->sph_idx, c->beta, c->D, c->kbc,
-                                                       c->nsphere, mode, scale_or_tau);
+                                                       c->nsphere, mode, scale_or_tau, fold ? phase : nullptr, fold > 0 ? 1 : 0);
     return launched(c, "kb_scatter");
 }
 
 // dst += sum beta f <beta|src>, all projections taken from src before any scatter (R-11)
 }  // namespace
-int sgw::kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau) {
+int sgw::kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau, const cd* phase, int fold) {
     if (c->nsphere == 0) return 0;
     SGW_TRY(ensure_kbc(c, nvec));
     switch (c->nproj) {
-        case 1: return kb_apply_np<1>(c, nvec, src, dst, mode, scale_or_tau);
-        case 2: return kb_apply_np<2>(c, nvec, src, dst, mode, scale_or_tau);
-        case 3: return kb_apply_np<3>(c, nvec, src, dst, mode, scale_or_tau);
-        case 4: return kb_apply_np<4>(c, nvec, src, dst, mode, scale_or_tau);
-        case 5: return kb_apply_np<5>(c, nvec, src, dst, mode, scale_or_tau);
-        case 6: return kb_apply_np<6>(c, nvec, src, dst, mode, scale_or_tau);
-        case 7: return kb_apply_np<7>(c, nvec, src, dst, mode, scale_or_tau);
-        case 8: return kb_apply_np<8>(c, nvec, src, dst, mode, scale_or_tau);
+        case 1: return kb_apply_np<1>(c, nvec, src, dst, mode, scale_or_tau, phase, fold);
+        case 2: return kb_apply_np<2>(c, nvec, src, dst, mode, scale_or_tau, phase, fold);
+        case 3: return kb_apply_np<3>(c, nvec, src, dst, mode, scale_or_tau, phase, fold);
+        case 4: return kb_apply_np<4>(c, nvec, src, dst, mode, scale_or_tau, phase, fold);
+        case 5: return kb_apply_np<5>(c, nvec, src, dst, mode, scale_or_tau, phase, fold);
+        case 6: return kb_apply_np<6>(c, nvec, src, dst, mode, scale_or_tau, phase, fold);
+        case 7: return kb_apply_np<7>(c, nvec, src, dst, mode, scale_or_tau, phase, fold);
+        case 8: return kb_apply_np<8>(c, nvec, src, dst, mode, scale_or_tau, phase, fold);
     }
     return set_error(SGW_EINVAL, "bad nproj");
 }
@@ -326,7 +329,13 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             cd* ps = psi + (long long)cv * ng;
             OpParams p = zero_params();
             p.out = ps;
-            if (kb) {
+            // lean passes with KB: the potential phases stay fused in the passes (on load in x, on store in z); the
+            // KB factors, which sit between them, are conjugated by the phase at their sphere points instead:
+            //   P (psi + conj(P) S[P psi]) = P psi + S[P psi]   and   P psi3 + P S[conj(P) (P psi3)] = P (psi3 + S[psi3])
+            const bool kb_fold = kb && c->use_engine == 2;
+            if (kb_fold) {
+                SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, +1));
+            } else if (kb) {
                 dim3 g2(blocks_for(ng, 256), nc);
                 apply_phase_kernel<<<g2, 256, 0, c->stream>>>(ps, c->phase, ng);
                 SGW_TRY(launched(c, "apply_phase"));
@@ -336,7 +345,8 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             }
             int rp = 1;
             if (c->use_engine) {
-                SGW_TRY(c->use_engine == 2 ? lean_td_step(c, nc, ps, kb, fuse_density && step + 1 < nsteps, merged, last) : eng_td_step(c, nc, ps, kb));
+                SGW_TRY(c->use_engine == 2 ? lean_td_step(c, nc, ps, kb && !kb_fold, fuse_density && step + 1 < nsteps, merged, last)
+                                           : eng_td_step(c, nc, ps, kb));
                 rp = 2;
             } else {
                 rp = run_plane(c, PL_TD, nc, ps, ps, p.pro_phase, false);
@@ -352,7 +362,9 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             p.mul_c = c->td_kin[2];
             if (!kb) p.epi_phase = c->phase;
             if (rp != 2) SGW_TRY(run_pass(c, 2, K_RT_TD, nc, ps, p));
-            if (kb) {
+            if (kb_fold) {
+                SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, -1));
+            } else if (kb) {
                 SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt));
                 dim3 g2(blocks_for(ng, 256), nc);
                 apply_phase_kernel<<<g2, 256, 0, c->stream>>>(ps, c->phase, ng);
