@@ -216,3 +216,32 @@ def test_spectral_bounds_vs_oracle_and_enclosure(api, torch_cuda, oracle):
         lo, hi = W.spectral_bounds(g, vloc, bool(kb.nsphere))
         assert lo <= emin <= emax <= hi
         ctx.close()
+
+
+@pytest.mark.parametrize("G,ctas", [("2", "2"), ("3", "1"), ("1", "1")])
+def test_lean_plane_kernel_group_and_cta_variants(api, torch_cuda, oracle, monkeypatch, G, ctas):
+    """The lean plane kernel with several planes per CTA-owned group (ragged last group: 5 * 32 planes is not a
+    multiple of 3) and with the one-CTA-per-SM (16-warp) variant, against the oracle."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_ENGINE", "2")
+    monkeypatch.setenv("SGW_LEAN_G", G)
+    monkeypatch.setenv("SGW_LEAN_CTAS", ctas)
+    n, nvec = 32, 5
+    g = W.Grid(n, n, n, 0.5, 0.5, 0.5)
+    rng = np.random.default_rng(11)
+    centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    psi = rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    emin, emax = W.spectral_bounds(g, vloc, False)
+    coeffs = rng.standard_normal(7)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+    assert relerr(t.cpu().numpy(), oracle.cheb_filter(g, vloc, None, psi, coeffs, emin, emax, ld=True)) < TOL_FULL
+    ctx.sgw_set_td(1, 2.0 / (nvec * g.dV) * 0.01)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_td_propagate(t, 0.05, 3)
+    want = oracle.td_propagate(g, vloc, None, psi, 0.05, 3, 1, 2.0 / (nvec * g.dV) * 0.01, ld=True)
+    assert relerr(t.cpu().numpy(), want) < TOL_FULL
+    ctx.close()
