@@ -218,10 +218,11 @@ def run_gpu(args):
     e2e_value = shard.whole_job_rate(units_rank, world, args.steps, ms_e2e)
     checksum = float(torch.view_as_real(h_out).abs().sum())
 
-    td, samples = None, None
+    td, samples, libcmp = None, None, None
     if world == 1 and not args.no_td:
         td = run_td(torch, api, dev, stream, args)
         samples = run_config_samples(torch, api, dev, stream)
+        libcmp = run_library_comparison(torch, ctx, w, psi0, dev, stream)
 
     if rank == 0:
         peak, peak_src = measured_peaks()
@@ -275,6 +276,7 @@ def run_gpu(args):
                          "passes": passes},
             "td": td,
             "other_configs": samples,
+            "library_comparison": libcmp,
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",
                              "sample": f"{cpu_nv} vectors x 32 H applies of the same filter, {WORKLOAD} grid ({cpu_dt:.1f} s)"},
         }
@@ -315,6 +317,42 @@ def run_td(torch, api, dev, stream, args):
            "norm_drift": float(np.max(np.abs(norms / norms0 - 1.0)))}
     ctx.close()
     return out
+
+
+def run_library_comparison(torch, ctx, w, psi0, dev, stream):
+    """Context only (BASELINE.json north_star: "cuFFT is only a timed comparison"): one H application on the bench
+    workload built from torch.fft.fftn / ifftn (cuFFT) and torch element-wise ops, against sgw_apply_H."""
+    import math
+    g = w.grid
+
+    def k1(n, h):
+        return 2.0 * math.pi * torch.fft.fftfreq(n, d=h, device=dev, dtype=torch.float64)
+    kz, ky, kx = torch.meshgrid(k1(g.nz, g.hz), k1(g.ny, g.hy), k1(g.nx, g.hx), indexing="ij")
+    k2 = 0.5 * (kx * kx + ky * ky + kz * kz)
+    v = torch.from_numpy(w.vloc).to(dev)
+
+    def lib_apply(x):
+        return torch.fft.ifftn(k2 * torch.fft.fftn(x, dim=(1, 2, 3)), dim=(1, 2, 3)) + v * x
+
+    out = torch.empty_like(psi0)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    res = {}
+    for name, fn in (("cufft_torch", lambda: lib_apply(psi0)), ("sgw_apply_H", lambda: ctx.sgw_apply_H(psi0, out))):
+        fn()
+        torch.cuda.synchronize(dev)
+        e0.record(stream)
+        for _ in range(5):
+            r = fn()
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        res[name] = g.ng * w.nvec * 5 / (e0.elapsed_time(e1) * 1e-3)
+        del r
+    ref = lib_apply(psi0)
+    res["max_abs_diff"] = float((ref - out).abs().max())
+    res["what"] = "one H application on the bench workload; torch.fft (cuFFT) + element-wise ops vs sgw_apply_H; context only"
+    del ref, out
+    torch.cuda.empty_cache()
+    return res
 
 
 def run_config_samples(torch, api, dev, stream):
