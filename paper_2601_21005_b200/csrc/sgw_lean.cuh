@@ -123,7 +123,7 @@ __device__ __forceinline__ void lean_tile(const LeanArgs& a, int pass, const cd*
     for (int rd = 0; rd < ROUNDS; ++rd) {
         const int task = gt + rd * GT;
         if (task < TASKS) {
-            const int k1 = task % R1, bB = task / R1;
+            const int bB = task % B, k1 = task / B;          // pencils fastest: a quarter warp reads B = 8 distinct banks (odd pencil stride)
             cd* xB = xch + bB * SB + k1 * SK;
             // one twiddle table read serves both directions: forward y[m] *= W^(m k1), inverse y[m] *= conj(W^(m k1))
             // (small R2 only: for R2 >= 12 the cached twiddles would not fit the register budget)
