@@ -27,9 +27,9 @@ from paper_2601_21005_b200 import shard, workloads as W  # noqa: E402
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (z round trip + recurrence on
 # cfg1), from the ncu --set full capture summarised in profiles/r01_v2_cfg1.md: 3.69 GB without and 5.52 GB with
 # the series flush (every third term) -> average per launch
-# lean passes (default): x+y plane pass 3.06 GB without and 5.50 GB with the series flush (every second term),
+# lean passes (default): x+y plane pass 3.08 GB without and 5.53 GB with the series flush (every second term),
 # z pass 2.67 GB, from profiles/r01_lean_cfg1.md
-NCU_TRAFFIC_BYTES = {"lean": {"y_acc": (3.06e9 + 5.50e9) / 2.0, "z_cheb": 2.67e9},
+NCU_TRAFFIC_BYTES = {"lean": {"y_acc": (3.08e9 + 5.53e9) / 2.0, "z_cheb": 2.67e9},
                      "v2": {"z_cheb": (2 * 3.69e9 + 5.52e9) / 3.0, "y_acc": 2.18e9}, "engine": {}}
 TRAFFIC_SOURCE = {"lean": "profiles/r01_lean_cfg1.md", "v2": "profiles/r01_v2_cfg1.md", "engine": "profiles/r01_engine_v3_cfg1.md"}
 KERNEL_NAMES = {"lean": {"y_acc": "plane_lean_kernel<96,8,real,8> (x and y round trips of whole planes, recurrence on store)",
