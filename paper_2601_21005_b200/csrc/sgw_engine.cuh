@@ -350,7 +350,7 @@ __global__ void __launch_bounds__(EngCfg<N, B>::T, EngCfg<N, B>::MINB) engine_ke
         for (int rd = 0; rd < ROUNDS; ++rd) {
             const int task = gt + rd * GT;
             if (task < TASKS) {
-                const int k1 = task % R1, bB = task / R1;
+                const int bB = task % B, k1 = task / B;      // pencils fastest: bank-conflict free (odd pencil stride)
                 cd* xB = xch + bB * SB + k1 * SK;
                 cd y[R2];
 #pragma unroll

@@ -1,5 +1,6 @@
-// sgw_program.cu -- host side of the pass engine: builds programs of segments (sgw_engine.cuh) for
-// H apply, the Chebyshev filter and the split-operator step, and launches them.
+// sgw_program.cu -- host side of the fused passes: the lean streaming passes (sgw_lean.cuh; the default: second
+// half of this file) and the pass engine (sgw_engine.cuh: programs of segments with dependency counters), each
+// implementing H apply, the Chebyshev filter and the split-operator step.
 #include <cstdlib>
 #include <cstring>
 #include <vector>
