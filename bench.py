@@ -397,6 +397,53 @@ def run_config_samples(torch, api, dev, stream):
     return out
 
 
+def run_full_config(args):
+    """One full-size, full-length run of a BASELINE.json config (not the bench contract's line: a separate report
+    used for profiles/r01_full_configs.md): the whole filter on all vectors, then (cfg2, cfg4) the whole propagation."""
+    import torch
+    from paper_2601_21005_b200 import api
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream(dev)
+    w = W.make_workload(args.full_config)
+    max_nvec = min(w.nvec, 64)
+    ctx = api.context_for(w, max_nvec=max_nvec, stream=stream, device="cuda:0")
+    psi = torch.empty((w.nvec,) + w.grid.shape, dtype=torch.complex128, device=dev)
+    for v0 in range(0, w.nvec, max_nvec):
+        ctx.sgw_random_vectors(W.SEED_VEC, v0, min(max_nvec, w.nvec - v0), psi[v0:])
+    warm = psi[:1].clone()                                   # lazy workspace allocation and first-launch costs
+    ctx.sgw_cheb_filter(warm, w.coeffs[:3], w.emin, w.emax)
+    del warm
+    sampler = ClockSampler(0)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(dev)
+    e0.record(stream)
+    ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    ms_f = e0.elapsed_time(e1)
+    out = {"config": args.full_config, "grid": list(w.grid.shape), "atoms": w.atoms, "nvec": w.nvec, "nterms": w.nterms,
+           "kb_spheres": int(w.kb.nsphere), "filter_s": ms_f * 1e-3,
+           "filter_units_per_s": w.grid.ng * w.nvec * (w.nterms - 1) / (ms_f * 1e-3),
+           "filter_output_finite": all(bool(torch.isfinite(torch.view_as_real(psi[v])).all()) for v in range(w.nvec))}
+    if w.td_steps:
+        n0 = ctx.sgw_norms(psi)
+        ctx.sgw_set_td(1, w.rho_scale)
+        e0.record(stream)
+        ctx.sgw_td_propagate(psi, w.dt, w.td_steps)
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        ms_t = e0.elapsed_time(e1)
+        out.update({"td_steps": w.td_steps, "td_s": ms_t * 1e-3,
+                    "td_units_per_s": w.grid.ng * w.nvec * w.td_steps / (ms_t * 1e-3),
+                    "td_norm_drift": float((ctx.sgw_norms(psi) / n0 - 1.0).abs().max())})
+    out["clocks"] = sampler.stop()
+    out["gpu_launches"] = ctx.sgw_launch_count()
+    assert ctx.sgw_sync_check() == 0
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -406,7 +453,12 @@ def main():
     ap.add_argument("--nterms", type=int, default=None,
                     help="shorten the filter (profiling runs under ncu only; the default is the config's 512)")
     ap.add_argument("--no-td", action="store_true", help="skip the TD-step sample (cfg2) and the short samples of cfg0/cfg3/cfg4")
+    ap.add_argument("--full-config", default=None, choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"],
+                    help="run one BASELINE.json config at full size and length and print its own JSON report")
     args = ap.parse_args()
+    if args.full_config:
+        run_full_config(args)
+        return
     if args.impl == "reference":
         run_reference(args)
     else:
