@@ -325,12 +325,59 @@ __global__ void __launch_bounds__(LeanCfg<N, B, WPC>::T, LeanCfg<N, B, WPC>::MIN
     }
 }
 
+// Cluster variant of the plane kernel: a thread-block cluster of CS CTAs (CS SMs' worth of warp groups) owns one
+// plane at a time, so the planes in flight - what has to stay in L2 between the row tiles and the column tiles -
+// are 1/CS of the resident CTAs, and CS * NWG groups share a plane's N/B tiles (12 groups for the 12 tiles of a
+// 96^2 plane with CS = 3).  The x->y handoff is a cluster barrier with release/acquire semantics.
+__device__ __forceinline__ void cluster_barrier() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;\n" ::: "memory");
+}
+template <int N, int B, bool CPLX, int CS>
+__global__ void __launch_bounds__(LeanCfg<N, B, 8>::T, LeanCfg<N, B, 8>::MINB) plane_cluster_kernel(const LeanArgs a) {
+    using C = LeanCfg<N, B, 8>;
+    constexpr int R2 = C::R2, GT = C::GT, NWG = C::NWG;
+    constexpr unsigned TPP = N / B;
+    constexpr int NXY = N * N;
+    extern __shared__ __align__(16) char smraw[];
+    cd* twA = reinterpret_cast<cd*>(smraw);
+    cd* twB = twA + N;
+    char* ktab = reinterpret_cast<char*>(twB + N);
+    const int tid = threadIdx.x, grp = tid / GT, gt = tid % GT;
+    cd* xch = reinterpret_cast<cd*>(ktab + 2 * N * (CPLX ? 16 : 8)) + grp * C::XCH;
+    lean_tables<N, B, 8, CPLX>(a, twA, twB, ktab);
+    const char* ktab_y = ktab + N * (CPLX ? 16 : 8);
+    unsigned crank, cid, ncl;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(crank));
+    asm volatile("mov.u32 %0, %%clusterid.x;\n" : "=r"(cid));
+    asm volatile("mov.u32 %0, %%nclusterid.x;\n" : "=r"(ncl));
+    const int n2x = gt % R2, bAx = gt / R2, e0x = bAx * N + n2x;                 // x: lanes along n
+    const int bAy = gt % B, n2y = gt / B, e0y = n2y * N + bAy;                   // y: lanes along b
+    const unsigned me = crank * NWG + grp, gsz = CS * NWG;
+    for (unsigned p = cid; p < a.ntiles; p += ncl) {
+        const int gp = (int)(p % (unsigned)a.nz) * NXY;
+        for (unsigned q = me; q < TPP; q += gsz) {
+            const long long o = (long long)p * NXY + (long long)q * (B * N) + e0x;
+            const int g = gp + (int)q * (B * N) + e0x;
+            lean_tile<N, B, 8, CPLX, true, H_KEEP, H_KEEP>(a, 0, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g, R2, xch,
+                                                           twA, twB, ktab, grp, gt, n2x, bAx);
+        }
+        cluster_barrier();                                   // every row tile of the plane is stored and visible
+        for (unsigned q = me; q < TPP; q += gsz) {
+            const long long o = (long long)p * NXY + (long long)q * B + e0y;
+            const int g = gp + (int)q * B + e0y;
+            lean_tile<N, B, 8, CPLX, false, H_STREAM, H_STREAM>(a, 1, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g,
+                                                                R2 * N, xch, twA, twB, ktab_y, grp, gt, n2y, bAy);
+        }
+    }
+}
+
 struct LeanCall {
     LeanArgs args;
     int cplx;
     int kind;                 // 0..2: axis pass along x, y, z; 3: plane pass (x then y); 4 / 5: z / y pass on a cubic grid
     int ctas_per_sm;          // 0 = as many as fit
     int wpc;                  // plane kernel: warps per CTA, 8 (two CTAs per SM) or 16 (one)
+    int cluster;              // plane kernel: 1 = cluster-owned planes (plane_cluster_kernel), 0 = CTA-owned
     cudaStream_t stream;
 };
 // returns 0, -(stage*1000 + cudaError) on failure, or 1 if this (N, B) is not instantiated

@@ -210,6 +210,46 @@ static int lean_launch_kernel(K kern, int threads, size_t smem, long long want_c
     return e == cudaSuccess ? 0 : -(4000 + (int)e);
 }
 
+// cluster size for the cluster-owned plane kernel: CS * NWG groups should divide the N/B tiles of a plane
+template <int N, int B> struct ClusterSize {
+    static constexpr int NWG = LeanCfg<N, B, 8>::NWG, TPP = N / B;
+    static constexpr int CS = (TPP % (3 * NWG) == 0 && TPP / (3 * NWG) <= 1) ? 3
+                              : (TPP % (8 * NWG) == 0) ? 8 : (TPP % (4 * NWG) == 0) ? 4 : (TPP % (2 * NWG) == 0) ? 2 : 1;
+};
+
+template <int B, bool CPLX>
+static int launch_plane_cluster(const LeanCall* c) {
+    constexpr int N = SGW_N;
+    constexpr int CS = ClusterSize<N, B>::CS;
+    if (CS < 2 || N % B) return 1;
+    using Cfg = LeanCfg<N, B, 8>;
+    const size_t smem = CPLX ? Cfg::SMEM_CPLX : Cfg::SMEM_REAL;
+    auto kern = plane_cluster_kernel<N, B, CPLX, CS>;
+    static int max_clusters = 0;
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.blockDim = dim3(Cfg::T); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream; cfg.attrs = attr; cfg.numAttrs = 1;
+    if (!max_clusters) {
+        cudaError_t e = smem > 48 * 1024 ? cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) : cudaSuccess;
+        if (e != cudaSuccess) return -(1000 + (int)e);
+        if (CS > 8) { e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1); if (e != cudaSuccess) return -(1000 + (int)e); }
+        cfg.gridDim = dim3(CS * 148);
+        int n = 0;
+        e = cudaOccupancyMaxActiveClusters(&n, kern, &cfg);
+        if (e != cudaSuccess) return -(2000 + (int)e);
+        if (n < 1) return 1;
+        max_clusters = n;
+    }
+    long long ncl = max_clusters;
+    if (ncl > (long long)c->args.ntiles) ncl = c->args.ntiles;
+    if (ncl <= 0) return 0;
+    cfg.gridDim = dim3((unsigned)(ncl * CS));
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, c->args);
+    return e == cudaSuccess ? 0 : -(4000 + (int)e);
+}
+
 template <int B, bool CPLX>
 static int launch_lean_b(const LeanCall* c) {
     constexpr int N = SGW_N;
@@ -225,6 +265,7 @@ static int launch_lean_b(const LeanCall* c) {
         case 4: return lean_launch_kernel(axis_lean_kernel<N, B, CPLX, 2, true>, Cfg::T, smem, tiles_ctas, c->ctas_per_sm, c->args, c->stream, &occ[4]);
         case 3: {
             if (N % B) return 1;
+            if (c->cluster) { const int rc = launch_plane_cluster<B, CPLX>(c); if (rc != 1) return rc; }
             const long long ngroups = ((long long)c->args.ntiles + c->args.G - 1) / c->args.G;
             if (c->wpc == 16) {
                 using PCfg = LeanCfg<N, B, 16>;

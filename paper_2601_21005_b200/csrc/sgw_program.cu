@@ -393,9 +393,11 @@ struct LeanOp {
     const cd* kc[3];
 };
 
-int lean_launch(sgw_ctx* c, int axis_n, int kind, const LeanArgs& args, bool cplx, int ctas_per_sm, int prof_tag, int wpc = 8) {
+int lean_launch(sgw_ctx* c, int axis_n, int kind, const LeanArgs& args, bool cplx, int ctas_per_sm, int prof_tag, int wpc = 8,
+                int cluster = 0) {
     LeanCall call;
     call.wpc = wpc;
+    call.cluster = cluster;
     call.args = args;
     call.cplx = cplx ? 1 : 0;
     call.kind = kind;
@@ -414,7 +416,7 @@ int lean_launch(sgw_ctx* c, int axis_n, int kind, const LeanArgs& args, bool cpl
 
 // true if the fused x+y plane kernel applies: square planes whose CTA-owned groups (cur and acc of every
 // resident CTA's group) stay inside L2
-bool lean_use_plane(const sgw_ctx* c, bool cplx, int* G, int* ctas, int* wpc) {
+bool lean_use_plane(const sgw_ctx* c, bool cplx, int* G, int* ctas, int* wpc, int* cluster) {
     if (c->nx != c->ny) return false;
     const int n = c->nx, B = c->engB[0];
     if (n % B) return false;
@@ -424,6 +426,15 @@ bool lean_use_plane(const sgw_ctx* c, bool cplx, int* G, int* ctas, int* wpc) {
     // live misses 38 % of the re-reads and is still faster than one CTA per SM); then one 16-warp CTA per SM.
     const double plane_bytes = 16.0 * n * n * (cplx ? 1.0 : 2.0);
     const int g = c->lean_G > 0 ? c->lean_G : 1;
+    // Cluster-owned planes (plane_cluster_kernel: 4 CTAs per 128^2 plane, 8 per 256^2 plane): measured faster for the
+    // real family on those sizes (cfg2 filter 37.9 -> 38.5, cfg3 filter 31.2 -> 33.4 G units/s: 256^2 planes then
+    // also transpose through L2) and slower for the complex family and for 96^2 / 384^2 planes.  SGW_LEAN_CLUSTER=0/1
+    // overrides.
+    int use_cluster = (!cplx && (n == 128 || n == 256)) ? 1 : 0;
+    { const char* e = getenv("SGW_LEAN_CLUSTER"); if (e) use_cluster = atoi(e) ? 1 : 0; }
+    *cluster = use_cluster;
+    if (use_cluster && (n == 256 || n == 384)) { *G = 1; *ctas = 2; *wpc = 8; return true; }
+    if (use_cluster) { *G = 1; *ctas = 2; *wpc = 8; return true; }
     int w = 8, per_sm = 2;
     if (plane_bytes * g * 2 * c->num_sms > 90.0e6) { w = 16; per_sm = 1; }
     if (c->lean_ctas == 1) { w = 16; per_sm = 1; }
@@ -443,14 +454,14 @@ int lean_apply(sgw_ctx* c, int nv, const LeanOp& op, int kind_tag, bool allow_pl
     a.rho = op.rho; a.dens_scale = op.dens_scale;
     a.hs = op.hs; a.c0 = op.c0; a.c1 = op.c1;
     a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
-    int G = 1, ctas = 0, wpc = 8;
-    if (allow_plane && lean_use_plane(c, op.cplx, &G, &ctas, &wpc)) {
+    int G = 1, ctas = 0, wpc = 8, cluster = 0;
+    if (allow_plane && lean_use_plane(c, op.cplx, &G, &ctas, &wpc, &cluster)) {
         a.tw = c->tw[0];
         a.kre[0] = op.kre[0]; a.kre[1] = op.kre[1]; a.kc[0] = op.kc[0]; a.kc[1] = op.kc[1];
         a.flags[0] = op.fx; a.alpha[0] = op.ax; a.flags[1] = op.fy; a.alpha[1] = op.ay;
         a.ntiles = (unsigned)((long long)nv * c->nz);
         a.G = G;
-        SGW_TRY(lean_launch(c, 0, 3, a, op.cplx, ctas, 1 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_ACC), wpc));
+        SGW_TRY(lean_launch(c, 0, 3, a, op.cplx, ctas, 1 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_ACC), wpc, cluster));
     } else {
         a.tw = c->tw[0];
         a.kre[0] = op.kre[0]; a.kc[0] = op.kc[0]; a.kre[1] = nullptr; a.kc[1] = nullptr;

@@ -247,6 +247,34 @@ def test_lean_plane_kernel_group_and_cta_variants(api, torch_cuda, oracle, monke
     ctx.close()
 
 
+@pytest.mark.parametrize("n,nz,nvec", [(64, 48, 4), (96, 24, 5), (128, 24, 4), (256, 12, 4)])
+def test_lean_plane_cluster_kernel(api, torch_cuda, oracle, monkeypatch, n, nz, nvec):
+    """The cluster-owned plane kernel (clusters of 2 / 3 / 4 / 8 CTAs for 64^2 / 96^2 / 128^2 / 256^2 planes), forced
+    on for both families, against the oracle; nvec * nz planes exceed the resident clusters (at most 2 * 148 / size),
+    so the plane loop runs a ragged second round."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_ENGINE", "2")
+    monkeypatch.setenv("SGW_LEAN_CLUSTER", "1")
+    g = W.Grid(n, n, nz, 0.5, 0.5, 0.5)
+    rng = np.random.default_rng(23)
+    centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    psi = rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    emin, emax = W.spectral_bounds(g, vloc, False)
+    coeffs = rng.standard_normal(6)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+    assert relerr(t.cpu().numpy(), oracle.cheb_filter(g, vloc, None, psi, coeffs, emin, emax, ld=True)) < TOL_FULL
+    ctx.sgw_set_td(1, 2.0 / (nvec * g.dV) * 0.01)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_td_propagate(t, 0.05, 2)
+    want = oracle.td_propagate(g, vloc, None, psi, 0.05, 2, 1, 2.0 / (nvec * g.dV) * 0.01, ld=True)
+    assert relerr(t.cpu().numpy(), want) < TOL_FULL
+    ctx.close()
+
+
 def test_cfg1_full_length_three_implementations_agree(api, torch_cuda, monkeypatch):
     """cfg1 at full size and full length (64 vectors, all 512 terms), where the oracle would need hours: the three
     pass implementations are independent formulations of the recurrence (lean and engine accumulate in place with
