@@ -293,7 +293,7 @@ def run_td(torch, api, dev, stream, args):
     psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
     ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)            # filtered start vectors (untimed)
     ctx.sgw_set_td(1, w.rho_scale)
-    nsteps = 100
+    nsteps = args.td_steps
     ctx.sgw_td_propagate(psi, w.dt, 10)                            # warm-up
     norms0 = ctx.sgw_norms(psi).cpu().numpy()
     torch.cuda.synchronize(dev)
@@ -455,7 +455,17 @@ def main():
     ap.add_argument("--no-td", action="store_true", help="skip the TD-step sample (cfg2) and the short samples of cfg0/cfg3/cfg4")
     ap.add_argument("--full-config", default=None, choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"],
                     help="run one BASELINE.json config at full size and length and print its own JSON report")
+    ap.add_argument("--td-only", action="store_true",
+                    help="run only the TD-step sample (cfg2) and print its JSON object (profiling runs under ncu)")
+    ap.add_argument("--td-steps", type=int, default=100, help="timed steps of the TD-step sample (default 100 of the 2000)")
     args = ap.parse_args()
+    if args.td_only:
+        import torch
+        from paper_2601_21005_b200 import api
+        dev = torch.device("cuda:0")
+        torch.cuda.set_device(dev)
+        print(json.dumps(run_td(torch, api, dev, torch.cuda.current_stream(dev), args)))
+        return
     if args.full_config:
         run_full_config(args)
         return
