@@ -251,9 +251,16 @@ extern "C" int sgw_sync_check(sgw_ctx* c) {
     return sgw::eng_check_error(c);
 }
 
+void sgw::drop_filter_graph(sgw_ctx* c) {
+    if (c->fgraph) { cudaGraphExecDestroy(c->fgraph); c->fgraph = nullptr; }
+    c->fg_psi = nullptr;
+}
+
 extern "C" int sgw_destroy(sgw_ctx* c) {
     if (!c) return SGW_OK;
     cudaStreamSynchronize(c->stream);
+    sgw::drop_filter_graph(c);
+    if (c->gstream) cudaStreamDestroy(c->gstream);
     for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
     for (int a = 0; a < 3; ++a) {
         cudaFree(c->tw[a]); cudaFree(c->kin[a]); cudaFree(c->cheb_kin[a]); cudaFree(c->td_kin[a]); cudaFree(c->ws[a]);
@@ -358,6 +365,7 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
 
 extern "C" int sgw_set_vloc(sgw_ctx* c, const double* d_vloc) {
     if (!c) return set_error(SGW_EINVAL, "sgw_set_vloc: null context");
+    sgw::drop_filter_graph(c);
     if (!d_vloc) { cudaStreamSynchronize(c->stream); cudaFree(c->vloc); c->vloc = nullptr; return SGW_OK; }
     int rc = 0;
     if (!c->vloc) rc = dev_alloc(&c->vloc, c->ng);
@@ -371,6 +379,7 @@ extern "C" int sgw_set_nonlocal(sgw_ctx* c, int nsphere, const int64_t* d_ptr, c
                                 const double* d_beta, const double* d_D) {
     if (!c || nsphere < 0) return set_error(SGW_EINVAL, "sgw_set_nonlocal: bad argument");
     cudaStreamSynchronize(c->stream);
+    sgw::drop_filter_graph(c);
     cudaFree(c->sph_ptr); cudaFree(c->sph_idx); cudaFree(c->beta); cudaFree(c->D);
     c->sph_ptr = nullptr; c->sph_idx = nullptr; c->beta = nullptr; c->D = nullptr; c->nsphere = 0;
     if (nsphere == 0) return SGW_OK;

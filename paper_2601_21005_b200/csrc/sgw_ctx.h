@@ -70,6 +70,14 @@ struct sgw_ctx {
     size_t cnt_cap;
     int* d_err;
     int l2_chunk;                            // vectors per L2-resident chunk (0 = whole batch)
+    // launch-bound grids: one whole sgw_cheb_filter call captured as a CUDA graph and cached (sgw_solvers.cu)
+    cudaStream_t gstream;                    // internal capture stream (lazy)
+    cudaGraphExec_t fgraph;                  // instantiated graph of the last small filter call, or NULL
+    void* fg_psi;                            // its key: vector block, counts, window, coefficients
+    int fg_nvec, fg_nterms;
+    double fg_emin, fg_emax;
+    std::vector<double> fg_coeffs;
+    int64_t fg_launches;                     // kernel nodes in the graph
     // optional per-pass device timing (sgw_profile_*): event pairs around pass launches
     bool prof_on;
     std::vector<cudaEvent_t> prof_ev;        // 2 per recorded launch
@@ -100,4 +108,6 @@ void prof_end(sgw_ctx* c, cudaEvent_t e1);
 int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau, const cd* phase = nullptr,
              int fold = 0);
 int ensure_ws(sgw_ctx* c, int n);
+// forget the cached filter graph (the operator or its buffers changed)
+void drop_filter_graph(sgw_ctx* c);
 }  // namespace sgw

@@ -202,11 +202,9 @@ extern "C" int sgw_hartree(sgw_ctx* c, int nvec, const void* d_psi, double rho_s
     return check_cuda(cudaMemcpyAsync(d_vh, c->vh, c->ng * sizeof(double), cudaMemcpyDeviceToDevice, c->stream), "copy vh");
 }
 
-extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, double Emin, double Emax,
-                               int nterms) {
-    if (!c || nvec < 0 || (nvec > 0 && !d_psi) || !h_coeffs || nterms < 1 || !(Emax > Emin))
-        return set_error(SGW_EINVAL, "sgw_cheb_filter: bad argument");
-    if (nvec == 0) return SGW_OK;
+namespace {
+// the launches of one filter call, in stream order on c->stream (arguments already checked)
+int cheb_filter_body(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, double Emin, double Emax, int nterms) {
     const long long ng = c->ng;
     const double Eb = 0.5 * (Emax + Emin), dE = 0.5 * (Emax - Emin), s = 2.0 / dE;
     if (nterms == 1) {
@@ -270,6 +268,58 @@ extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* 
         }
         SGW_TRY(check_cuda(cudaMemcpyAsync(X0, O, (size_t)nv * ng * sizeof(cd), cudaMemcpyDeviceToDevice, c->stream), "copy out"));
     }
+    return SGW_OK;
+}
+
+// Small grids are launch-bound (cfg0: 2 MB per array, 256 launches of a few us each): the whole call is captured
+// once on an internal stream, instantiated as a CUDA graph and replayed on the caller's stream for as long as the
+// call repeats with the same vector block, window and coefficients.  SGW_GRAPH=0 disables, SGW_GRAPH_BYTES moves
+// the size limit (bytes of one vector block; default 16 MB).
+bool filter_graph_wanted(const sgw_ctx* c, int nvec, int nterms) {
+    if (c->use_engine != 2 || c->prof_on || c->nsphere > 0 || nvec > c->max_nvec || nterms < 3) return false;
+    const char* e = getenv("SGW_GRAPH");
+    if (e && atoi(e) == 0) return false;
+    double limit = 16.0e6;
+    const char* b = getenv("SGW_GRAPH_BYTES");
+    if (b && atof(b) > 0) limit = atof(b);
+    return (double)nvec * (double)c->ng * sizeof(cd) <= limit;
+}
+}  // namespace
+
+extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, double Emin, double Emax,
+                               int nterms) {
+    if (!c || nvec < 0 || (nvec > 0 && !d_psi) || !h_coeffs || nterms < 1 || !(Emax > Emin))
+        return set_error(SGW_EINVAL, "sgw_cheb_filter: bad argument");
+    if (nvec == 0) return SGW_OK;
+    if (!filter_graph_wanted(c, nvec, nterms)) return cheb_filter_body(c, nvec, d_psi, h_coeffs, Emin, Emax, nterms);
+    const bool hit = c->fgraph && c->fg_psi == d_psi && c->fg_nvec == nvec && c->fg_nterms == nterms && c->fg_emin == Emin &&
+                     c->fg_emax == Emax && (int)c->fg_coeffs.size() == nterms &&
+                     memcmp(c->fg_coeffs.data(), h_coeffs, nterms * sizeof(double)) == 0;
+    if (!hit) {
+        drop_filter_graph(c);
+        SGW_TRY(ensure_ws(c, 2));                     // no allocation inside the capture
+        if (!c->gstream) SGW_TRY(check_cuda(cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking), "graph stream"));
+        cudaStream_t user = c->stream;
+        const int64_t before = c->launches;
+        SGW_TRY(check_cuda(cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeRelaxed), "begin capture"));
+        c->stream = c->gstream;
+        const int rc = cheb_filter_body(c, nvec, d_psi, h_coeffs, Emin, Emax, nterms);
+        c->stream = user;
+        cudaGraph_t g = nullptr;
+        const cudaError_t ce = cudaStreamEndCapture(c->gstream, &g);
+        const int64_t nodes = c->launches - before;
+        c->launches = before;
+        if (rc != 0) { if (g) cudaGraphDestroy(g); return rc; }
+        SGW_TRY(check_cuda(ce, "end capture"));
+        const cudaError_t ie = cudaGraphInstantiate(&c->fgraph, g, 0);
+        cudaGraphDestroy(g);
+        if (ie != cudaSuccess) { c->fgraph = nullptr; return check_cuda(ie, "graph instantiate"); }
+        c->fg_psi = d_psi; c->fg_nvec = nvec; c->fg_nterms = nterms; c->fg_emin = Emin; c->fg_emax = Emax;
+        c->fg_coeffs.assign(h_coeffs, h_coeffs + nterms);
+        c->fg_launches = nodes;
+    }
+    SGW_TRY(check_cuda(cudaGraphLaunch(c->fgraph, c->stream), "graph launch"));
+    c->launches += c->fg_launches;
     return SGW_OK;
 }
 

@@ -142,6 +142,49 @@ def test_cheb_cfg0_full(api, torch_cuda, oracle):
     ctx.close()
 
 
+def test_cheb_small_grid_graph_capture_replay_and_rekey(api, torch_cuda, oracle, monkeypatch):
+    """Launch-bound grids run the filter as a cached CUDA graph (sgw_solvers.cu): the first call captures, a repeat
+    with the same vector block, window and coefficients replays, any change re-captures; set_vloc drops the
+    graph.  Every result is compared with the oracle, and with the plain launch sequence bit for bit."""
+    torch = torch_cuda
+    g, vloc, _, rng = problem(16, 16, 24, kb=False, seed=5)
+    emin, emax = W.spectral_bounds(g, vloc, False)
+    c1, c2 = rng.standard_normal(20), rng.standard_normal(20)
+    psi = rvec(rng, g, 3)
+    want1 = oracle.cheb_filter(g, vloc, None, psi, c1, emin, emax, ld=True)
+    want2 = oracle.cheb_filter(g, vloc, None, psi, c2, emin, emax, ld=True)
+    ctx = make_ctx(api, torch, g, vloc, None, 3)
+    src = torch.from_numpy(psi).cuda()
+    t = src.clone()
+    n0 = ctx.sgw_launch_count()
+    ctx.sgw_cheb_filter(t, c1, emin, emax)                       # capture + launch
+    per_call = ctx.sgw_launch_count() - n0
+    assert per_call >= 19 * 2
+    got_capture = t.cpu().numpy()
+    assert relerr(got_capture, want1) < TOL_FULL
+    t.copy_(src)
+    ctx.sgw_cheb_filter(t, c1, emin, emax)                       # replay
+    assert ctx.sgw_launch_count() - n0 == 2 * per_call
+    assert np.array_equal(t.cpu().numpy(), got_capture)
+    t.copy_(src)
+    ctx.sgw_cheb_filter(t, c2, emin, emax)                       # other coefficients: new graph
+    assert relerr(t.cpu().numpy(), want2) < TOL_FULL
+    t2 = src.clone()
+    ctx.sgw_cheb_filter(t2, c2, emin, emax)                      # other vector block: new graph
+    assert np.array_equal(t2.cpu().numpy(), t.cpu().numpy())
+    vloc2 = 0.5 * vloc
+    ctx.sgw_set_vloc(torch.from_numpy(vloc2).cuda())             # operator changed: graph dropped
+    t2.copy_(src)
+    ctx.sgw_cheb_filter(t2, c2, emin, emax)
+    want3 = oracle.cheb_filter(g, vloc2, None, psi, c2, emin, emax, ld=True)
+    assert relerr(t2.cpu().numpy(), want3) < TOL_FULL
+    monkeypatch.setenv("SGW_GRAPH", "0")                         # plain launches give the same bits
+    t3 = src.clone()
+    ctx.sgw_cheb_filter(t3, c2, emin, emax)
+    assert np.array_equal(t3.cpu().numpy(), t2.cpu().numpy())
+    ctx.close()
+
+
 @pytest.mark.parametrize("nterms", [1, 2, 3, 4, 5, 6, 7, 33])
 def test_cheb_term_counts_with_kb_and_sub_batches(api, torch_cuda, oracle, nterms):
     torch = torch_cuda
