@@ -359,7 +359,7 @@ def run_config_samples(torch, api, dev, stream):
     """Short samples of the other BASELINE.json configs (shapes and potentials as specified, fewer vectors / terms /
     steps, stated per entry): evidence that every config runs on the same kernels, not headline numbers."""
     out = {}
-    specs = [("cfg0", dict(), 128, 0, "32^3, 4 vectors, all 128 terms (launch-latency bound)"),
+    specs = [("cfg0", dict(), 128, 0, "32^3, 4 vectors, all 128 terms (launch-latency bound; replayed as one cached CUDA graph)"),
              ("cfg3", dict(nvec=8, nterms=17), 17, 4, "256^3, Si705H300 + KB projectors, 8 of 256 vectors, 16 of 2047 applications, 4 TD-Hartree steps"),
              ("cfg4", dict(nvec=2, nterms=9), 9, 2, "384^3, Si8381H1620 + KB projectors, 2 of 32 vectors, 8 of 2047 applications, 2 of 500 TD-Hartree steps")]
     for name, kw, nterms, nsteps, what in specs:

@@ -236,6 +236,12 @@ __device__ __forceinline__ void lean_tables(const LeanArgs& a, cd* twA, cd* twB,
     __syncthreads();
 }
 
+// Programmatic dependent launch (opt-in, SGW_PDL=1: lean_launch_kernel sets the stream-serialization attribute): a pass lets the next
+// launch start at once and loads its own constant tables (twiddles, k-space multipliers: written before any pass of
+// the call) before it waits for the preceding grid's memory.  Both are no-ops for a plain launch.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // One pass along AXIS (0 x, 1 y, 2 z) over all tiles; groups take tiles round robin.
 //   x: tile t = B consecutive rows (rows are contiguous across planes and vectors)
 //   y: tile t = (plane, column block);  z: tile t = (vector, xy block)
@@ -250,7 +256,9 @@ __global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) axis_le
     char* ktab = reinterpret_cast<char*>(twB + N);
     const int tid = threadIdx.x, grp = tid / GT, gt = tid % GT;
     cd* xch = reinterpret_cast<cd*>(ktab + 2 * N * (CPLX ? 16 : 8)) + grp * C::XCH;
+    pdl_launch_dependents();
     lean_tables<N, B, 8, CPLX>(a, twA, twB, ktab);
+    pdl_wait();
 
     const int nxy = CUBE ? N * N : a.nx * a.ny;
     const long long ng = (long long)nxy * a.nz;
@@ -297,7 +305,9 @@ __global__ void __launch_bounds__(LeanCfg<N, B, WPC>::T, LeanCfg<N, B, WPC>::MIN
     char* ktab = reinterpret_cast<char*>(twB + N);
     const int tid = threadIdx.x, grp = tid / GT, gt = tid % GT;
     cd* xch = reinterpret_cast<cd*>(ktab + 2 * N * (CPLX ? 16 : 8)) + grp * C::XCH;
+    pdl_launch_dependents();
     lean_tables<N, B, WPC, CPLX>(a, twA, twB, ktab);
+    pdl_wait();
     const char* ktab_y = ktab + N * (CPLX ? 16 : 8);
 
     const int n2x = gt % R2, bAx = gt / R2, e0x = bAx * N + n2x;                 // x: lanes along n

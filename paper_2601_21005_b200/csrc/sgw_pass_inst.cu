@@ -205,8 +205,18 @@ static int lean_launch_kernel(K kern, int threads, size_t smem, long long want_c
     long long grid = (long long)per_sm * num_sms;
     if (grid > want_ctas) grid = want_ctas;
     if (grid <= 0) return 0;
-    kern<<<(unsigned)grid, threads, smem, stream>>>(args);
-    cudaError_t e = cudaGetLastError();
+    // SGW_PDL=1: programmatic dependent launch, the pass may start while its predecessor drains (it waits for the
+    // predecessor's memory after loading its tables, sgw_lean.cuh).  Off by default: measured neutral on cfg1-cfg3
+    // (within 0.5 %) and slower inside the cfg0 graph (0.99 -> 1.15 ms), DESIGN.md section 10
+    const char* pe = getenv("SGW_PDL");
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)threads); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = (pe && atoi(pe) == 1) ? 1 : 0;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, args);
+    if (e == cudaSuccess) e = cudaGetLastError();
     return e == cudaSuccess ? 0 : -(4000 + (int)e);
 }
 

@@ -185,6 +185,28 @@ def test_cheb_small_grid_graph_capture_replay_and_rekey(api, torch_cuda, oracle,
     ctx.close()
 
 
+def test_programmatic_dependent_launch_option_gives_the_same_bits(api, torch_cuda, monkeypatch):
+    """SGW_PDL=1 launches the lean passes with programmatic stream serialization (each waits for its predecessor's
+    memory after loading its tables): filter and propagation results must not change by a bit."""
+    torch = torch_cuda
+    g, vloc, _, rng = problem(32, 32, 16, kb=False, seed=9)
+    emin, emax = W.spectral_bounds(g, vloc, False)
+    coeffs = rng.standard_normal(24)
+    psi = rvec(rng, g, 3)
+    res = {}
+    for pdl in ("0", "1"):
+        monkeypatch.setenv("SGW_PDL", pdl)
+        monkeypatch.setenv("SGW_GRAPH", pdl)                      # plain launches vs graph + PDL edges
+        ctx = make_ctx(api, torch, g, vloc, None, 3)
+        t = torch.from_numpy(psi).cuda()
+        ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+        ctx.sgw_set_td(0, 0.0)                                    # frozen potential: no atomics, bits are reproducible
+        ctx.sgw_td_propagate(t, 0.05, 5)
+        res[pdl] = t.cpu().numpy()
+        ctx.close()
+    assert np.array_equal(res["0"], res["1"])
+
+
 @pytest.mark.parametrize("nterms", [1, 2, 3, 4, 5, 6, 7, 33])
 def test_cheb_term_counts_with_kb_and_sub_batches(api, torch_cuda, oracle, nterms):
     torch = torch_cuda
