@@ -84,9 +84,10 @@ int sgw_apply_H(sgw_ctx* ctx, int nvec, const void* d_in, void* d_out);
  * Ht = (H - Eb)/dE, Eb = (Emax+Emin)/2, dE = (Emax-Emin)/2; three-term recurrence, nterms-1
  * applications of H.  h_coeffs: nterms host doubles.  Requires nterms >= 1 and Emax > Emin.
  * Asynchronous on the context's stream.  When one vector block is at most 16 MB and there is no
- * nonlocal term the call is launch-bound: its launches are captured once into a CUDA graph that the
- * context keeps and replays while (d_psi, nvec, nterms, Emin, Emax, h_coeffs[]) repeat; same kernels,
- * same order, same bits.  sgw_set_vloc / sgw_set_nonlocal drop the graph.  SGW_GRAPH=0 disables. */
+ * nonlocal term the call is launch-bound: when it repeats with the same (d_psi, nvec, nterms, Emin,
+ * Emax, h_coeffs[]) its launches are captured into a CUDA graph that the context keeps and replays
+ * from then on; same kernels, same order, same bits.  sgw_set_vloc / sgw_set_nonlocal drop the
+ * graph.  SGW_GRAPH=0 disables. */
 int sgw_cheb_filter(sgw_ctx* ctx, int nvec, void* d_psi, const double* h_coeffs, double Emin,
                     double Emax, int nterms);
 

@@ -271,9 +271,9 @@ int cheb_filter_body(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, 
     return SGW_OK;
 }
 
-// Small grids are launch-bound (cfg0: 2 MB per array, 256 launches of a few us each): the whole call is captured
-// once on an internal stream, instantiated as a CUDA graph and replayed on the caller's stream for as long as the
-// call repeats with the same vector block, window and coefficients.  SGW_GRAPH=0 disables, SGW_GRAPH_BYTES moves
+// Small grids are launch-bound (cfg0: 2 MB per array, 256 launches of a few us each): when a call repeats with the
+// same vector block, window and coefficients, its launches are captured on an internal stream, instantiated as a
+// CUDA graph and replayed on the caller's stream from then on (the first call with a key launches plainly).  SGW_GRAPH=0 disables, SGW_GRAPH_BYTES moves
 // the size limit (bytes of one vector block; default 16 MB).
 bool filter_graph_wanted(const sgw_ctx* c, int nvec, int nterms) {
     if (c->use_engine != 2 || c->prof_on || c->nsphere > 0 || nvec > c->max_nvec || nterms < 3) return false;
@@ -292,11 +292,18 @@ extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* 
         return set_error(SGW_EINVAL, "sgw_cheb_filter: bad argument");
     if (nvec == 0) return SGW_OK;
     if (!filter_graph_wanted(c, nvec, nterms)) return cheb_filter_body(c, nvec, d_psi, h_coeffs, Emin, Emax, nterms);
-    const bool hit = c->fgraph && c->fg_psi == d_psi && c->fg_nvec == nvec && c->fg_nterms == nterms && c->fg_emin == Emin &&
-                     c->fg_emax == Emax && (int)c->fg_coeffs.size() == nterms &&
-                     memcmp(c->fg_coeffs.data(), h_coeffs, nterms * sizeof(double)) == 0;
-    if (!hit) {
+    const bool same = c->fg_psi == d_psi && c->fg_nvec == nvec && c->fg_nterms == nterms && c->fg_emin == Emin &&
+                      c->fg_emax == Emax && (int)c->fg_coeffs.size() == nterms &&
+                      memcmp(c->fg_coeffs.data(), h_coeffs, nterms * sizeof(double)) == 0;
+    if (!same) {
+        // first call with this key: plain launches (capture + instantiation cost more than they save on a single
+        // call); the key is remembered and a repeat captures
         drop_filter_graph(c);
+        c->fg_psi = d_psi; c->fg_nvec = nvec; c->fg_nterms = nterms; c->fg_emin = Emin; c->fg_emax = Emax;
+        c->fg_coeffs.assign(h_coeffs, h_coeffs + nterms);
+        return cheb_filter_body(c, nvec, d_psi, h_coeffs, Emin, Emax, nterms);
+    }
+    if (!c->fgraph) {
         SGW_TRY(ensure_ws(c, 2));                     // no allocation inside the capture
         if (!c->gstream) SGW_TRY(check_cuda(cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking), "graph stream"));
         cudaStream_t user = c->stream;
@@ -314,8 +321,6 @@ extern "C" int sgw_cheb_filter(sgw_ctx* c, int nvec, void* d_psi, const double* 
         const cudaError_t ie = cudaGraphInstantiate(&c->fgraph, g, 0);
         cudaGraphDestroy(g);
         if (ie != cudaSuccess) { c->fgraph = nullptr; return check_cuda(ie, "graph instantiate"); }
-        c->fg_psi = d_psi; c->fg_nvec = nvec; c->fg_nterms = nterms; c->fg_emin = Emin; c->fg_emax = Emax;
-        c->fg_coeffs.assign(h_coeffs, h_coeffs + nterms);
         c->fg_launches = nodes;
     }
     SGW_TRY(check_cuda(cudaGraphLaunch(c->fgraph, c->stream), "graph launch"));

@@ -143,9 +143,9 @@ def test_cheb_cfg0_full(api, torch_cuda, oracle):
 
 
 def test_cheb_small_grid_graph_capture_replay_and_rekey(api, torch_cuda, oracle, monkeypatch):
-    """Launch-bound grids run the filter as a cached CUDA graph (sgw_solvers.cu): the first call captures, a repeat
-    with the same vector block, window and coefficients replays, any change re-captures; set_vloc drops the
-    graph.  Every result is compared with the oracle, and with the plain launch sequence bit for bit."""
+    """Launch-bound grids run a repeated filter call as a cached CUDA graph (sgw_solvers.cu): the first call with a
+    key (vector block, window, coefficients) launches plainly, its repeat captures, later repeats replay, any change
+    starts over; set_vloc drops graph and key.  Every result is compared with the oracle, and with the plain launch sequence bit for bit."""
     torch = torch_cuda
     g, vloc, _, rng = problem(16, 16, 24, kb=False, seed=5)
     emin, emax = W.spectral_bounds(g, vloc, False)
@@ -157,27 +157,35 @@ def test_cheb_small_grid_graph_capture_replay_and_rekey(api, torch_cuda, oracle,
     src = torch.from_numpy(psi).cuda()
     t = src.clone()
     n0 = ctx.sgw_launch_count()
-    ctx.sgw_cheb_filter(t, c1, emin, emax)                       # capture + launch
+    ctx.sgw_cheb_filter(t, c1, emin, emax)                       # new key: plain launches
     per_call = ctx.sgw_launch_count() - n0
     assert per_call >= 19 * 2
     got_capture = t.cpu().numpy()
     assert relerr(got_capture, want1) < TOL_FULL
+    for rep in (2, 3, 4):                                        # repeat: capture + launch, then replays
+        t.copy_(src)
+        ctx.sgw_cheb_filter(t, c1, emin, emax)
+        assert ctx.sgw_launch_count() - n0 == rep * per_call
+        assert np.array_equal(t.cpu().numpy(), got_capture)
     t.copy_(src)
-    ctx.sgw_cheb_filter(t, c1, emin, emax)                       # replay
-    assert ctx.sgw_launch_count() - n0 == 2 * per_call
-    assert np.array_equal(t.cpu().numpy(), got_capture)
+    ctx.sgw_cheb_filter(t, c2, emin, emax)                       # other coefficients: graph dropped
+    assert relerr(t.cpu().numpy(), want2) < TOL_FULL
     t.copy_(src)
-    ctx.sgw_cheb_filter(t, c2, emin, emax)                       # other coefficients: new graph
+    ctx.sgw_cheb_filter(t, c2, emin, emax)                       # and re-captured on the repeat
     assert relerr(t.cpu().numpy(), want2) < TOL_FULL
     t2 = src.clone()
-    ctx.sgw_cheb_filter(t2, c2, emin, emax)                      # other vector block: new graph
+    ctx.sgw_cheb_filter(t2, c2, emin, emax)                      # other vector block: new key
     assert np.array_equal(t2.cpu().numpy(), t.cpu().numpy())
-    vloc2 = 0.5 * vloc
-    ctx.sgw_set_vloc(torch.from_numpy(vloc2).cuda())             # operator changed: graph dropped
     t2.copy_(src)
     ctx.sgw_cheb_filter(t2, c2, emin, emax)
+    assert np.array_equal(t2.cpu().numpy(), t.cpu().numpy())
+    vloc2 = 0.5 * vloc
+    ctx.sgw_set_vloc(torch.from_numpy(vloc2).cuda())             # operator changed: graph and key dropped
     want3 = oracle.cheb_filter(g, vloc2, None, psi, c2, emin, emax, ld=True)
-    assert relerr(t2.cpu().numpy(), want3) < TOL_FULL
+    for _ in range(3):
+        t2.copy_(src)
+        ctx.sgw_cheb_filter(t2, c2, emin, emax)
+        assert relerr(t2.cpu().numpy(), want3) < TOL_FULL
     monkeypatch.setenv("SGW_GRAPH", "0")                         # plain launches give the same bits
     t3 = src.clone()
     ctx.sgw_cheb_filter(t3, c2, emin, emax)
@@ -199,7 +207,10 @@ def test_programmatic_dependent_launch_option_gives_the_same_bits(api, torch_cud
         monkeypatch.setenv("SGW_GRAPH", pdl)                      # plain launches vs graph + PDL edges
         ctx = make_ctx(api, torch, g, vloc, None, 3)
         t = torch.from_numpy(psi).cuda()
+        src = t.clone()
         ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+        t.copy_(src)
+        ctx.sgw_cheb_filter(t, coeffs, emin, emax)                # the repeat is the captured graph when SGW_GRAPH=1
         ctx.sgw_set_td(0, 0.0)                                    # frozen potential: no atomics, bits are reproducible
         ctx.sgw_td_propagate(t, 0.05, 5)
         res[pdl] = t.cpu().numpy()
