@@ -427,6 +427,24 @@ def run_full_config(args):
            "kb_spheres": int(w.kb.nsphere), "filter_s": ms_f * 1e-3,
            "filter_units_per_s": w.grid.ng * w.nvec * (w.nterms - 1) / (ms_f * 1e-3),
            "filter_output_finite": all(bool(torch.isfinite(torch.view_as_real(psi[v])).all()) for v in range(w.nvec))}
+    if args.repeat > 0:
+        # the same call again on the restored vectors: launch-bound grids capture a CUDA graph on the first repeat
+        # and replay it afterwards
+        psi0 = torch.empty_like(psi)
+        for v0 in range(0, w.nvec, max_nvec):
+            ctx.sgw_random_vectors(W.SEED_VEC, v0, min(max_nvec, w.nvec - v0), psi0[v0:])
+        rep = []
+        for _ in range(args.repeat):
+            psi.copy_(psi0)
+            torch.cuda.synchronize(dev)
+            e0.record(stream)
+            ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
+            e1.record(stream)
+            torch.cuda.synchronize(dev)
+            rep.append(e0.elapsed_time(e1) * 1e-3)
+        out["filter_repeat_s"] = rep
+        out["filter_repeat_units_per_s"] = w.grid.ng * w.nvec * (w.nterms - 1) / min(rep)
+        del psi0
     if w.td_steps:
         n0 = ctx.sgw_norms(psi)
         ctx.sgw_set_td(1, w.rho_scale)
@@ -455,6 +473,8 @@ def main():
     ap.add_argument("--no-td", action="store_true", help="skip the TD-step sample (cfg2) and the short samples of cfg0/cfg3/cfg4")
     ap.add_argument("--full-config", default=None, choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"],
                     help="run one BASELINE.json config at full size and length and print its own JSON report")
+    ap.add_argument("--repeat", type=int, default=0,
+                    help="with --full-config: repeat the filter call this many times on the restored vectors and report each time")
     ap.add_argument("--td-only", action="store_true",
                     help="run only the TD-step sample (cfg2) and print its JSON object (profiling runs under ncu)")
     ap.add_argument("--td-steps", type=int, default=100, help="timed steps of the TD-step sample (default 100 of the 2000)")
