@@ -21,9 +21,10 @@
 //
 // Pins (tests/test_oracle_*.py): splitmix64 published stream; FFT vs O(N^2) DFT and numpy.fft;
 // plane-wave eigenvalues; dense-H built independently with numpy; eigh brute force; Hartree erf
-// closed form; TD closed forms and order-2 convergence; power-iteration bounds vs dense eigenvalues.  "parity unpinned": the TD-Hartree
-// trajectory and the KB factor NL(tau) inside the propagator beyond unitarity/limit checks
-// (they are defined by the algorithm below, R-8, R-9, R-11).
+// closed form; TD closed forms and order-2 convergence; TD-Hartree energy drift proportional to dt; overlapping KB
+// spheres converge to the dense propagator; power-iteration bounds vs dense eigenvalues.  "parity unpinned": config-level
+// outputs; the TD-Hartree trajectory and the KB factor NL(tau) inside the propagator are pinned to first order in the
+// step only (sign, scale, per-step rebuild), their O(tau^2) terms are defined by the algorithm below (R-8, R-9, R-11).
 #include <cmath>
 #include <complex>
 #include <cstdint>

@@ -265,6 +265,73 @@ def test_td_hartree_mode_uses_start_of_step_density(oracle):
     assert np.abs(oracle.norms(c) / oracle.norms(psi) - 1).max() < 1e-13
 
 
+def test_td_hartree_trajectory_conserves_energy_to_first_order_in_dt(oracle):
+    """Pin for the multi-step TD-Hartree trajectory (R-8): the exact flow of
+    i d/dt psi_v = (T + V_loc + V_H[rho(t)]) psi_v, rho = rho_scale sum_v |psi_v|^2, conserves
+    E = rho_scale sum_v <psi_v|T + V_loc|psi_v> dV + 1/2 int rho V_H.  The split-operator step with the start-of-step
+    density is first-order consistent with that flow, so the drift over a fixed time halves with dt; a potential that
+    is not rebuilt every step, or enters with the wrong sign or scale, leaves a drift that does not shrink.  The
+    energy is evaluated here with numpy.fft for T and the (erf-pinned) oracle Hartree potential."""
+    n, h = 12, 0.7
+    g = W.Grid(n, n, n, h, h, h)
+    L = n * h
+    rng = np.random.default_rng(4)
+    vloc = W.gaussian_vloc(g, rng.uniform(0, L, size=(2, 3)), [1.0, 1.5], [1.0, 1.2])
+    z, y, x = np.meshgrid(*(np.arange(n) * h,) * 3, indexing="ij")
+
+    def packet(c, s, k):
+        d2 = sum(np.minimum(np.abs(a - ci), L - np.abs(a - ci)) ** 2 for a, ci in zip((x, y, z), c))
+        return np.exp(-d2 / (2 * s * s)) * np.exp(1j * (k[0] * x + k[1] * y + k[2] * z))
+
+    kk = 2 * np.pi / L
+    psi = np.stack([packet((3.0, 4.0, 4.5), 1.3, (kk, 0, 0)), packet((5.0, 3.5, 4.0), 1.5, (0, -kk, kk))])
+    psi /= np.sqrt((np.abs(psi) ** 2).sum(axis=(1, 2, 3), keepdims=True) * g.dV)
+    rs = 4.0                                                     # 4 electrons per orbital: max V_H ~ 5 Ha
+    kx = 2 * np.pi * np.fft.fftfreq(n, h)
+    k2 = kx[:, None, None] ** 2 + kx[None, :, None] ** 2 + kx[None, None, :] ** 2
+
+    def energy(p):
+        e = 0.0
+        for v in p:
+            e += rs * (0.5 * (k2 * np.abs(np.fft.fftn(v)) ** 2).sum() / v.size + (vloc * np.abs(v) ** 2).sum()) * g.dV
+        vh, rho = oracle.hartree(g, p, rs)
+        return e + 0.5 * (rho * vh).sum() * g.dV
+
+    e0 = energy(psi)
+    drift = []
+    for dt in (0.1, 0.05, 0.025):
+        out = oracle.td_propagate(g, vloc, None, psi, dt, int(round(1.0 / dt)), hartree_mode=1, rho_scale=rs)
+        drift.append(abs(energy(out) - e0))
+    assert 1.8 < drift[0] / drift[1] < 2.2 and 1.8 < drift[1] / drift[2] < 2.2
+    assert drift[2] < 0.004 * abs(e0)
+    vh0, _ = oracle.hartree(g, psi, rs)
+    frozen = oracle.td_propagate(g, vloc + vh0, None, psi, 0.025, 40)     # same start, V_H never rebuilt
+    assert abs(energy(frozen) - e0) > 20 * drift[2]
+
+
+def test_td_overlapping_kb_spheres_converge_to_the_dense_propagator(oracle):
+    """Pin for the KB factor NL(tau) with overlapping, off-grid (non-orthonormal) projectors (R-11): NL(tau) agrees with
+    exp(-i V_NL tau) to first order in tau, so the split-operator product converges to the dense exp(-i H t) at
+    least linearly; a wrong sign, a missing dV or a wrong D would leave an error that does not shrink."""
+    g = W.Grid(6, 6, 6, 0.8, 0.8, 0.8)
+    rng = np.random.default_rng(5)
+    centers = np.array([[1.9, 2.3, 2.1], [2.9, 2.6, 2.4]])      # 1.1 bohr apart, radius 1.7: 23 shared points
+    kb = W.kb_projectors(g, centers, radius=1.7, sigma=0.6)
+    a, b = (set(kb.sph_idx[kb.sph_ptr[i]:kb.sph_ptr[i + 1]].tolist()) for i in (0, 1))
+    assert len(a & b) > 10
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0], [0.9, 1.1])
+    H = dense_H(g, vloc, kb)
+    psi = rvec(rng, g, 1)
+    t = 0.4
+    exact = (expm(-1j * H * t) @ psi.reshape(-1)).reshape(psi.shape)
+    errs = []
+    for nst in (8, 16, 32, 64):
+        out = oracle.td_propagate(g, vloc, kb, psi, t / nst, nst)
+        errs.append(np.linalg.norm(out - exact) / np.linalg.norm(exact))
+    assert all(errs[i] / errs[i + 1] > 2.0 for i in range(3))
+    assert errs[-1] < 5e-5
+
+
 # ------------------------------------------------------------------ spectral bounds (NEXT-1; PAPER.md:53)
 def test_power_iteration_bounds_converge_to_dense_extreme_eigenvalues(oracle):
     """Shifted power iteration (R-20) against numpy's eigvalsh of the independently built dense H:
