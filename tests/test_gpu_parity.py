@@ -302,6 +302,58 @@ def test_td_steps_vs_oracle(api, torch_cuda, oracle, mode, use_kb):
     ctx.close()
 
 
+def test_td_hartree_energy_drift_halves_with_dt_at_48_cubed(api, torch_cuda):
+    """A property that holds at any size (no oracle run needed): the TD-Hartree flow conserves
+    E = rho_scale sum_v <psi_v|T + V_loc|psi_v> dV + 1/2 int rho V_H, and the split-operator step with the start-of-step
+    density is first-order consistent with it, so the drift over a fixed time halves with dt (the same pin as
+    tests/test_oracle_physics.py::test_td_hartree_trajectory_conserves_energy_to_first_order_in_dt, here on the CUDA
+    path at 48^3 with 4 vectors; energy from sgw_apply_H and sgw_hartree)."""
+    torch = torch_cuda
+    n, h = 48, 0.5
+    g = W.Grid(n, n, n, h, h, h)
+    L = n * h
+    rng = np.random.default_rng(4)
+    vloc = W.gaussian_vloc(g, rng.uniform(0.3 * L, 0.7 * L, size=(3, 3)), [1.0, 1.5, 0.8], [1.0, 1.2, 0.9])
+    z, y, x = np.meshgrid(*(np.arange(n) * h,) * 3, indexing="ij")
+
+    def packet(c, s, k):
+        d2 = sum(np.minimum(np.abs(a - ci), L - np.abs(a - ci)) ** 2 for a, ci in zip((x, y, z), c))
+        return np.exp(-d2 / (2 * s * s)) * np.exp(1j * (k[0] * x + k[1] * y + k[2] * z))
+
+    kk = 2 * np.pi / L
+    psi = np.stack([packet((10.0, 12.0, 12.5), 1.3, (3 * kk, 0, 0)), packet((13.0, 11.5, 12.0), 1.5, (0, -3 * kk, 2 * kk)),
+                    packet((12.0, 14.0, 11.0), 1.2, (kk, kk, -2 * kk)), packet((11.0, 10.5, 13.5), 1.6, (0, 0, 0))])
+    psi /= np.sqrt((np.abs(psi) ** 2).sum(axis=(1, 2, 3), keepdims=True) * g.dV)
+    rs = 2.0
+    ctx = make_ctx(api, torch, g, vloc, None, 4)
+    src = torch.from_numpy(psi).cuda()
+
+    def energy(t):
+        ht = torch.empty_like(t)
+        ctx.sgw_apply_H(t, ht)
+        e1 = rs * float((t.conj() * ht).sum().real) * g.dV
+        vh, rho = ctx.sgw_hartree(t, rs, want_rho=True)
+        return e1 + 0.5 * float((rho * vh).sum()) * g.dV
+
+    e0 = energy(src)
+    ctx.sgw_set_td(1, rs)
+    drift = []
+    for dt in (0.1, 0.05, 0.025):
+        t = src.clone()
+        ctx.sgw_td_propagate(t, dt, int(round(1.0 / dt)))
+        drift.append(abs(energy(t) - e0))
+    assert 1.7 < drift[0] / drift[1] < 2.3 and 1.7 < drift[1] / drift[2] < 2.3, (e0, drift)
+    assert drift[2] < 0.01 * abs(e0), (e0, drift)
+    ctx.sgw_set_td(0, 0.0)
+    vh0 = ctx.sgw_hartree(src, rs)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda() + vh0)        # V_H frozen at its start value
+    t = src.clone()
+    ctx.sgw_td_propagate(t, 0.025, 40)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    assert abs(energy(t) - e0) > 10 * drift[2], (e0, drift)
+    ctx.close()
+
+
 def test_td_reverse_and_plane_wave(api, torch_cuda):
     torch = torch_cuda
     g, vloc, kb, rng = problem(32, 16, 8, kb=False, seed=4)
