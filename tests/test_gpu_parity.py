@@ -233,6 +233,35 @@ def test_cheb_term_counts_with_kb_and_sub_batches(api, torch_cuda, oracle, nterm
     ctx.close()
 
 
+def test_cheb_low_degree_terms_equal_H_applications_at_cfg1_grid(api, torch_cuda):
+    """Holds at any size: T_1(Ht) psi = Ht psi, T_2 = 2 Ht^2 - 1, T_3 = 4 Ht^3 - 3 Ht with Ht = (H - Eb)/dE (Eq. 3), so
+    unit-coefficient filters on the cfg1 grid (96^3, 8 vectors: several plane groups and z tiles per CTA) must equal
+    products built from sgw_apply_H."""
+    torch = torch_cuda
+    w = W.make_workload("cfg1", nvec=8)
+    ctx = api.context_for(w)
+    src = ctx.sgw_random_vectors(W.SEED_VEC, 0, 8)
+    eb, de = 0.5 * (w.emax + w.emin), 0.5 * (w.emax - w.emin)
+
+    def ht(t):
+        return (ctx.sgw_apply_H(t) - eb * t) / de
+
+    h1 = ht(src); h2 = ht(h1); h3 = ht(h2)
+    want = {1: h1, 2: 2 * h2 - src, 3: 4 * h3 - 3 * h1}
+    for n, ref in want.items():
+        c = np.zeros(n + 1); c[n] = 1.0
+        t = src.clone()
+        ctx.sgw_cheb_filter(t, c, w.emin, w.emax)
+        err = float(((t - ref).abs() ** 2).sum().sqrt() / (ref.abs() ** 2).sum().sqrt())
+        assert err < 1e-12, (n, err)
+    c = np.array([0.3, -0.2, 0.5, 0.1])
+    t = src.clone()
+    ctx.sgw_cheb_filter(t, c, w.emin, w.emax)
+    ref = c[0] * src + c[1] * want[1] + c[2] * want[2] + c[3] * want[3]
+    assert float(((t - ref).abs() ** 2).sum().sqrt() / (ref.abs() ** 2).sum().sqrt()) < 1e-12
+    ctx.close()
+
+
 def test_cheb_against_dense_diagonalisation(api, torch_cuda):
     """No oracle: 8^3 grid, dense H from numpy.fft, eigh, polynomial of the eigenvalues."""
     torch = torch_cuda
