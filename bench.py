@@ -1,9 +1,11 @@
 #!/usr/bin/env python
-"""bench.py -- throughput of the sGW hot path on B200 (contract: see DESIGN.md "Measurement").
+"""bench.py -- throughput of the sGW hot path on B200 (contract: DESIGN.md section 6 "Measurement").
 
-A step = one pass of the whole hot path over one batch: the Chebyshev filter of BASELINE.json
-configs[1] (96^3 grid, Si35H36-shaped potential, 64 +-1 vectors, 512 terms = 511 H applications).
-value = grid-pt * vector * H-applies per second, inputs resident in HBM.
+A step = one pass of the whole hot path over one batch of the LARGEST single-GPU
+config, BASELINE.json configs[4]: 384^3 grid (h = 0.6), Si8381H1620-shaped V_loc + 8381 Kleinman-Bylander spheres,
+all 32 vectors in flight: +-1 vectors from the hash (a1), a slice of 16 of the 2047 Chebyshev applications (a2-a7)
+and 4 of the 500 split-operator steps with the per-step Hartree rebuild (a8-a10) -- the config's 4:1 ratio.
+value = grid-pt * vector * H-applies per second (1 TD step = 1 application, R-19), inputs resident in HBM.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 """
@@ -11,7 +13,9 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -24,23 +28,13 @@ sys.path.insert(0, ROOT)
 
 from paper_2601_21005_b200 import shard, workloads as W  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (z round trip + recurrence on
-# cfg1), from the ncu --set full capture summarised in profiles/r01_v2_cfg1.md: 3.69 GB without and 5.52 GB with
-# the series flush (every third term) -> average per launch
-# lean passes (default): x+y plane pass 3.08 GB without and 5.53 GB with the series flush (every second term),
-# z pass 2.67 GB, from profiles/r01_lean_cfg1.md
-NCU_TRAFFIC_BYTES = {"lean": {"y_acc": (3.08e9 + 5.53e9) / 2.0, "z_cheb": 2.67e9},
-                     "v2": {"z_cheb": (2 * 3.69e9 + 5.52e9) / 3.0, "y_acc": 2.18e9}, "engine": {}}
-TRAFFIC_SOURCE = {"lean": "profiles/r01_lean_cfg1.md", "v2": "profiles/r01_v2_cfg1.md", "engine": "profiles/r01_engine_v3_cfg1.md"}
-KERNEL_NAMES = {"lean": {"y_acc": "plane_lean_kernel<96,8,real,8> (x and y round trips of whole planes, recurrence on store)",
-                         "z_cheb": "axis_lean_kernel<96,8,real,z,cube> (z round trip, accumulate)",
-                         "x_store": "axis_lean_kernel<96,8,real,x>"},
-                "v2": {"y_acc": "plane_kernel<96,24> (x+y round trips)",
-                       "z_cheb": "pipe_kernel<96,8,POpCheb> (z round trip + recurrence)"},
-                "engine": {"engine": "engine_kernel<96,8> (all passes)"}}
-METRIC = "grid-pt*vector H-applies/s (Chebyshev filter)"
+METRIC = "grid-pt*vector H-applies/s (Chebyshev filter + TD step)"
 UNIT = "grid-pt*vec*H-applies/s"
-WORKLOAD = "cfg1"
+WORKLOAD = "cfg4"
+SLICE_APPLIES = 16          # of the 2047 Chebyshev applications per step
+SLICE_TD = 4                # of the 500 TD-Hartree steps per step
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
+SUBCELL_N = 128             # oracle timing sample: central 128^3 sub-cell of the workload
 
 
 def measured_peaks():
@@ -49,6 +43,15 @@ def measured_peaks():
         d = json.load(open(p))
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(kernel_key):
+    """dram bytes per launch of a kernel from the ncu --set full capture summarised in profiles/ (or None)."""
+    if not os.path.exists(TRAFFIC_JSON):
+        return None, None
+    d = json.load(open(TRAFFIC_JSON))
+    e = d.get("kernels", {}).get(kernel_key)
+    return (e["dram_bytes_per_launch"], d.get("source")) if e else (None, d.get("source"))
 
 
 class ClockSampler:
@@ -96,46 +99,115 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def oracle_sample(w, nvec, napplies):
-    """Time the oracle (double, OpenMP over vectors) on nvec vectors x napplies H applications."""
+# ------------------------------------------------------------------------------------------------------------
+# the oracle arm (cpu_baseline and --impl reference): the only place bench.py executes oracle/
+# ------------------------------------------------------------------------------------------------------------
+_SUB = {}
+
+
+def subcell_workload():
+    if "w" not in _SUB:
+        _SUB["w"] = W.make_workload(WORKLOAD, n=SUBCELL_N, nterms=2048, subcell=True)
+    return _SUB["w"]
+
+
+def oracle_sample(nvec, napplies, nsteps):
+    """Time the oracle (double, OpenMP over vectors) on the central SUBCELL_N^3 sub-cell of the bench workload (same
+    spacing, its atoms and KB spheres): nvec vectors x (napplies Chebyshev applications + nsteps TD-Hartree steps)."""
     from oracle import sgw_oracle as o
     o.build()
+    w = subcell_workload()
     threads = o.max_threads()
     nvec = min(nvec, max(1, threads))
     psi = o.random_vectors(w.grid, W.SEED_VEC, 0, nvec)
     coeffs = np.ascontiguousarray(w.coeffs[:napplies + 1])
     t0 = time.perf_counter()
-    o.cheb_filter(w.grid, w.vloc, w.kb, psi, coeffs, w.emin, w.emax, ld=False)
+    psi = o.cheb_filter(w.grid, w.vloc, w.kb, psi, coeffs, w.emin, w.emax, ld=False)
+    if nsteps:
+        o.td_propagate(w.grid, w.vloc, w.kb, psi, w.dt, nsteps, 1, 2.0 / (nvec * w.grid.dV), ld=False)
     dt = time.perf_counter() - t0
-    units = w.grid.ng * nvec * napplies
-    return units / dt, dt, nvec, min(threads, nvec)
+    units = w.grid.ng * nvec * (napplies + nsteps)
+    what = (f"central {SUBCELL_N}^3 sub-cell of {WORKLOAD} (h=0.6, {w.atoms}, {w.kb.nsphere} KB spheres): {nvec} vectors x "
+            f"({napplies} Chebyshev applications + {nsteps} TD-Hartree steps)")
+    return units / dt, dt, nvec, min(threads, nvec), what
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    w = W.make_workload(WORKLOAD)
     cores = os.cpu_count() or 1
-    nv, nap = min(w.nvec, cores), 4
-    for _ in range(args.warmup):
-        oracle_sample(w, nv, 1)
-    tot_units, tot_t, used = 0.0, 0.0, 1
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(cores, 1, 0)
+    tot_units, tot_t, used, what = 0.0, 0.0, 1, ""
     for _ in range(args.steps):
-        v, dt, nvec, used = oracle_sample(w, nv, nap)
+        v, dt, nvec, used, what = oracle_sample(cores, 4, 1)
         tot_units += v * dt
         tot_t += dt
     val = tot_units / tot_t
-    sample = f"{nv} vectors x {nap} H applies of the {w.nterms}-term filter per step, {WORKLOAD} grid and potential"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{WORKLOAD}: 96^3 grid h=0.45, {w.atoms}-shaped V_loc, 512-term sqrt-Fermi-Dirac filter",
-                   "sample": sample},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
+        "config": {"workload": workload_name(32), "sample": what + " per step (4:1 as in the GPU arm's slice)"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": used, "kind": "oracle", "sample": what + " per step"},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
+
+
+def workload_name(nvec):
+    return (f"{WORKLOAD} (BASELINE.json configs[4], the largest single-GPU config): 384^3 grid h=0.6, Si8381H1620-shaped V_loc + "
+            f"8381 KB spheres (4 projectors each), {nvec} +-1 vectors in flight per GPU; per step: {SLICE_APPLIES} of the 2047 "
+            f"Chebyshev applications (sqrt-Fermi-Dirac coefficients 0..{SLICE_APPLIES}) + {SLICE_TD} of the 500 TD steps "
+            f"(dt=0.05, Hartree rebuilt every step)")
+
+
+# ------------------------------------------------------------------------------------------------------------
+# the GPU arm
+# ------------------------------------------------------------------------------------------------------------
+AXES = {0: "x", 1: "y", 2: "z"}
+KINDS = ["store", "acc", "hfin", "cheb", "td", "mul3d", "fwd", "inv", "kb_project", "kb_scatter", "density"]
+
+
+def collect_passes(ctx):
+    out = {}
+    for a in range(3):
+        for k in range(len(KINDS)):
+            n, ms = ctx.sgw_profile_get(a, k)
+            if n:
+                out[f"{AXES[a]}_{KINDS[k]}" if k < 8 else KINDS[k]] = {"launches": n, "ms_total": ms}
+    return out
+
+
+def pass_model(passes, nvec, n, kb_frac):
+    """Algorithmic bytes per grid-pt*vector of each profiled launch kind and a display name."""
+    plane_f = "x_store" not in passes            # filter: fused x+y plane pass (no separate x launch)
+    plane_t = "x_td" not in passes
+    m = {
+        "x_store": (48.0 + 16.0 + 8.0 / nvec, f"axis_lean_kernel<{n},8,real,x> (x round trip, potential, recurrence, series every 2nd term)"),
+        "y_acc": ((48.0 + 16.0 + 8.0 / nvec, f"plane_lean/plane_cluster kernel<{n},8,real> (x and y round trips of whole planes)") if plane_f
+                  else (48.0, f"axis_lean_kernel<{n},8,real,y> (y round trip, accumulate)")),
+        "z_cheb": (48.0, f"axis_lean_kernel<{n},8,real,z> (z round trip, accumulate)"),
+        "x_td": (32.0 + 16.0 / nvec, f"axis_lean_kernel<{n},8,complex,x> (x factor of exp(-iT dt), phase on load)"),
+        "y_td": ((32.0 + 16.0 / nvec, f"plane_lean kernel<{n},8,complex> (x and y factors of exp(-iT dt))") if plane_t
+                 else (32.0, f"axis_lean_kernel<{n},8,complex,y> (y factor of exp(-iT dt))")),
+        "z_td": (32.0 + 16.0 / nvec, f"axis_lean_kernel<{n},8,complex,z> (z factor, phase / density on store)"),
+        "kb_project": (16.0 * kb_frac + 32.0 * kb_frac / nvec, "kb_project_kernel<4> (gather-dot over sphere points)"),
+        "kb_scatter": (32.0 * kb_frac + 32.0 * kb_frac / nvec, "kb_scatter_kernel<4> (FP64 atomics where spheres overlap)"),
+        "density": (16.0, "density_kernel (rho from all vectors)"),
+    }
+    return m
+
+
+def bound_fraction(bytes_per_unit, flops_per_unit, units, seconds, hbm_gbs, fp64_flops):
+    """achieved fraction of the roofline = W * max(B_c / BW, F_c / P64) / t."""
+    t_hbm = bytes_per_unit / (hbm_gbs * 1e9)
+    t_f64 = flops_per_unit / fp64_flops if fp64_flops else 0.0
+    lim = max(t_hbm, t_f64)
+    return {"bytes_per_unit": bytes_per_unit, "flops_per_unit": flops_per_unit,
+            "bound": "hbm" if t_hbm >= t_f64 else "fp64",
+            "achieved": bytes_per_unit * units / seconds / 1e9, "unit": "GB/s", "frac": lim * units / seconds,
+            "frac_hbm": t_hbm * units / seconds, "frac_fp64": t_f64 * units / seconds}
 
 
 def run_gpu(args):
@@ -153,14 +225,17 @@ def run_gpu(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    w = W.make_workload(WORKLOAD, nterms=args.nterms)
+    w = W.make_workload(WORKLOAD, nvec=args.nvec)
     g = w.grid
-    nvec, napply = w.nvec, w.nterms - 1
-    units_rank = g.ng * nvec * napply
+    nvec = w.nvec
+    coeffs = np.ascontiguousarray(w.coeffs[:SLICE_APPLIES + 1])
+    units_f, units_t = g.ng * nvec * SLICE_APPLIES, g.ng * nvec * SLICE_TD
+    units_rank = units_f + units_t
     stream = torch.cuda.current_stream(dev)
     ctx = api.context_for(w, max_nvec=nvec, stream=stream, device=f"cuda:{local}")
-    psi0 = ctx.sgw_random_vectors(W.SEED_VEC, shard.first_vector(rank, nvec), nvec)   # each rank filters its own vectors
-    psi = torch.empty_like(psi0)
+    first = shard.first_vector(rank, nvec)                   # each rank owns its own vectors (replicas, weak scaling)
+    psi = torch.empty((nvec,) + g.shape, dtype=torch.complex128, device=dev)
+    ctx.sgw_set_td(1, w.rho_scale)
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -168,9 +243,18 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    def step():
-        psi.copy_(psi0)
-        ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+
+    def step(e=None):
+        ctx.sgw_random_vectors(W.SEED_VEC, first, nvec, psi)                 # a1
+        if e:
+            e[0].record(stream)
+        ctx.sgw_cheb_filter(psi, coeffs, w.emin, w.emax)                      # a2-a7
+        if e:
+            e[1].record(stream)
+        ctx.sgw_td_propagate(psi, w.dt, SLICE_TD)                             # a8-a10
+        if e:
+            e[2].record(stream)
 
     for _ in range(args.warmup):
         step()
@@ -178,288 +262,288 @@ def run_gpu(args):
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    ctx.sgw_profile_reset()
-    ctx.sgw_profile_enable(1)
     l0 = ctx.sgw_launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(stream)
-    for _ in range(args.steps):
-        step()
+    for k in range(args.steps):
+        step(ev[k])
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
     launches = ctx.sgw_launch_count() - l0
     clocks = sampler.stop() if rank == 0 else None
-    prof = {(a, k): ctx.sgw_profile_get(a, k) for a in range(3) for k in range(8)}
-    ctx.sgw_profile_enable(0)
+    ms_f = sum(e[0].elapsed_time(e[1]) for e in ev)
+    ms_t = sum(e[1].elapsed_time(e[2]) for e in ev)
     ms = shard.max_over_ranks(ms, dev)
     value = shard.whole_job_rate(units_rank, world, args.steps, ms)
+    fp64_flops = ctx.sgw_probe_fp64()                                         # at the clocks the run leaves the device at
 
-    # ---- end to end: host buffers, H2D of the inputs and D2H of the result inside the timed region
-    h_in = psi0.cpu().pin_memory()
-    h_out = torch.empty_like(h_in).pin_memory()
-    nbytes = h_in.numel() * 16
+    # ---- per-pass breakdown: one separate step with an event pair around every launch (not the headline loop)
+    ctx.sgw_profile_reset()
+    ctx.sgw_profile_enable(1)
+    ctx.sgw_random_vectors(W.SEED_VEC, first, nvec, psi)
+    ctx.sgw_cheb_filter(psi, coeffs, w.emin, w.emax)
+    passes_f = collect_passes(ctx)
+    ctx.sgw_profile_reset()
+    ctx.sgw_td_propagate(psi, w.dt, SLICE_TD)
+    passes_t = collect_passes(ctx)
+    ctx.sgw_profile_enable(0)
+    norms = ctx.sgw_norms(psi)
+    finite = bool(torch.isfinite(norms).all())
 
-    def step_e2e():
-        psi.copy_(h_in, non_blocking=True)
-        ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
-        h_out.copy_(psi, non_blocking=True)
+    # ---- end to end: host buffers, H2D of the start vectors and D2H of the result inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        e2e = run_e2e(torch, ctx, w, psi, coeffs, stream, dev, first, barrier, min(args.steps, 2), world, units_rank)
 
-    step_e2e()
-    barrier()
-    e0.record(stream)
-    for _ in range(args.steps):
-        step_e2e()
-    e1.record(stream)
-    barrier()
-    ms_e2e = e0.elapsed_time(e1)
-    ms_e2e = shard.max_over_ranks(ms_e2e, dev)
-    e2e_value = shard.whole_job_rate(units_rank, world, args.steps, ms_e2e)
-    checksum = float(torch.view_as_real(h_out).abs().sum())
-
-    td, samples, libcmp = None, None, None
-    if world == 1 and not args.no_td:
-        td = run_td(torch, api, dev, stream, args)
-        samples = run_config_samples(torch, api, dev, stream)
-        libcmp = run_library_comparison(torch, ctx, w, psi0, dev, stream)
+    others = None
+    if world == 1 and not args.no_others:
+        del psi
+        ctx.close()
+        torch.cuda.empty_cache()
+        others = run_other_configs(torch, api, dev, stream, args, fp64_flops)
 
     if rank == 0:
         peak, peak_src = measured_peaks()
-        names = {0: "x", 1: "y", 2: "z"}
-        kinds = ["store", "acc", "hfin", "cheb", "td", "mul3d", "fwd", "inv"]
-        passes = {f"{names[a]}_{kinds[k]}": {"launches": n, "ms_total": t_} for (a, k), (n, t_) in prof.items() if n}
-        impl = {"0": "v2", "1": "engine"}.get(os.environ.get("SGW_ENGINE", "2"), "lean")
-        if impl == "engine" or not passes:
-            # pass engine: one persistent kernel runs all passes of up to 256 terms; its launch time is the step's
-            passes = {"engine": {"launches": max(1, int(launches) // 2), "ms_total": ms}}
-        dom = max(passes.items(), key=lambda kv: kv[1]["ms_total"])
-        # algorithmic bytes per grid-pt*vector of each pass: complex = 16 B
-        series_share = 32.0 / 3.0                                   # series r/w every third term
-        bytes_per_unit = {"x_store": 32.0, "y_acc": 48.0, "z_cheb": 64.0 + series_share + 8.0 / nvec,
-                          "engine": (96.0 + 16.0 + 8.0 / nvec)}          # engine: per term, all three passes
-        if impl == "lean":
-            # x+y plane pass: read cur and acc, write acc (the x->y transpose goes through L2), series r/w every
-            # second term, potential table; z pass: read cur and acc, write acc
-            bytes_per_unit = {"y_acc": 48.0 + 16.0 + 8.0 / nvec, "z_cheb": 48.0, "x_store": 48.0}
-        dn, dv = dom
+        kb_frac = float(w.kb.sph_idx.size) / g.ng
+        model = pass_model({**passes_f, **passes_t}, nvec, g.nx, kb_frac)
+        allp = {k: dict(v, stage="filter") for k, v in passes_f.items()}
+        allp.update({k: dict(v, stage="td") for k, v in passes_t.items()})
+        dn, dv = max(allp.items(), key=lambda kv: kv[1]["ms_total"])
+        bpu, kname = model.get(dn, (32.0, dn))
         units_launch = g.ng * nvec
-        if dn == "engine":
-            units_launch = units_rank * args.steps / dv["launches"]
         avg_ms = dv["ms_total"] / dv["launches"]
-        ach = bytes_per_unit.get(dn, 32.0) * units_launch / (avg_ms * 1e-3) / 1e9
-        strict_bytes = 80.0 + 8.0 / nvec                            # compulsory bytes per term
-        term_gbs = strict_bytes * units_rank * args.steps / (ms * 1e-3) / 1e9
-        moved = sum(bytes_per_unit.get(k_, 32.0) * units_launch * v_["launches"] for k_, v_ in passes.items())
-        cpu_val, cpu_dt, cpu_nv, cpu_cores = oracle_sample(w, os.cpu_count() or 1, 32)
+        ach = bpu * units_launch / (avg_ms * 1e-3) / 1e9
+        traffic, traffic_src = ncu_traffic(dn)
+        lg = math.log2(g.ng)
+        cheb = bound_fraction(80.0 + 8.0 / nvec, 10.0 * lg + 20.0, units_f * args.steps, ms_f * 1e-3, peak, fp64_flops)
+        td = bound_fraction(32.0 + 40.0 / nvec, 10.0 * lg + 30.0, units_t * args.steps, ms_t * 1e-3, peak, fp64_flops)
+        for name, ps in (("filter", passes_f), ("td", passes_t)):
+            for k_, v_ in ps.items():
+                b_ = model.get(k_, (None, None))[0]
+                v_["avg_ms"] = v_["ms_total"] / v_["launches"]
+                if b_:
+                    v_["bytes_per_unit"] = b_
+                    v_["algorithmic_gbs"] = b_ * units_launch / (v_["avg_ms"] * 1e-3) / 1e9
+                    v_["frac_of_hbm_peak"] = v_["algorithmic_gbs"] / peak
+        cpu_val, cpu_dt, cpu_nv, cpu_cores, cpu_what = oracle_sample(os.cpu_count() or 1, 4, 1)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{WORKLOAD}: 96^3 grid h=0.45, {w.atoms}-shaped V_loc, {nvec} +-1 vectors per GPU, "
-                                   f"{w.nterms}-term sqrt-Fermi-Dirac Chebyshev filter ({napply} H applies)",
-                       "l2": "inputs larger than L2 (each array 906 MB per GPU)", "passes_per_term": 3,
-                       "launches_per_term": 2 if impl != "engine" else 0},
+            "config": {"workload": workload_name(nvec),
+                       "l2": f"inputs larger than L2 (each vector array {g.ng * nvec * 16 / 1e9:.1f} GB per GPU)",
+                       "timing": "headline loop without per-launch events; pass breakdown from one separate profiled step",
+                       "kinetic_operator": "full 1/2 k^2 (the paper's E_cut = 28 Ha cap is reading R-14: see sgw_set_kinetic_cutoff / other_configs)"},
             "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
-                    "ms_per_step": ms_e2e / args.steps, "checksum": checksum},
+            "e2e": e2e,
             "gpu_launches": int(launches),
-            "roofline": {"bound": "hbm", "implementation": impl, "kernel": KERNEL_NAMES[impl].get(dn, dn),
-                         "achieved": ach, "peak": peak,
-                         "unit": "GB/s", "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES[impl].get(dn),
-                         "traffic_source": TRAFFIC_SOURCE[impl] + " (ncu --set full, dram bytes per launch)",
-                         "algorithmic_bytes_per_launch": bytes_per_unit.get(dn, 32.0) * units_launch, "peak_source": peak_src,
-                         "avg_launch_ms": avg_ms, "bytes_per_unit": bytes_per_unit.get(dn, 32.0),
-                         "kernel_share_of_step": dv["ms_total"] / ms,
-                         "term_strict": {"bytes_per_unit": strict_bytes, "achieved": term_gbs, "frac": term_gbs / peak},
-                         "term_moved": {"achieved": moved / (ms * 1e-3) / 1e9, "frac": moved / (ms * 1e-3) / 1e9 / peak},
-                         "passes": passes},
-            "td": td,
-            "other_configs": samples,
-            "library_comparison": libcmp,
-            "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",
-                             "sample": f"{cpu_nv} vectors x 32 H applies of the same filter, {WORKLOAD} grid ({cpu_dt:.1f} s)"},
+            "stage_rates": {"filter_units_per_s": units_f * args.steps / (ms_f * 1e-3), "filter_ms_per_application": ms_f / args.steps / SLICE_APPLIES,
+                            "td_units_per_s": units_t * args.steps / (ms_t * 1e-3), "td_ms_per_step": ms_t / args.steps / SLICE_TD},
+            "roofline": {"bound": "hbm", "kernel": kname, "stage": dv["stage"], "achieved": ach, "peak": peak, "unit": "GB/s",
+                         "frac": ach / peak, "traffic": traffic, "traffic_source": traffic_src,
+                         "algorithmic_bytes_per_launch": bpu * units_launch, "bytes_per_unit": bpu, "avg_launch_ms": avg_ms,
+                         "peak_source": peak_src, "kernel_share_of_profiled_step": dv["ms_total"] / sum(v["ms_total"] for v in allp.values()),
+                         "term_strict": cheb, "passes": passes_f},
+            "roofline_td": dict(td, passes=passes_t, peak=peak),
+            "fp64_peak_measured": {"flops_per_s": fp64_flops, "how": "sgw_probe_fp64: dependent-free DFMA loop right after the timed region",
+                                   "nominal_flops_per_s": 148 * 64 * 2 * 1.965e9},
+            "checks": {"finite": finite},
+            "other_configs": others,
+            "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores, "kind": "oracle", "sample": f"{cpu_what} ({cpu_dt:.1f} s)"},
         }
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 
 
-def run_td(torch, api, dev, stream, args):
-    """Second stage of the metric: split-operator steps with the per-step Hartree rebuild on BASELINE.json
-    configs[2] (128^3, Si87H76-shaped, 16 filtered vectors, dt = 0.05); a 100-step sample of the 2000."""
+def run_e2e(torch, ctx, w, psi, coeffs, stream, dev, first, barrier, steps, world, units_rank):
+    """The same step through the C-ABI with HOST buffers: start vectors copied host -> device and the result copied
+    device -> host inside the timed region (one pinned buffer per vector, so a failed pin degrades per vector)."""
+    nvec = w.nvec
+    ctx.sgw_random_vectors(W.SEED_VEC, first, nvec, psi)
+    pinned = True
+    h_in, h_out = [], []
+    for v in range(nvec):
+        try:
+            a = torch.empty(w.grid.shape, dtype=torch.complex128, pin_memory=True)
+            b = torch.empty(w.grid.shape, dtype=torch.complex128, pin_memory=True)
+        except RuntimeError:
+            pinned = False
+            a = torch.empty(w.grid.shape, dtype=torch.complex128)
+            b = torch.empty(w.grid.shape, dtype=torch.complex128)
+        a.copy_(psi[v])
+        h_in.append(a)
+        h_out.append(b)
+    nbytes = nvec * w.grid.ng * 16
+
+    def step():
+        for v in range(nvec):
+            psi[v].copy_(h_in[v], non_blocking=True)
+        ctx.sgw_cheb_filter(psi, coeffs, w.emin, w.emax)
+        ctx.sgw_td_propagate(psi, w.dt, SLICE_TD)
+        for v in range(nvec):
+            h_out[v].copy_(psi[v], non_blocking=True)
+
+    step()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms = shard.max_over_ranks(e0.elapsed_time(e1), dev)
+    checksum = float(sum(float(torch.view_as_real(b[0]).abs().sum()) for b in h_out))
+    return {"value": shard.whole_job_rate(units_rank, world, steps, ms), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+            "d2h_bytes_per_step": nbytes, "ms_per_step": ms / steps, "steps": steps, "pinned": pinned, "checksum_plane0": checksum,
+            "note": "the config uploads once per 2047 applications + 500 steps; this slice pays the same transfer for 16 + 4"}
+
+
+def timed(torch, stream, dev, fn):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(dev)
+    e0.record(stream)
+    fn()
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    return e0.elapsed_time(e1)
+
+
+def run_other_configs(torch, api, dev, stream, args, fp64_flops):
+    """The other BASELINE.json configs, each with its own strict-roofline fraction: cfg1 and cfg2 at full vector count
+    and (cfg1) full length, cfg3 as one 64-vector sub-batch, cfg0 (launch-latency bound)."""
+    peak, _ = measured_peaks()
+    out = {}
+    # cfg1: the whole 512-term filter on 64 vectors (round 1's headline)
+    w = W.make_workload("cfg1")
+    ctx = api.context_for(w, max_nvec=w.nvec, stream=stream, device=str(dev))
+    psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
+    ctx.sgw_cheb_filter(psi, w.coeffs[:9], w.emin, w.emax)
+    best = min(timed(torch, stream, dev, lambda: (ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec, psi),
+                                                   ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax))) for _ in range(2))
+    units = w.grid.ng * w.nvec * (w.nterms - 1)
+    out["cfg1"] = {"what": "96^3, Si35H36 V_loc, 64 vectors, all 512 terms (511 applications), RNG included", "filter_ms": best,
+                   "filter_units_per_s": units / (best * 1e-3),
+                   "term_strict": bound_fraction(80.0 + 8.0 / w.nvec, 10.0 * math.log2(w.grid.ng) + 20.0, units, best * 1e-3, peak, fp64_flops)}
+    # ADVICE r1: the cost of the paper's operator with its kinetic-energy cutoff (non-separable, five-pass route)
+    if hasattr(ctx, "sgw_set_kinetic_cutoff"):
+        ctx.sgw_set_kinetic_cutoff(28.0)
+        wc = W.make_workload("cfg1")
+        emax_c = 3 * 0 + min(28.0, 0.5 * 3 * (math.pi / w.grid.hx) ** 2) + float(wc.vloc.max())
+        co = W.cheb_coeffs(W.sqrt_fermi, w.emin, emax_c, 65)
+        ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec, psi)
+        msc = timed(torch, stream, dev, lambda: ctx.sgw_cheb_filter(psi, co, w.emin, emax_c))
+        out["cfg1"]["with_kinetic_cutoff_28Ha"] = {"what": "same grid and vectors, kinetic operator min(1/2 k^2, 28 Ha) (P:142), 64 applications",
+                                                    "filter_units_per_s": w.grid.ng * w.nvec * 64 / (msc * 1e-3)}
+        ctx.sgw_set_kinetic_cutoff(0.0)
+    ctx.close()
+    del psi
+    torch.cuda.empty_cache()
+    # cfg2: TD steps with the Hartree rebuild
     w = W.make_workload("cfg2", nterms=33)
     ctx = api.context_for(w, max_nvec=w.nvec, stream=stream, device=str(dev))
     psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
-    ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)            # filtered start vectors (untimed)
+    ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
     ctx.sgw_set_td(1, w.rho_scale)
-    nsteps = args.td_steps
-    ctx.sgw_td_propagate(psi, w.dt, 10)                            # warm-up
-    norms0 = ctx.sgw_norms(psi).cpu().numpy()
-    torch.cuda.synchronize(dev)
-    l0 = ctx.sgw_launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    ctx.sgw_td_propagate(psi, w.dt, nsteps)
-    e1.record(stream)
-    torch.cuda.synchronize(dev)
-    ms = e0.elapsed_time(e1)
-    norms = ctx.sgw_norms(psi).cpu().numpy()
-    units = w.grid.ng * w.nvec * nsteps
-    peak, _ = measured_peaks()
-    strict = 32.0 + 40.0 / w.nvec                                  # SURVEY 8(d): compulsory bytes per grid-pt*vector*step
-    gbs = strict * units / (ms * 1e-3) / 1e9
-    out = {"metric": "grid-pt*vector H-applies/s (TD step)", "value": units / (ms * 1e-3), "unit": UNIT,
-           "workload": f"cfg2: 128^3 grid h=0.5, {w.atoms}-shaped V_loc, {w.nvec} filtered vectors, dt=0.05, Hartree "
-                       f"rebuilt every step; {nsteps} of the 2000 steps timed",
-           "ms_per_step": ms / nsteps, "gpu_launches": int(ctx.sgw_launch_count() - l0),
-           "strict": {"bytes_per_unit": strict, "achieved": gbs, "frac": gbs / peak},
-           "norm_drift": float(np.max(np.abs(norms / norms0 - 1.0)))}
+    ctx.sgw_td_propagate(psi, w.dt, 10)
+    n0 = ctx.sgw_norms(psi)
+    nst = args.td_steps
+    ms = timed(torch, stream, dev, lambda: ctx.sgw_td_propagate(psi, w.dt, nst))
+    units = w.grid.ng * w.nvec * nst
+    out["cfg2"] = {"what": f"128^3, Si87H76 V_loc, 16 filtered vectors, {nst} of the 2000 TD-Hartree steps", "td_ms_per_step": ms / nst,
+                   "td_units_per_s": units / (ms * 1e-3), "norm_drift": float((ctx.sgw_norms(psi) / n0 - 1.0).abs().max()),
+                   "td_strict": bound_fraction(32.0 + 40.0 / w.nvec, 10.0 * math.log2(w.grid.ng) + 30.0, units, ms * 1e-3, peak, fp64_flops)}
+    ctx.close()
+    del psi
+    torch.cuda.empty_cache()
+    # cfg3: one 64-vector sub-batch of the 256
+    w = W.make_workload("cfg3", nvec=64)
+    ctx = api.context_for(w, max_nvec=64, stream=stream, device=str(dev))
+    psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, 64)
+    ctx.sgw_cheb_filter(psi[:2].clone(), w.coeffs[:3], w.emin, w.emax)
+    ms = timed(torch, stream, dev, lambda: ctx.sgw_cheb_filter(psi, w.coeffs[:17], w.emin, w.emax))
+    units = w.grid.ng * 64 * 16
+    ctx.sgw_set_td(1, w.rho_scale)
+    ctx.sgw_td_propagate(psi, w.dt, 1)
+    mst = timed(torch, stream, dev, lambda: ctx.sgw_td_propagate(psi, w.dt, 4))
+    out["cfg3"] = {"what": "256^3, Si705H300 V_loc + 705 KB spheres, one 64-vector sub-batch of the 256, 16 of the 2047 applications; 4 TD-Hartree steps",
+                   "filter_units_per_s": units / (ms * 1e-3),
+                   "term_strict": bound_fraction(80.0 + 8.0 / 64, 10.0 * math.log2(w.grid.ng) + 20.0, units, ms * 1e-3, peak, fp64_flops),
+                   "td_units_per_s": w.grid.ng * 64 * 4 / (mst * 1e-3)}
+    ctx.close()
+    del psi
+    torch.cuda.empty_cache()
+    # cfg0: launch-latency bound; the repeated call replays a cached CUDA graph
+    w = W.make_workload("cfg0")
+    ctx = api.context_for(w, max_nvec=w.nvec, stream=stream, device=str(dev))
+    psi0 = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
+    psi = psi0.clone()
+    best = None
+    for _ in range(4):
+        psi.copy_(psi0)
+        m_ = timed(torch, stream, dev, lambda: ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax))
+        best = m_ if best is None or m_ < best else best
+    out["cfg0"] = {"what": "32^3, 4 vectors, all 128 terms (launch-latency bound: roofline fraction not meaningful)", "filter_ms": best,
+                   "filter_units_per_s": w.grid.ng * w.nvec * 127 / (best * 1e-3)}
     ctx.close()
     return out
 
 
-def run_library_comparison(torch, ctx, w, psi0, dev, stream):
-    """Context only (BASELINE.json north_star: "cuFFT is only a timed comparison"): one H application on the bench
-    workload built from torch.fft.fftn / ifftn (cuFFT) and torch element-wise ops, against sgw_apply_H."""
-    import math
-    g = w.grid
+def write_traffic(csv_path, source):
+    """Post-processing of an ncu raw page (ncu -i <rep> --page raw --csv > csv): dram bytes per launch per kernel kind,
+    written to profiles/r02_traffic.json, which the bench line's roofline.traffic reads."""
+    import csv
+    rows = list(csv.reader(open(csv_path)))
+    hdr = rows[0]
+    col = {n: i for i, n in enumerate(hdr)}
+    rd, wr, nm, dur = col["dram__bytes_read.sum"], col["dram__bytes_write.sum"], col["Kernel Name"], col["gpu__time_duration.sum"]
+    units = rows[1]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
 
-    def k1(n, h):
-        return 2.0 * math.pi * torch.fft.fftfreq(n, d=h, device=dev, dtype=torch.float64)
-    kz, ky, kx = torch.meshgrid(k1(g.nz, g.hz), k1(g.ny, g.hy), k1(g.nx, g.hx), indexing="ij")
-    k2 = 0.5 * (kx * kx + ky * ky + kz * kz)
-    v = torch.from_numpy(w.vloc).to(dev)
-
-    def lib_apply(x):
-        return torch.fft.ifftn(k2 * torch.fft.fftn(x, dim=(1, 2, 3)), dim=(1, 2, 3)) + v * x
-
-    out = torch.empty_like(psi0)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    res = {}
-    for name, fn in (("cufft_torch", lambda: lib_apply(psi0)), ("sgw_apply_H", lambda: ctx.sgw_apply_H(psi0, out))):
-        fn()
-        torch.cuda.synchronize(dev)
-        e0.record(stream)
-        for _ in range(5):
-            r = fn()
-        e1.record(stream)
-        torch.cuda.synchronize(dev)
-        res[name] = g.ng * w.nvec * 5 / (e0.elapsed_time(e1) * 1e-3)
-        del r
-    ref = lib_apply(psi0)
-    res["max_abs_diff"] = float((ref - out).abs().max())
-    res["what"] = "one H application on the bench workload; torch.fft (cuFFT) + element-wise ops vs sgw_apply_H; context only"
-    del ref, out
-    torch.cuda.empty_cache()
-    return res
-
-
-def run_config_samples(torch, api, dev, stream):
-    """Short samples of the other BASELINE.json configs (shapes and potentials as specified, fewer vectors / terms /
-    steps, stated per entry): evidence that every config runs on the same kernels, not headline numbers."""
-    out = {}
-    specs = [("cfg0", dict(), 128, 0, "32^3, 4 vectors, all 128 terms (launch-latency bound; replayed as one cached CUDA graph)"),
-             ("cfg3", dict(nvec=8, nterms=17), 17, 4, "256^3, Si705H300 + KB projectors, 8 of 256 vectors, 16 of 2047 applications, 4 TD-Hartree steps"),
-             ("cfg4", dict(nvec=2, nterms=9), 9, 2, "384^3, Si8381H1620 + KB projectors, 2 of 32 vectors, 8 of 2047 applications, 2 of 500 TD-Hartree steps")]
-    for name, kw, nterms, nsteps, what in specs:
-        w = W.make_workload(name, **kw)
-        ctx = api.context_for(w, max_nvec=w.nvec, stream=stream, device=str(dev))
-        psi0 = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
-        psi = psi0.clone()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        best = None
-        for _ in range(3):
-            psi.copy_(psi0)
-            torch.cuda.synchronize(dev)
-            e0.record(stream)
-            ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
-            e1.record(stream)
-            torch.cuda.synchronize(dev)
-            ms = e0.elapsed_time(e1)
-            best = ms if best is None or ms < best else best
-        entry = {"sample": what, "filter_units_per_s": w.grid.ng * w.nvec * (nterms - 1) / (best * 1e-3), "filter_ms": best}
-        if nsteps:
-            ctx.sgw_set_td(1, w.rho_scale)
-            ctx.sgw_td_propagate(psi, w.dt, 1)
-            torch.cuda.synchronize(dev)
-            e0.record(stream)
-            ctx.sgw_td_propagate(psi, w.dt, nsteps)
-            e1.record(stream)
-            torch.cuda.synchronize(dev)
-            ms = e0.elapsed_time(e1)
-            entry["td_units_per_s"] = w.grid.ng * w.nvec * nsteps / (ms * 1e-3)
-            entry["td_ms_per_step"] = ms / nsteps
-        out[name] = entry
-        ctx.close()
-        del psi, psi0
-        torch.cuda.empty_cache()
-    return out
+    def key_of(name):
+        fam = "td" if ("true" in name.split("<")[1].split(">")[0].split(",")[2:3] or ", true" in name) and "lean" in name else None
+        if "kb_project" in name:
+            return "kb_project"
+        if "kb_scatter" in name:
+            return "kb_scatter"
+        if "density" in name:
+            return "density"
+        if "plane" in name:
+            return "y_td" if fam else "y_acc"
+        if "axis_lean" in name:
+            args_ = name.split("<")[1].split(">")[0].replace(" ", "").split(",")
+            axis = {"0": "x", "1": "y", "2": "z"}[args_[3]]
+            cplx = args_[2] in ("true", "1")
+            if cplx:
+                return f"{axis}_td"
+            return {"x": "x_store", "y": "y_acc", "z": "z_cheb"}[axis]
+        return None
+    acc = {}
+    for r in rows[2:]:
+        k = key_of(r[nm])
+        if not k:
+            continue
+        b = float(r[rd].replace(",", "")) * scale.get(units[rd], 1.0) + float(r[wr].replace(",", "")) * scale.get(units[wr], 1.0)
+        e = acc.setdefault(k, {"launches": 0, "bytes": 0.0, "kernel": r[nm][:120]})
+        e["launches"] += 1
+        e["bytes"] += b
+    out = {"source": source, "kernels": {k: {"dram_bytes_per_launch": v["bytes"] / v["launches"], "launches": v["launches"], "kernel": v["kernel"]}
+                                          for k, v in acc.items()}}
+    json.dump(out, open(TRAFFIC_JSON, "w"), indent=1)
+    print(json.dumps(out, indent=1))
 
 
-def run_full_config(args):
-    """One full-size, full-length run of a BASELINE.json config (not the bench contract's line: a separate report
-    used for profiles/r01_full_configs.md): the whole filter on all vectors, then (cfg2, cfg4) the whole propagation."""
-    import torch
-    from paper_2601_21005_b200 import api
-    dev = torch.device("cuda", 0)
-    torch.cuda.set_device(0)
-    stream = torch.cuda.current_stream(dev)
-    w = W.make_workload(args.full_config)
-    max_nvec = min(w.nvec, 64)
-    ctx = api.context_for(w, max_nvec=max_nvec, stream=stream, device="cuda:0")
-    psi = torch.empty((w.nvec,) + w.grid.shape, dtype=torch.complex128, device=dev)
-    for v0 in range(0, w.nvec, max_nvec):
-        ctx.sgw_random_vectors(W.SEED_VEC, v0, min(max_nvec, w.nvec - v0), psi[v0:])
-    warm = psi[:1].clone()                                   # lazy workspace allocation and first-launch costs
-    ctx.sgw_cheb_filter(warm, w.coeffs[:3], w.emin, w.emax)
-    del warm
-    sampler = ClockSampler(0)
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize(dev)
-    e0.record(stream)
-    ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
-    e1.record(stream)
-    torch.cuda.synchronize(dev)
-    ms_f = e0.elapsed_time(e1)
-    out = {"config": args.full_config, "grid": list(w.grid.shape), "atoms": w.atoms, "nvec": w.nvec, "nterms": w.nterms,
-           "kb_spheres": int(w.kb.nsphere), "filter_s": ms_f * 1e-3,
-           "filter_units_per_s": w.grid.ng * w.nvec * (w.nterms - 1) / (ms_f * 1e-3),
-           "filter_output_finite": all(bool(torch.isfinite(torch.view_as_real(psi[v])).all()) for v in range(w.nvec))}
-    if args.repeat > 0:
-        # the same call again on the restored vectors: launch-bound grids capture a CUDA graph on the first repeat
-        # and replay it afterwards (DESIGN.md section 6)
-        psi0 = torch.empty_like(psi)
-        for v0 in range(0, w.nvec, max_nvec):
-            ctx.sgw_random_vectors(W.SEED_VEC, v0, min(max_nvec, w.nvec - v0), psi0[v0:])
-        rep = []
-        for _ in range(args.repeat):
-            psi.copy_(psi0)
-            torch.cuda.synchronize(dev)
-            e0.record(stream)
-            ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
-            e1.record(stream)
-            torch.cuda.synchronize(dev)
-            rep.append(e0.elapsed_time(e1) * 1e-3)
-        out["filter_repeat_s"] = rep
-        out["filter_repeat_units_per_s"] = w.grid.ng * w.nvec * (w.nterms - 1) / min(rep)
-        del psi0
-    if w.td_steps:
-        n0 = ctx.sgw_norms(psi)
-        ctx.sgw_set_td(1, w.rho_scale)
-        e0.record(stream)
-        ctx.sgw_td_propagate(psi, w.dt, w.td_steps)
-        e1.record(stream)
-        torch.cuda.synchronize(dev)
-        ms_t = e0.elapsed_time(e1)
-        out.update({"td_steps": w.td_steps, "td_s": ms_t * 1e-3,
-                    "td_units_per_s": w.grid.ng * w.nvec * w.td_steps / (ms_t * 1e-3),
-                    "td_norm_drift": float((ctx.sgw_norms(psi) / n0 - 1.0).abs().max())})
-    out["clocks"] = sampler.stop()
-    out["gpu_launches"] = ctx.sgw_launch_count()
-    assert ctx.sgw_sync_check() == 0
-    print(json.dumps(out))
+def spawn_ranks(args):
+    """python bench.py --gpus N outside torchrun: start the N ranks ourselves (one process per GPU)."""
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
 
 
 def main():
@@ -468,27 +552,19 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="sgw", choices=["sgw", "reference"])
-    ap.add_argument("--nterms", type=int, default=None,
-                    help="shorten the filter (profiling runs under ncu only; the default is the config's 512)")
-    ap.add_argument("--no-td", action="store_true", help="skip the TD-step sample (cfg2) and the short samples of cfg0/cfg3/cfg4")
-    ap.add_argument("--full-config", default=None, choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"],
-                    help="run one BASELINE.json config at full size and length and print its own JSON report")
-    ap.add_argument("--repeat", type=int, default=0,
-                    help="with --full-config: repeat the filter call this many times on the restored vectors and report each time")
-    ap.add_argument("--td-only", action="store_true",
-                    help="run only the TD-step sample (cfg2) and print its JSON object (profiling runs under ncu)")
-    ap.add_argument("--td-steps", type=int, default=100, help="timed steps of the TD-step sample (default 100 of the 2000)")
+    ap.add_argument("--nvec", type=int, default=None, help="vectors in flight (profiling runs under ncu only; default: the config's 32)")
+    ap.add_argument("--no-others", action="store_true", help="skip the other configs (cfg0-cfg3)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs under ncu only)")
+    ap.add_argument("--td-steps", type=int, default=100, help="timed steps of the cfg2 TD entry (default 100 of the 2000)")
+    ap.add_argument("--write-traffic", default=None, metavar="NCU_RAW_CSV",
+                    help="post-process an ncu raw page into profiles/r02_traffic.json and exit (no GPU needed)")
+    ap.add_argument("--traffic-source", default="profiles/r02_cfg4_ncu.md")
     args = ap.parse_args()
-    if args.td_only:
-        import torch
-        from paper_2601_21005_b200 import api
-        dev = torch.device("cuda:0")
-        torch.cuda.set_device(dev)
-        print(json.dumps(run_td(torch, api, dev, torch.cuda.current_stream(dev), args)))
+    if args.write_traffic:
+        write_traffic(args.write_traffic, args.traffic_source)
         return
-    if args.full_config:
-        run_full_config(args)
-        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -14,19 +14,28 @@
  *  - Complex vectors are interleaved (re,im) IEEE double, 16 B per element, layout
  *    [nvec][nz][ny][nx] with x fastest; flat grid index g = ix + nx*(iy + ny*iz) (packed
  *    (N_g x n) multi-index arrays).  Real fields (V_loc, rho, V_H) are [nz][ny][nx] doubles.
- *  - All work is enqueued on the CUDA stream given to sgw_init_grid and is asynchronous with
- *    respect to the host; the library synchronises only inside sgw_init_grid / sgw_set_* /
- *    sgw_destroy (setup) and on error paths.  k-space data never crosses the boundary.
+ *  - All work is enqueued on the CUDA stream given to sgw_init_grid and is asynchronous with respect to the
+ *    host.  The calls that block the host are: sgw_init_grid, sgw_set_vloc, sgw_set_nonlocal, sgw_destroy (setup;
+ *    they allocate and synchronise the stream), sgw_sync_check, sgw_profile_get / _reset / _enable(0),
+ *    sgw_spectral_bounds and sgw_probe_fp64 (they return host values), the FIRST sgw_cheb_filter / sgw_spectral_bounds call on a context
+ *    (it allocates the two workspace arrays of max_nvec vectors: cudaMalloc), and error paths.  sgw_random_vectors,
+ *    sgw_apply_H, sgw_hartree, sgw_td_propagate, sgw_norms and every later sgw_cheb_filter only enqueue work.
+ *    k-space data never crosses the boundary.
  *  - Supported axis lengths: 8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256, 384 (products of 2 and
  *    3 with a compiled two-stage factorisation); nx must be a multiple of 4.  Others: SGW_ESIZE.
  *  - The library owns only its context (tables, workspace for max_nvec vectors).  Calls with
  *    nvec > max_nvec are processed in sub-batches of max_nvec (vectors are independent in the
  *    filter; in the TD step the density is accumulated over all sub-batches first).
- *  - Three implementations of the fused passes are built in and selected by the environment variable
- *    SGW_ENGINE when the context is created: 2 (default) lean streaming passes (autonomous warp groups,
- *    register operands, a plane kernel for x+y); 0 staged kernels (cp.async-pipelined operands in shared
- *    memory); 1 pass engine (one persistent kernel executing a program of passes with dependency counters).
- *    All compute the same results.
+ *  - Run-time switches, all read ONCE in sgw_init_grid (defaults are the measured best):
+ *      SGW_LEAN_B=4|8        pencils per tile of the fused passes (default 8 when nx and ny are multiples of 8)
+ *      SGW_LEAN_G=n          plane kernel: planes per CTA-owned group (default 1)
+ *      SGW_LEAN_CTAS=1|2     plane kernel: one 16-warp or two 8-warp CTAs per SM (default: by L2 footprint)
+ *      SGW_LEAN_CLUSTER=0|1  plane kernel: cluster-owned planes off / on (default: on for real 128^2, 256^2 planes)
+ *      SGW_LEAN_CHUNK=n      filter: n vectors at a time through all terms (default: all vectors per term)
+ *      SGW_L2_CHUNK=n        propagation: n vectors at a time through a step (default: all vectors)
+ *      SGW_PDL=1             programmatic dependent launch of the passes (default off)
+ *      SGW_GRAPH=0           never replay a repeated small filter call as a CUDA graph (default on)
+ *      SGW_GRAPH_BYTES=b     largest vector block that takes the graph path (default 16e6)
  *  - There is no CPU fallback: without a CUDA device sgw_init_grid fails with SGW_ECUDA.
  */
 #ifndef SGW_H
@@ -48,8 +57,9 @@ typedef struct sgw_ctx sgw_ctx;
 
 /* Create a context for an nx*ny*nz periodic grid with spacings hx,hy,hz (bohr) (N_g =
  * N_x N_y N_z).  k_i = 2 pi m/(N_i h_i), m in [-N_i/2, N_i/2) (R: SURVEY 8(a) a3).  max_nvec
- * sizes the internal workspace (2 or 3 complex arrays of max_nvec*N_g, allocated lazily by the first
- * call that needs them).  cuda_stream is a cudaStream_t owned by the caller (NULL = default
+ * sizes the internal workspace (2 complex arrays of max_nvec*N_g, allocated by the first sgw_cheb_filter /
+ * sgw_spectral_bounds call) and the projection buffer of the nonlocal term.  The device current at this call is
+ * the context's device.  cuda_stream is a cudaStream_t owned by the caller (NULL = default
  * stream).  *ctx is written on success only. */
 int sgw_init_grid(sgw_ctx** ctx, int nx, int ny, int nz, double hx, double hy, double hz,
                   int max_nvec, void* cuda_stream);
@@ -129,16 +139,22 @@ int64_t sgw_launch_count(const sgw_ctx* ctx);
 /* Per-pass device timing for measurement (bench.py's roofline): while enabled, every FFT pass launch
  * is bracketed by a pair of CUDA events on the context's stream (at most 60000 launches between
  * collections).  sgw_profile_get synchronises the stream and returns, for passes along `axis`
- * (0 x, 1 y, 2 z) of `kind` (0 store, 1 accumulate, 2 H-final, 3 Chebyshev, 4 TD, 5 Poisson kernel,
- * 6 forward, 7 inverse), the number of launches timed and their summed duration in ms since the
- * last sgw_profile_reset. */
+ * (0 x, 1 y, 2 z) of `kind` (0 x pass of an operator application, 1 y pass or fused x+y plane pass, 2 z pass of
+ * H apply, 3 z pass of a Chebyshev term, 4 split-operator passes, 5 / 6 / 7 Poisson z round trip / forward /
+ * inverse passes), the number of launches timed and their summed duration in ms since the last
+ * sgw_profile_reset.  Booked under axis 0 as well: kind 8 / 9 the gather-dot / scatter kernels of the nonlocal term,
+ * kind 10 the density kernel. */
 int sgw_profile_enable(sgw_ctx* ctx, int on);
 int sgw_profile_reset(sgw_ctx* ctx);
 int sgw_profile_get(sgw_ctx* ctx, int axis, int kind, int64_t* count, double* total_ms);
 
-/* Synchronises the context's stream and reports asynchronous failures: SGW_ECUDA if a kernel faulted or
- * if a dependency wait inside the pass engine gave up (the engine never hangs: a bounded spin sets a
- * flag instead); SGW_OK otherwise.  The only call besides setup that blocks the host. */
+/* Measurement helper ("FP64 peak ... must be probed"): runs a dependent-free DFMA loop (8 independent
+ * chains per thread, 32 warps per SM, 2 CTAs per SM) on the context's stream at whatever clocks the device is at
+ * and writes the best of three timed repetitions, in FP64 flop/s (2 per DFMA), to *h_flops_per_s.  Blocks the host. */
+int sgw_probe_fp64(sgw_ctx* ctx, double* h_flops_per_s);
+
+/* Synchronises the context's stream and reports asynchronous failures: SGW_ECUDA if a kernel faulted,
+ * SGW_OK otherwise. */
 int sgw_sync_check(sgw_ctx* ctx);
 
 /* Message for the last error on the calling thread ("" if none). */

@@ -19,7 +19,8 @@ _lib = None
 ERRORS = {-1: "SGW_EINVAL", -2: "SGW_ESIZE", -3: "SGW_ENOMEM", -4: "SGW_ECUDA"}
 EXPORTS = ["sgw_init_grid", "sgw_destroy", "sgw_set_vloc", "sgw_set_nonlocal", "sgw_random_vectors",
            "sgw_apply_H", "sgw_cheb_filter", "sgw_hartree", "sgw_set_td", "sgw_td_propagate", "sgw_norms",
-           "sgw_launch_count", "sgw_last_error", "sgw_sync_check", "sgw_spectral_bounds", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get"]
+           "sgw_launch_count", "sgw_last_error", "sgw_sync_check", "sgw_spectral_bounds", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get",
+           "sgw_probe_fp64"]
 
 
 class SGWError(RuntimeError):
@@ -55,6 +56,7 @@ def load():
         lib.sgw_profile_enable.argtypes = [vp, i]
         lib.sgw_profile_reset.argtypes = [vp]
         lib.sgw_profile_get.argtypes = [vp, i, i, C.POINTER(i64), C.POINTER(d)]
+        lib.sgw_probe_fp64.argtypes = [vp, C.POINTER(d)]
         _lib = lib
     return _lib
 
@@ -174,6 +176,11 @@ class Context:
         n, ms = C.c_int64(), C.c_double()
         _check(self.lib.sgw_profile_get(self._h, axis, kind, C.byref(n), C.byref(ms)))
         return n.value, ms.value
+
+    def sgw_probe_fp64(self):
+        r = C.c_double()
+        _check(self.lib.sgw_probe_fp64(self._h, C.byref(r)))
+        return r.value
 
     def sgw_spectral_bounds(self, niter, seed):
         emin, emax = C.c_double(), C.c_double()

@@ -8,8 +8,6 @@
 
 #define SGW_DECL(N)                                             \
     extern "C" int sgw_pass_launch_##N(const sgw::PassCall*);   \
-    extern "C" int sgw_plane_launch_##N(const sgw::PlaneCall*); \
-    extern "C" int sgw_eng_launch_##N(const sgw::EngCall*, int); \
     extern "C" int sgw_lean_launch_##N(const sgw::LeanCall*, int);
 SGW_DECL(8) SGW_DECL(12) SGW_DECL(16) SGW_DECL(24) SGW_DECL(32) SGW_DECL(48) SGW_DECL(64) SGW_DECL(96)
 SGW_DECL(128) SGW_DECL(192) SGW_DECL(256) SGW_DECL(384)
@@ -29,41 +27,19 @@ int check_cuda(cudaError_t e, const char* what) {
                      std::string(what) + ": " + cudaGetErrorString(e));
 }
 
+#define SGW_SIZES(X) X(8) X(12) X(16) X(24) X(32) X(48) X(64) X(96) X(128) X(192) X(256) X(384)
 static pass_launch_fn launcher_for(int n) {
     switch (n) {
 #define SGW_CASE(N) case N: return sgw_pass_launch_##N;
-        SGW_CASE(8) SGW_CASE(12) SGW_CASE(16) SGW_CASE(24) SGW_CASE(32) SGW_CASE(48) SGW_CASE(64) SGW_CASE(96)
-        SGW_CASE(128) SGW_CASE(192) SGW_CASE(256) SGW_CASE(384)
+        SGW_SIZES(SGW_CASE)
 #undef SGW_CASE
         default: return nullptr;
     }
 }
-
-static plane_launch_fn plane_launcher_for(int n) {
-    switch (n) {
-#define SGW_CASE(N) case N: return sgw_plane_launch_##N;
-        SGW_CASE(8) SGW_CASE(12) SGW_CASE(16) SGW_CASE(24) SGW_CASE(32) SGW_CASE(48) SGW_CASE(64) SGW_CASE(96)
-        SGW_CASE(128) SGW_CASE(192) SGW_CASE(256) SGW_CASE(384)
-#undef SGW_CASE
-        default: return nullptr;
-    }
-}
-
-static eng_launch_fn eng_launcher_for(int n) {
-    switch (n) {
-#define SGW_CASE(N) case N: return sgw_eng_launch_##N;
-        SGW_CASE(8) SGW_CASE(12) SGW_CASE(16) SGW_CASE(24) SGW_CASE(32) SGW_CASE(48) SGW_CASE(64) SGW_CASE(96)
-        SGW_CASE(128) SGW_CASE(192) SGW_CASE(256) SGW_CASE(384)
-#undef SGW_CASE
-        default: return nullptr;
-    }
-}
-
 static lean_launch_fn lean_launcher_for(int n) {
     switch (n) {
 #define SGW_CASE(N) case N: return sgw_lean_launch_##N;
-        SGW_CASE(8) SGW_CASE(12) SGW_CASE(16) SGW_CASE(24) SGW_CASE(32) SGW_CASE(48) SGW_CASE(64) SGW_CASE(96)
-        SGW_CASE(128) SGW_CASE(192) SGW_CASE(256) SGW_CASE(384)
+        SGW_SIZES(SGW_CASE)
 #undef SGW_CASE
         default: return nullptr;
     }
@@ -87,42 +63,6 @@ void prof_end(sgw_ctx* c, cudaEvent_t e1) {
     c->prof_used++;
 }
 
-int run_plane(sgw_ctx* c, int mode, int nvec, const cd* in, cd* out, const cd* phase, bool cheb_tables) {
-    if (!c->plane || nvec <= 0) return 1;
-    PlaneCall call;
-    call.mode = mode;
-    call.a.in = in; call.a.out = out; call.a.phase = phase;
-    call.a.kre_x = cheb_tables ? c->cheb_kin[0] : c->kin[0];
-    call.a.kre_y = cheb_tables ? c->cheb_kin[1] : c->kin[1];
-    call.a.kc_x = c->td_kin[0]; call.a.kc_y = c->td_kin[1];
-    call.a.nplanes = (unsigned)((long long)c->nz * nvec);
-    call.a.nz = (unsigned)c->nz;
-    call.a.G = c->plane_G;
-    call.tw = c->tw[0];
-    call.ctas_per_sm = c->plane_ctas;
-    call.stream = c->stream;
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (c->prof_on && c->prof_used < 60000) {
-        if (c->prof_ev.size() < 2 * (c->prof_used + 1)) {
-            cudaEvent_t a, b;
-            if (cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) {
-                c->prof_ev.push_back(a); c->prof_ev.push_back(b); c->prof_tag.push_back(0);
-            }
-        }
-        if (c->prof_ev.size() >= 2 * (c->prof_used + 1)) {
-            e0 = c->prof_ev[2 * c->prof_used]; e1 = c->prof_ev[2 * c->prof_used + 1];
-            c->prof_tag[c->prof_used] = 1 * K_NKINDS + (mode == PL_TD ? K_RT_TD : K_RT_ACC);   // booked as the y pass
-            cudaEventRecord(e0, c->stream);
-        }
-    }
-    const int rc = c->plane(&call);
-    if (rc == 1) return 1;
-    if (rc != 0) return set_error(rc, std::string("plane launch failed: ") + cudaGetErrorString(cudaGetLastError()));
-    if (e1) { cudaEventRecord(e1, c->stream); c->prof_used++; }
-    c->launches++;
-    return 0;
-}
-
 PassGeom geom_for_axis(const sgw_ctx* c, int axis, int nvec, long long* ntiles) {
     PassGeom g;
     g.ng = c->ng;
@@ -143,33 +83,21 @@ PassGeom geom_for_axis(const sgw_ctx* c, int axis, int nvec, long long* ntiles) 
     return g;
 }
 
-int run_pass(sgw_ctx* c, int axis, int kind, int nvec, const cd* in, const OpParams& p) {
+int run_pass(sgw_ctx* c, int axis, int kind, int variant, const cd* in, const OpParams& p) {
     PassCall call;
     call.kind = kind;
-    call.gm = geom_for_axis(c, axis, nvec, &call.ntiles);
+    call.variant = variant;
+    call.gm = geom_for_axis(c, axis, 1, &call.ntiles);
     call.in = in;
     call.tw = c->tw[axis];
     call.p = p;
     call.stream = c->stream;
     if (call.ntiles <= 0) return 0;
     if (call.ntiles > 0x7fffffffLL) return set_error(SGW_EINVAL, "too many tiles for one launch");
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (c->prof_on && c->prof_used < 60000) {
-        if (c->prof_ev.size() < 2 * (c->prof_used + 1)) {
-            cudaEvent_t a, b;
-            if (cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) {
-                c->prof_ev.push_back(a); c->prof_ev.push_back(b); c->prof_tag.push_back(0);
-            }
-        }
-        if (c->prof_ev.size() >= 2 * (c->prof_used + 1)) {
-            e0 = c->prof_ev[2 * c->prof_used]; e1 = c->prof_ev[2 * c->prof_used + 1];
-            c->prof_tag[c->prof_used] = axis * K_NKINDS + kind;
-            cudaEventRecord(e0, c->stream);
-        }
-    }
+    cudaEvent_t e1 = prof_begin(c, axis * K_NKINDS + kind);
     int rc = c->pass[axis](&call);
-    if (rc != 0) return set_error(rc, std::string("pass launch failed: ") + cudaGetErrorString(cudaGetLastError()));
-    if (e1) { cudaEventRecord(e1, c->stream); c->prof_used++; }
+    if (rc != 0) return set_error(SGW_ECUDA, std::string("pass launch failed: ") + cudaGetErrorString(cudaGetLastError()));
+    prof_end(c, e1);
     c->launches++;
     return 0;
 }
@@ -248,7 +176,7 @@ extern "C" int sgw_sync_check(sgw_ctx* c) {
     if (!c) return set_error(SGW_EINVAL, "sgw_sync_check: null context");
     int rc = check_cuda(cudaStreamSynchronize(c->stream), "sgw_sync_check");
     if (rc) return rc;
-    return sgw::eng_check_error(c);
+    return check_cuda(cudaGetLastError(), "sgw_sync_check");
 }
 
 void sgw::drop_filter_graph(sgw_ctx* c) {
@@ -263,13 +191,19 @@ extern "C" int sgw_destroy(sgw_ctx* c) {
     if (c->gstream) cudaStreamDestroy(c->gstream);
     for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
     for (int a = 0; a < 3; ++a) {
-        cudaFree(c->tw[a]); cudaFree(c->kin[a]); cudaFree(c->cheb_kin[a]); cudaFree(c->td_kin[a]); cudaFree(c->ws[a]);
+        cudaFree(c->tw[a]); cudaFree(c->kin[a]); cudaFree(c->kin_raw[a]); cudaFree(c->cheb_kin[a]); cudaFree(c->td_kin[a]);
     }
+    cudaFree(c->ws[0]); cudaFree(c->ws[1]);
     cudaFree(c->vloc); cudaFree(c->vtab); cudaFree(c->vk3d); cudaFree(c->sph_ptr); cudaFree(c->sph_idx);
     cudaFree(c->beta); cudaFree(c->D); cudaFree(c->kbc); cudaFree(c->pois); cudaFree(c->rho); cudaFree(c->vh);
-    cudaFree(c->phase); cudaFree(c->phase_last); cudaFree(c->vprev); cudaFree(c->d_segs); cudaFree(c->d_cnt); cudaFree(c->d_err);
+    cudaFree(c->phase); cudaFree(c->phase_last); cudaFree(c->vprev); cudaFree(c->red);
     delete c;
     return SGW_OK;
+}
+
+static int env_int(const char* name, int dflt) {
+    const char* e = getenv(name);
+    return e ? atoi(e) : dflt;
 }
 
 extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, double hy, double hz, int max_nvec,
@@ -284,73 +218,61 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
         return set_error(SGW_ECUDA, "sgw_init_grid: no CUDA device (there is no CPU fallback)");
-    sgw_ctx* c = new sgw_ctx();
-    memset((void*)&c->tw, 0, sizeof(c->tw));
+    sgw_ctx* c = new sgw_ctx();      // value-initialised: every pointer NULL, every counter 0
     c->nx = nx; c->ny = ny; c->nz = nz; c->hx = hx; c->hy = hy; c->hz = hz;
     c->ng = (long long)nx * ny * nz;
     c->max_nvec = max_nvec;
     c->stream = (cudaStream_t)cuda_stream;
+    int rc = check_cuda(cudaGetDevice(&c->device), "cudaGetDevice");
+    if (!rc) rc = check_cuda(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device), "SM count");
     c->B = (nx % 8 == 0) ? 8 : 4;
     c->Bx = ((long long)ny * nz) % 8 == 0 ? 8 : (((long long)ny * nz) % 4 == 0 ? 4 : 1);
+    c->leanB = (nx % 8 == 0 && ny % 8 == 0) ? 8 : 4;
+    // run-time switches (all read here, once per context; listed in include/sgw.h)
+    c->lean_G = env_int("SGW_LEAN_G", 0);
+    c->lean_ctas = env_int("SGW_LEAN_CTAS", 0);
+    c->lean_cluster = env_int("SGW_LEAN_CLUSTER", -1);
+    c->lean_chunk = env_int("SGW_LEAN_CHUNK", 0);
+    c->l2_chunk = env_int("SGW_L2_CHUNK", 0);
+    c->pdl = env_int("SGW_PDL", 0) == 1;
+    c->graph_on = env_int("SGW_GRAPH", 1) != 0;
+    c->graph_bytes = 16.0e6;
+    { const char* b = getenv("SGW_GRAPH_BYTES"); if (b && atof(b) > 0) c->graph_bytes = atof(b); }
+    { const int b = env_int("SGW_LEAN_B", 0); if (b == 4 || (b == 8 && c->leanB == 8)) c->leanB = b; }
     const double hh[3] = {hx, hy, hz};
-    int rc = 0;
     for (int a = 0; a < 3 && !rc; ++a) {
         c->dims[a] = dims[a]; c->hs[a] = hh[a];
         c->pass[a] = launcher_for(dims[a]);
-        c->kin[a] = nullptr; c->cheb_kin[a] = nullptr; c->td_kin[a] = nullptr; c->ws[a] = nullptr; c->tw[a] = nullptr;
+        c->lean[a] = lean_launcher_for(dims[a]);
         const int N = dims[a];
         std::vector<cd> tw(N);
-        std::vector<double> kin(N);
-        c->h_kin[a].resize(N);
+        std::vector<double> kin(N), raw(N);
         for (int j = 0; j < N; ++j) {
             const long double ang = -2.0L * acosl(-1.0L) * (long double)j / (long double)N;
             tw[j] = make_double2((double)cosl(ang), (double)sinl(ang));
             const int m = (2 * j >= N) ? j - N : j;
             const long double k = 2.0L * acosl(-1.0L) * (long double)m / ((long double)N * (long double)hh[a]);
-            c->h_kin[a][j] = (double)(0.5L * k * k);
+            raw[j] = (double)(0.5L * k * k);
             kin[j] = (double)(0.5L * k * k / (long double)N);
         }
         if (!rc) rc = dev_alloc(&c->tw[a], N);
         if (!rc) rc = dev_alloc(&c->kin[a], N);
+        if (!rc) rc = dev_alloc(&c->kin_raw[a], N);
         if (!rc) rc = dev_alloc(&c->cheb_kin[a], N);
         if (!rc) rc = dev_alloc(&c->td_kin[a], N);
         if (!rc) rc = upload(c->tw[a], tw.data(), N, c->stream);
         if (!rc) rc = upload(c->kin[a], kin.data(), N, c->stream);
+        if (!rc) rc = upload(c->kin_raw[a], raw.data(), N, c->stream);
     }
-    c->td_kin_valid = false; c->td_dt = 0;
-    c->vloc = nullptr; c->vtab = nullptr; c->vk3d = nullptr;
-    c->nsphere = 0; c->nproj = 0; c->sph_ptr = nullptr; c->sph_idx = nullptr; c->beta = nullptr; c->D = nullptr;
-    c->kbc = nullptr; c->kbc_cap = 0;
-    c->pois = nullptr; c->rho = nullptr; c->vh = nullptr; c->phase = nullptr; c->phase_last = nullptr; c->vprev = nullptr;
-    c->hartree_mode = 0; c->rho_scale = 0; c->launches = 0;
-    c->prof_on = false; c->prof_used = 0;
-    { const char* e = getenv("SGW_L2_CHUNK"); c->l2_chunk = e ? atoi(e) : 0; }
-    c->plane = nullptr; c->plane_G = 2; c->plane_ctas = 0;
-    if (nx == ny && nx % 8 == 0 && !(getenv("SGW_NOPLANE") && atoi(getenv("SGW_NOPLANE")))) c->plane = plane_launcher_for(nx);
-    { const char* e = getenv("SGW_PLANE_G"); if (e && atoi(e) > 0) c->plane_G = atoi(e); }
-    { const char* e = getenv("SGW_PLANE_CTAS"); if (e) c->plane_ctas = atoi(e); }
-    for (int a = 0; a < 3; ++a) c->lean[a] = lean_launcher_for(dims[a]);
-    c->lean_G = 0; c->lean_ctas = 0;
-    { const char* e = getenv("SGW_LEAN_G"); if (e) c->lean_G = atoi(e); }
-    { const char* e = getenv("SGW_LEAN_CTAS"); if (e) c->lean_ctas = atoi(e); }
-    for (int a = 0; a < 3; ++a) { c->eng[a] = eng_launcher_for(dims[a]); c->engB[a] = (nx % 8 == 0 && ny % 8 == 0) ? 8 : 4; }
-    c->use_engine = 2; c->eng_max_ctas = 0; c->eng_resident = -1; c->eng_pc = 0;
-    c->d_segs = nullptr; c->segs_cap = 0; c->d_cnt = nullptr; c->cnt_cap = 0; c->d_err = nullptr;
-    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, 0);
-    { const char* e = getenv("SGW_ENGINE"); if (e) c->use_engine = atoi(e); }
-    { const char* e = getenv("SGW_ENG_CTAS"); if (e) c->eng_max_ctas = atoi(e); }
-    { const char* e = getenv("SGW_ENG_RESIDENT"); if (e) c->eng_resident = atoi(e); }
-    { const char* e = getenv("SGW_ENG_PC"); if (e) c->eng_pc = atoi(e); }
-    c->eng_l2_prefetch = 0;
-    { const char* e = getenv("SGW_ENG_L2PF"); if (e) c->eng_l2_prefetch = atoi(e); }
-    { const char* e = getenv("SGW_ENG_B"); if (e && (atoi(e) == 4 || (atoi(e) == 8 && c->engB[0] == 8))) for (int a = 0; a < 3; ++a) c->engB[a] = atoi(e); }
-    for (int i = 0; i < 3 * K_NKINDS; ++i) { c->prof_ms[i] = 0; c->prof_n[i] = 0; }
     if (!rc) rc = dev_alloc(&c->vtab, c->ng);
     if (!rc) rc = dev_alloc(&c->vk3d, c->ng);
     if (!rc) rc = dev_alloc(&c->pois, c->ng);
     if (!rc) rc = dev_alloc(&c->rho, c->ng);
     if (!rc) rc = dev_alloc(&c->vh, c->ng);
     if (!rc) rc = dev_alloc(&c->phase, c->ng);
+    if (!rc) rc = dev_alloc(&c->phase_last, c->ng);
+    if (!rc) rc = dev_alloc(&c->vprev, c->ng);
+    if (!rc) rc = dev_alloc(&c->red, 4);
     if (!rc) {
         const double Lx = nx * hx, Ly = ny * hy, Lz = nz * hz;
         const double Rc = 0.5 * fmin(Lx, fmin(Ly, Lz));
@@ -380,23 +302,29 @@ extern "C" int sgw_set_nonlocal(sgw_ctx* c, int nsphere, const int64_t* d_ptr, c
     if (!c || nsphere < 0) return set_error(SGW_EINVAL, "sgw_set_nonlocal: bad argument");
     cudaStreamSynchronize(c->stream);
     sgw::drop_filter_graph(c);
-    cudaFree(c->sph_ptr); cudaFree(c->sph_idx); cudaFree(c->beta); cudaFree(c->D);
-    c->sph_ptr = nullptr; c->sph_idx = nullptr; c->beta = nullptr; c->D = nullptr; c->nsphere = 0;
+    cudaFree(c->sph_ptr); cudaFree(c->sph_idx); cudaFree(c->beta); cudaFree(c->D); cudaFree(c->kbc);
+    c->sph_ptr = nullptr; c->sph_idx = nullptr; c->beta = nullptr; c->D = nullptr; c->kbc = nullptr; c->nsphere = 0;
     if (nsphere == 0) return SGW_OK;
     if (!d_ptr || !d_idx || !d_beta || !d_D || nproj < 1 || nproj > 8)
         return set_error(SGW_EINVAL, "sgw_set_nonlocal: bad argument");
+    // every copy is ordered on the context's stream (the caller's arrays may have been produced on it, and a
+    // non-blocking stream is not ordered against the legacy default stream), then one synchronisation
+    cudaStream_t st = c->stream;
     int64_t npts = 0;
-    int rc = check_cuda(cudaMemcpy(&npts, d_ptr + nsphere, sizeof(int64_t), cudaMemcpyDeviceToHost), "read sph_ptr");
+    int rc = check_cuda(cudaMemcpyAsync(&npts, d_ptr + nsphere, sizeof(int64_t), cudaMemcpyDeviceToHost, st), "read sph_ptr");
+    if (!rc) rc = check_cuda(cudaStreamSynchronize(st), "read sph_ptr");
     if (rc) return rc;
     if (npts < 0) return set_error(SGW_EINVAL, "sgw_set_nonlocal: negative point count");
     if (!rc) rc = dev_alloc(&c->sph_ptr, (size_t)nsphere + 1);
     if (!rc) rc = dev_alloc(&c->sph_idx, (size_t)npts);
     if (!rc) rc = dev_alloc(&c->beta, (size_t)npts * nproj);
     if (!rc) rc = dev_alloc(&c->D, (size_t)nsphere * nproj);
-    if (!rc) rc = check_cuda(cudaMemcpy(c->sph_ptr, d_ptr, (nsphere + 1) * sizeof(int64_t), cudaMemcpyDeviceToDevice), "copy");
-    if (!rc && npts) rc = check_cuda(cudaMemcpy(c->sph_idx, d_idx, npts * sizeof(int32_t), cudaMemcpyDeviceToDevice), "copy");
-    if (!rc && npts) rc = check_cuda(cudaMemcpy(c->beta, d_beta, npts * nproj * sizeof(double), cudaMemcpyDeviceToDevice), "copy");
-    if (!rc) rc = check_cuda(cudaMemcpy(c->D, d_D, (size_t)nsphere * nproj * sizeof(double), cudaMemcpyDeviceToDevice), "copy");
+    if (!rc) rc = dev_alloc(&c->kbc, (size_t)c->max_nvec * nsphere * nproj);      // no allocation inside the hot calls
+    if (!rc) rc = check_cuda(cudaMemcpyAsync(c->sph_ptr, d_ptr, (nsphere + 1) * sizeof(int64_t), cudaMemcpyDeviceToDevice, st), "copy");
+    if (!rc && npts) rc = check_cuda(cudaMemcpyAsync(c->sph_idx, d_idx, npts * sizeof(int32_t), cudaMemcpyDeviceToDevice, st), "copy");
+    if (!rc && npts) rc = check_cuda(cudaMemcpyAsync(c->beta, d_beta, npts * nproj * sizeof(double), cudaMemcpyDeviceToDevice, st), "copy");
+    if (!rc) rc = check_cuda(cudaMemcpyAsync(c->D, d_D, (size_t)nsphere * nproj * sizeof(double), cudaMemcpyDeviceToDevice, st), "copy");
+    if (!rc) rc = check_cuda(cudaStreamSynchronize(st), "sgw_set_nonlocal");
     if (rc) return rc;
     c->nsphere = nsphere; c->nproj = nproj;
     return SGW_OK;

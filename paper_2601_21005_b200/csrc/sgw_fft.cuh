@@ -143,10 +143,10 @@ struct PassGeom {
 
 enum { MODE_RT = 0, MODE_FWD = 1, MODE_INV = 2 };
 
-// One CTA = B pencils of length N.  Op supplies:
-//   cd   pro(cd v, long long off, long long g)              value transform on load
+// One CTA = B pencils of length N.  Op supplies (sgw_ops.cuh):
+//   cd   load(const cd* in, long long off)                  input element
 //   cd   mult(cd X, int k, long long gk)                    k-space multiply (RT only)
-//   void epi(cd r, cd vin, long long off, long long g)      store; vin = prologue'd input (RT only)
+//   void epi(cd r, long long off, long long g)              store
 template <int N, int MODE, class Op>
 __global__ void __launch_bounds__(256) pass_kernel(PassGeom gm, const cd* __restrict__ in,
                                                     const cd* __restrict__ twN, Op op) {
@@ -166,14 +166,12 @@ __global__ void __launch_bounds__(256) pass_kernel(PassGeom gm, const cd* __rest
     const bool actA = tid < B * R2, actB = tid < B * R1;
 
     cd x[R1];
-    cd xin[R1];
     if (MODE != MODE_INV) {
         if (actA) {
 #pragma unroll
             for (int n1 = 0; n1 < R1; ++n1) {
                 const long long o = (long long)(n1 * R2 + n2) * gm.sN + (long long)bA * gm.sB;
-                x[n1] = op.pro(in[base + o], base + o, g0 + o);
-                if (MODE == MODE_RT) xin[n1] = x[n1];
+                x[n1] = op.load(in, base + o);
             }
             Dft<R1, -1>::run(x);
 #pragma unroll
@@ -195,7 +193,7 @@ __global__ void __launch_bounds__(256) pass_kernel(PassGeom gm, const cd* __rest
 #pragma unroll
             for (int k2 = 0; k2 < R2; ++k2) {
                 const long long o = (long long)(k1 + R1 * k2) * gm.sN + (long long)bB * gm.sB;
-                op.epi(y[k2], y[k2], base + o, g0 + o);
+                op.epi(y[k2], base + o, g0 + o);
             }
         } else {
             if (MODE == MODE_RT) {
@@ -208,7 +206,7 @@ __global__ void __launch_bounds__(256) pass_kernel(PassGeom gm, const cd* __rest
 #pragma unroll
                 for (int k2 = 0; k2 < R2; ++k2) {
                     const long long o = (long long)(k1 + R1 * k2) * gm.sN + (long long)bB * gm.sB;
-                    y[k2] = op.pro(in[base + o], base + o, g0 + o);
+                    y[k2] = op.load(in, base + o);
                 }
             }
             Dft<R2, +1>::run(y);
@@ -228,7 +226,7 @@ __global__ void __launch_bounds__(256) pass_kernel(PassGeom gm, const cd* __rest
 #pragma unroll
             for (int n1 = 0; n1 < R1; ++n1) {
                 const long long o = (long long)(n1 * R2 + n2) * gm.sN + (long long)bA * gm.sB;
-                op.epi(x[n1], MODE == MODE_RT ? xin[n1] : x[n1], base + o, g0 + o);
+                op.epi(x[n1], base + o, g0 + o);
             }
         }
     }

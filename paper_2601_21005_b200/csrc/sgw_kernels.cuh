@@ -44,15 +44,6 @@ static __global__ void density_kernel(const cd* __restrict__ psi, int nvec, long
     if (rho2) rho2[i] = s;
 }
 
-static __global__ void real_to_complex_kernel(const double* __restrict__ r, cd* __restrict__ c, long long n) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) c[i] = make_double2(r[i], 0.0);
-}
-static __global__ void complex_to_real_kernel(const cd* __restrict__ c, double* __restrict__ r, long long n) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) r[i] = c[i].x;
-}
-
 // phase[g] = exp(-i (vloc[g] + vh[g]) * half_dt)
 static __global__ void phase_kernel(const double* __restrict__ vloc, const double* __restrict__ vh, double half_dt,
                                     cd* __restrict__ phase, long long n) {
@@ -69,13 +60,13 @@ static __global__ void phase_kernel(const double* __restrict__ vloc, const doubl
 // step n-1 and the opening factor exp(-i V_n dt/2) of step n are applied together on load in step n:
 //   table[g] = exp(-i (V_n + V_{n-1}) half_dt)   (first step of a call: exp(-i V_n half_dt));   vprev <- V_n
 //   last[g]  = exp(-i V_n half_dt)               (only for the last step of a call, applied on store)
-// vh_c: the Hartree potential as the real part of the Poisson solve's complex result (or NULL)
-static __global__ void phase_merge_kernel(const double* __restrict__ vloc, const cd* __restrict__ vh_c, double* __restrict__ vprev,
+// Frozen-potential form (V = V_loc); with the Hartree rebuild the same tables are written by the last pass of the
+// Poisson solve (OpPhaseMerge, sgw_ops.cuh).
+static __global__ void phase_merge_kernel(const double* __restrict__ vloc, double* __restrict__ vprev,
                                           double half_dt, int first, cd* __restrict__ table, cd* __restrict__ last, long long n) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    double v = vloc ? vloc[i] : 0.0;
-    if (vh_c) v += vh_c[i].x;
+    const double v = vloc ? vloc[i] : 0.0;
     double s, c;
     sincos((first ? v : v + vprev[i]) * half_dt, &s, &c);
     table[i] = make_double2(c, -s);
@@ -84,14 +75,6 @@ static __global__ void phase_merge_kernel(const double* __restrict__ vloc, const
         sincos(v * half_dt, &s, &c);
         last[i] = make_double2(c, -s);
     }
-}
-
-// psi[v][g] *= phase[g]
-static __global__ void apply_phase_kernel(cd* __restrict__ psi, const cd* __restrict__ phase, long long ng) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= ng) return;
-    cd* p = psi + (long long)blockIdx.y * ng;
-    p[i] = cmul(p[i], phase[i]);
 }
 
 static __global__ void scale_kernel(cd* __restrict__ psi, double a, long long n) {
@@ -104,6 +87,15 @@ static __global__ void vtab_kernel(const double* __restrict__ vloc, double s, do
                                    long long n) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) vtab[i] = s * ((vloc ? vloc[i] : 0.0) - Eb);
+}
+
+// out[j] = exp(-i kin[j] dt) / n   (split-operator kinetic factor per axis; 1/n = inverse-transform scale)
+static __global__ void td_table_kernel(const double* __restrict__ kin, double dt, cd* __restrict__ out, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double s, c;
+    sincos(kin[i] * dt, &s, &c);
+    out[i] = make_double2(c / n, -s / n);
 }
 
 static __global__ void scale_table_kernel(const double* __restrict__ in, double s, double* __restrict__ out, int n) {

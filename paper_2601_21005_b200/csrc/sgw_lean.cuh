@@ -3,7 +3,7 @@
 // One pass = for every tile of B pencils: acc <- hs * RT_axis(cur) [+ hs * V * cur] + alpha * acc (real k
 // table: H apply, Chebyshev term) or psi <- [phase] RT_axis([phase] psi) (complex k table:
 // split-operator factor).  What the profiles of the earlier kernels showed (profiles/
-// r01_v2_cfg1.md, r01_engine_v3_cfg1.md) shaped this one:
+// r01_lean_cfg1.md) shaped this one:
 //  * a tile belongs to an autonomous warp group (B * R2 threads, two warps for N = 96) with its own slice
 //    of shared memory and its own named barrier; 16 warps per SM in different phases hide each other's
 //    latency, nothing is staged through shared memory, and the only per-item work outside the
@@ -17,9 +17,38 @@
 // planes, does their row tiles, __syncthreads, then their column tiles, so the x->y transpose goes
 // through L2 and HBM sees cur once and acc once for the two passes.
 #pragma once
-#include "sgw_engine.cuh"   // Fact2, F_* flags
+#include "sgw_fft.cuh"
 
 namespace sgw {
+
+// two-stage factorisation N = R1 * R2: stage A (global load/store side) keeps R1 values per thread
+// with R2 threads per pencil; stage B (pure compute) is R1 independent radix-R2 round trips per pencil.
+template <int N> struct Fact2;
+#define SGW_FACT2(N_, R1_, R2_) \
+    template <> struct Fact2<N_> { static constexpr int R1 = R1_, R2 = R2_; };
+SGW_FACT2(8, 2, 4)
+SGW_FACT2(12, 3, 4)
+SGW_FACT2(16, 4, 4)
+SGW_FACT2(24, 6, 4)
+SGW_FACT2(32, 8, 4)
+SGW_FACT2(48, 12, 4)
+SGW_FACT2(64, 8, 8)
+SGW_FACT2(96, 12, 8)
+SGW_FACT2(128, 16, 8)
+SGW_FACT2(192, 12, 16)
+SGW_FACT2(256, 16, 16)
+SGW_FACT2(384, 16, 24)
+#undef SGW_FACT2
+
+// per-pass flags
+enum {
+    F_VTAB = 1,      // add hs * vtab[g] * cur to the result
+    F_FLUSH = 2,     // series <- [series] + c0 * acc_old + c1 * cur        (on load)
+    F_SINIT = 4,     // with F_FLUSH: series is written, not accumulated
+    F_PRO = 8,       // complex family: multiply by phase[g] on load
+    F_EPI = 16,      // complex family: multiply by phase[g] on store
+    F_DENS = 32      // complex family: rho[g] += dens_scale * |result|^2 (atomic)
+};
 
 struct LeanArgs {
     const cd* cur;            // input vectors
@@ -388,6 +417,9 @@ struct LeanCall {
     int ctas_per_sm;          // 0 = as many as fit
     int wpc;                  // plane kernel: warps per CTA, 8 (two CTAs per SM) or 16 (one)
     int cluster;              // plane kernel: 1 = cluster-owned planes (plane_cluster_kernel), 0 = CTA-owned
+    int pdl;                  // 1 = programmatic dependent launch (SGW_PDL=1)
+    int num_sms;              // of the context's device
+    int* occ;                 // context-owned cache of occupancy results for this axis length, 16 ints, zero-initialised
     cudaStream_t stream;
 };
 // returns 0, -(stage*1000 + cudaError) on failure, or 1 if this (N, B) is not instantiated

@@ -1,39 +1,44 @@
-// sgw_ops.cuh -- prologue / k-space / epilogue functors fused into the FFT passes, and the plain
-// struct through which the library core asks a per-length translation unit to launch a pass.
+// sgw_ops.cuh -- functors of the generic pass kernel (sgw_fft.cuh: pass_kernel), which serves the Poisson solve of
+// the Hartree rebuild (R-10), and the plain struct through which the library core asks a per-length translation
+// unit to launch such a pass.  The pass kinds double as the tags of the per-pass profile (sgw_profile_get).
 #pragma once
 #include "sgw_fft.cuh"
 
 namespace sgw {
 
 enum PassKind {
-    K_RT_STORE = 0,    // out = RT(in)                      RT multiplies by a real 1D table
-    K_RT_ACC = 1,      // out = RT(in) + acc
-    K_RT_HFIN = 2,     // out = RT(in) + acc + V*in                        (last pass of H apply)
-    K_RT_CHEB = 3,     // Chebyshev recurrence + series accumulation       (last pass of a term)
-    K_RT_TD = 4,       // out = [phase] RT([phase] in), complex 1D table   (split-operator factor)
-    K_RT_MUL3D = 5,    // out = RT(in) with a real 3D k-space table        (Poisson kernel)
-    K_FWD = 6,         // out = forward transform along the axis, natural k order
-    K_INV = 7,         // out = inverse transform (unnormalised)
-    K_NKINDS = 8
+    K_RT_STORE = 0,    // lean x pass of an operator application (store form)
+    K_RT_ACC = 1,      // lean y pass / x+y plane pass (accumulate form)
+    K_RT_HFIN = 2,     // lean z pass of H apply
+    K_RT_CHEB = 3,     // lean z pass of a Chebyshev term
+    K_RT_TD = 4,       // lean passes of a split-operator step
+    K_RT_MUL3D = 5,    // Poisson: z round trip with the real 3D table v(k)/N_g
+    K_FWD = 6,         // Poisson: forward transform along the axis, natural k order
+    K_INV = 7,         // Poisson: inverse transform (unnormalised)
+    K_KB_PROJECT = 8,  // nonlocal term: gather-dot (booked under axis 0)
+    K_KB_SCATTER = 9,  // nonlocal term: scatter (booked under axis 0)
+    K_DENSITY = 10,    // density_kernel (booked under axis 0)
+    K_NKINDS = 11
 };
 
 struct OpParams {
     cd* out;                 // result
-    const cd* acc;           // added to the result (may alias out)
-    const cd* prev;          // Chebyshev phi_{n-1} (may alias out)
-    cd* series;              // Chebyshev series accumulator
-    const double* vtab;      // real N_g table multiplying the input in the epilogue
-    const double* mul_re;    // real [N] k-space table (includes 1/N)
-    const cd* mul_c;         // complex [N] k-space table (includes 1/N)
+    const double* rin;       // K_FWD from a real field: the input is rin[g] + 0i (in is ignored)
     const double* mul3d;     // real N_g k-space table
-    const cd* pro_phase;     // complex N_g table applied on load (or NULL)
-    const cd* epi_phase;     // complex N_g table applied on store (or NULL)
-    double hs, c0, c1, c2;   // Chebyshev: scale of H term; series coefficients for prev, cur, next
-    int use_prev, flush, series_init;
+    // K_INV with the merged phase epilogue (R-8): V = vloc + Re(result)
+    const double* vloc;
+    double* vprev;           // in: V of the previous step; out: V
+    cd* table;               // exp(-i (V + vprev) half_dt)   (first != 0: exp(-i V half_dt))
+    cd* last;                // exp(-i V half_dt) or NULL
+    double* rho_reset;       // zeroed (the next step accumulates into it) or NULL
+    double* vh_out;          // Re(result) or NULL
+    double half_dt;
+    int first;
 };
 
 struct PassCall {
-    int kind;
+    int kind;                // PassKind
+    int variant;             // K_FWD: 1 = real input (rin);  K_INV: 1 = merged phase epilogue, 2 = real output (vh_out)
     PassGeom gm;
     long long ntiles;
     const cd* in;
@@ -45,56 +50,41 @@ struct PassCall {
 typedef int (*pass_launch_fn)(const PassCall*);
 
 // ---- functors -------------------------------------------------------------------------------
-struct OpBase {
+//   cd   load(const cd* in, long long off)                  input element
+//   cd   mult(cd X, int k, long long gk)                    k-space multiply (RT only)
+//   void epi(cd r, long long off, long long g)              store
+struct OpStore {
     OpParams p;
-    __device__ __forceinline__ cd pro(cd v, long long, long long) const { return v; }
-    __device__ __forceinline__ cd mult(cd X, int k, long long) const { return cscale(X, __ldg(p.mul_re + k)); }
+    __device__ __forceinline__ cd load(const cd* in, long long off) const { return in[off]; }
+    __device__ __forceinline__ cd mult(cd X, int, long long) const { return X; }
+    __device__ __forceinline__ void epi(cd r, long long off, long long) const { p.out[off] = r; }
 };
-struct OpStore : OpBase {
-    __device__ __forceinline__ void epi(cd r, cd, long long off, long long) const { p.out[off] = r; }
+// forward pass straight from the real density (replaces a separate real -> complex copy)
+struct OpFromReal : OpStore {
+    __device__ __forceinline__ cd load(const cd*, long long off) const { return make_double2(p.rin[off], 0.0); }
 };
-struct OpAcc : OpBase {
-    __device__ __forceinline__ void epi(cd r, cd, long long off, long long) const {
-        p.out[off] = cadd(r, p.acc[off]);
-    }
-};
-struct OpHFin : OpBase {
-    __device__ __forceinline__ void epi(cd r, cd vin, long long off, long long g) const {
-        cd a = p.acc[off];
-        const double v = p.vtab ? __ldg(p.vtab + g) : 0.0;
-        p.out[off] = make_double2(r.x + a.x + v * vin.x, r.y + a.y + v * vin.y);
-    }
-};
-struct OpCheb : OpBase {
-    __device__ __forceinline__ void epi(cd r, cd vin, long long off, long long g) const {
-        cd a = p.acc[off];
-        const double v = __ldg(p.vtab + g);
-        cd nx = make_double2(p.hs * (r.x + a.x + v * vin.x), p.hs * (r.y + a.y + v * vin.y));
-        cd pv = make_double2(0.0, 0.0);
-        if (p.use_prev) { pv = p.prev[off]; nx = csub(nx, pv); }
-        p.out[off] = nx;
-        if (p.flush) {
-            cd s = make_double2(p.c0 * pv.x + p.c1 * vin.x + p.c2 * nx.x, p.c0 * pv.y + p.c1 * vin.y + p.c2 * nx.y);
-            if (!p.series_init) s = cadd(s, p.series[off]);
-            p.series[off] = s;
-        }
-    }
-};
-struct OpTD {
-    OpParams p;
-    __device__ __forceinline__ cd pro(cd v, long long, long long g) const {
-        return p.pro_phase ? cmul(v, __ldg(p.pro_phase + g)) : v;
-    }
-    __device__ __forceinline__ cd mult(cd X, int k, long long) const { return cmul(X, __ldg(p.mul_c + k)); }
-    __device__ __forceinline__ void epi(cd r, cd, long long off, long long g) const {
-        p.out[off] = p.epi_phase ? cmul(r, __ldg(p.epi_phase + g)) : r;
-    }
-};
-struct OpMul3D {
-    OpParams p;
-    __device__ __forceinline__ cd pro(cd v, long long, long long) const { return v; }
+struct OpMul3D : OpStore {
     __device__ __forceinline__ cd mult(cd X, int, long long gk) const { return cscale(X, __ldg(p.mul3d + gk)); }
-    __device__ __forceinline__ void epi(cd r, cd, long long off, long long) const { p.out[off] = r; }
+};
+// last inverse pass of the Poisson solve writes only the real part (sgw_hartree)
+struct OpToReal : OpStore {
+    __device__ __forceinline__ void epi(cd r, long long off, long long) const { p.vh_out[off] = r.x; }
+};
+// last inverse pass of the Poisson solve inside the propagator: V_H never reaches memory; the merged half-step
+// phase tables of R-8 are written instead (see phase_merge_kernel for the frozen-potential form)
+struct OpPhaseMerge : OpStore {
+    __device__ __forceinline__ void epi(cd r, long long off, long long) const {
+        const double v = (p.vloc ? p.vloc[off] : 0.0) + r.x;
+        double s, c;
+        sincos((p.first ? v : v + p.vprev[off]) * p.half_dt, &s, &c);
+        p.table[off] = make_double2(c, -s);
+        p.vprev[off] = v;
+        if (p.last) {
+            sincos(v * p.half_dt, &s, &c);
+            p.last[off] = make_double2(c, -s);
+        }
+        if (p.rho_reset) p.rho_reset[off] = 0.0;
+    }
 };
 
 }  // namespace sgw

@@ -26,35 +26,28 @@ int launched(sgw_ctx* c, const char* what) {
 
 }  // namespace
 int sgw::ensure_ws(sgw_ctx* c, int n) {
-    for (int a = 0; a < n; ++a)
+    for (int a = 0; a < n && a < 2; ++a)
         if (!c->ws[a])
             SGW_TRY(check_cuda(cudaMalloc((void**)&c->ws[a], (size_t)c->max_nvec * c->ng * sizeof(cd)), "workspace"));
     return 0;
 }
 
 namespace {
-int ensure_kbc(sgw_ctx* c, int nvec) {
-    const long long need = (long long)nvec * c->nsphere * c->nproj;
-    if (need <= c->kbc_cap) return 0;
-    SGW_TRY(check_cuda(cudaStreamSynchronize(c->stream), "sync"));
-    cudaFree(c->kbc);
-    c->kbc = nullptr; c->kbc_cap = 0;
-    SGW_TRY(check_cuda(cudaMalloc((void**)&c->kbc, need * sizeof(cd)), "kb buffer"));
-    c->kbc_cap = need;
-    return 0;
-}
-
 template <int NP>
 int kb_apply_np(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau, const cd* phase, int fold) {
     dim3 grid(c->nsphere, nvec);
     const double dV = c->hx * c->hy * c->hz;
     // fold = +1: projections of phase*src, contribution times conj(phase)  (opening half step: the pass multiplies by phase on load)
     // fold = -1: projections of conj(phase)*src, contribution times phase  (closing half step: the pass multiplied by phase on store)
+    cudaEvent_t e1 = prof_begin(c, K_KB_PROJECT);
     kb_project_kernel<NP><<<grid, 128, 0, c->stream>>>(src, c->ng, c->sph_ptr, c->sph_idx, c->beta, dV, c->kbc, c->nsphere,
                                                        fold ? phase : nullptr, fold < 0 ? 1 : 0);
+    prof_end(c, e1);
     SGW_TRY(launched(c, "kb_project"));
+    e1 = prof_begin(c, K_KB_SCATTER);
     kb_scatter_kernel<NP><<<grid, 128, 0, c->stream>>>(dst, c->ng, c->sph_ptr, c->sph_idx, c->beta, c->D, c->kbc,
                                                        c->nsphere, mode, scale_or_tau, fold ? phase : nullptr, fold > 0 ? 1 : 0);
+    prof_end(c, e1);
     return launched(c, "kb_scatter");
 }
 
@@ -62,7 +55,7 @@ int kb_apply_np(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double s
 }  // namespace
 int sgw::kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau, const cd* phase, int fold) {
     if (c->nsphere == 0) return 0;
-    SGW_TRY(ensure_kbc(c, nvec));
+    if (nvec > c->max_nvec) return set_error(SGW_EINVAL, "kb_apply: more vectors than max_nvec");
     switch (c->nproj) {
         case 1: return kb_apply_np<1>(c, nvec, src, dst, mode, scale_or_tau, phase, fold);
         case 2: return kb_apply_np<2>(c, nvec, src, dst, mode, scale_or_tau, phase, fold);
@@ -83,28 +76,43 @@ OpParams zero_params() {
     return p;
 }
 
-// rho = scale * sum |psi|^2 ; V_H by the cut-Coulomb Poisson solve (R-10).  Results in c->vh (and rho/rho2).
-int hartree_into(sgw_ctx* c, int nvec, const cd* psi, double rho_scale, double* rho2, bool rho_ready = false,
-                 bool keep_complex = false) {
+// what the last inverse pass of the Poisson solve writes
+struct HartreeOut {
+    double* vh = nullptr;        // V_H itself (sgw_hartree), or
+    bool merge = false;          // the merged half-step phase tables of the propagator (R-8): c->phase, c->vprev, ...
+    int first = 0;
+    double half_dt = 0.0;
+    cd* last = nullptr;
+    double* rho_reset = nullptr;
+};
+
+// rho = scale * sum |psi|^2 ; V_H by the cut-Coulomb Poisson solve (R-10): forward x (straight from the real density),
+// forward y, z round trip with v(k)/N_g, inverse y, inverse x (which writes V_H or the phase tables): five launches.
+int hartree_into(sgw_ctx* c, int nvec, const cd* psi, double rho_scale, double* rho2, bool rho_ready, const HartreeOut& o) {
     const long long ng = c->ng;
     if (!rho_ready) {          // otherwise c->rho was accumulated by the last pass of the previous step
+        cudaEvent_t e1 = prof_begin(c, K_DENSITY);
         density_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(psi, nvec, ng, rho_scale, c->rho, rho2);
+        prof_end(c, e1);
         SGW_TRY(launched(c, "density"));
     }
-    real_to_complex_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->rho, c->pois, ng);
-    SGW_TRY(launched(c, "r2c"));
     OpParams p = zero_params();
     p.out = c->pois;
+    p.rin = c->rho;
     SGW_TRY(run_pass(c, 0, K_FWD, 1, c->pois, p));
-    SGW_TRY(run_pass(c, 1, K_FWD, 1, c->pois, p));
+    p.rin = nullptr;
+    SGW_TRY(run_pass(c, 1, K_FWD, 0, c->pois, p));
     p.mul3d = c->vk3d;
-    SGW_TRY(run_pass(c, 2, K_RT_MUL3D, 1, c->pois, p));
+    SGW_TRY(run_pass(c, 2, K_RT_MUL3D, 0, c->pois, p));
     p.mul3d = nullptr;
-    SGW_TRY(run_pass(c, 1, K_INV, 1, c->pois, p));
-    SGW_TRY(run_pass(c, 0, K_INV, 1, c->pois, p));
-    if (keep_complex) return 0;      // the caller reads V_H as the real part of c->pois
-    complex_to_real_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->pois, c->vh, ng);
-    return launched(c, "c2r");
+    SGW_TRY(run_pass(c, 1, K_INV, 0, c->pois, p));
+    if (o.merge) {
+        p.vloc = c->vloc; p.vprev = c->vprev; p.table = c->phase; p.last = o.last; p.rho_reset = o.rho_reset;
+        p.half_dt = o.half_dt; p.first = o.first;
+        return run_pass(c, 0, K_INV, 1, c->pois, p);
+    }
+    p.vh_out = o.vh;
+    return run_pass(c, 0, K_INV, 2, c->pois, p);
 }
 
 }  // namespace
@@ -153,15 +161,51 @@ static int power_iteration(sgw_ctx* c, double shift, int niter, uint64_t seed, i
 extern "C" int sgw_spectral_bounds(sgw_ctx* c, int niter, uint64_t seed, double* h_emin, double* h_emax) {
     if (!c || niter < 1 || !h_emin || !h_emax) return set_error(SGW_EINVAL, "sgw_spectral_bounds: bad argument");
     SGW_TRY(ensure_ws(c, 2));
-    double* d_red = nullptr;
-    SGW_TRY(check_cuda(cudaMalloc((void**)&d_red, 3 * sizeof(double)), "reduction buffer"));
     double la = 0.0, lb = 0.0;
-    int rc = power_iteration(c, 0.0, niter, seed, 0, d_red, &la);
-    if (!rc) rc = power_iteration(c, la, niter, seed, 1, d_red, &lb);
-    cudaFree(d_red);
-    if (rc) return rc;
+    SGW_TRY(power_iteration(c, 0.0, niter, seed, 0, c->red, &la));
+    SGW_TRY(power_iteration(c, la, niter, seed, 1, c->red, &lb));
     *h_emin = la < lb ? la : lb;
     *h_emax = la < lb ? lb : la;
+    return SGW_OK;
+}
+
+// dependent-free DFMA chains: 8 independent accumulators per thread, 32 warps per SM
+static __global__ void __launch_bounds__(1024) fp64_probe_kernel(double* out, int iters, double a, double b) {
+    double x[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) x[j] = 1.0 + 1e-3 * (threadIdx.x + j);
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) x[j] = fma(x[j], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) s += x[j];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" int sgw_probe_fp64(sgw_ctx* c, double* h_flops_per_s) {
+    if (!c || !h_flops_per_s) return set_error(SGW_EINVAL, "sgw_probe_fp64: bad argument");
+    const int blocks = 2 * c->num_sms, threads = 1024, iters = 1 << 15;
+    double* buf = nullptr;
+    SGW_TRY(check_cuda(cudaMalloc((void**)&buf, (size_t)blocks * threads * sizeof(double)), "probe buffer"));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {          // the first repetition warms up
+        cudaEventRecord(e0, c->stream);
+        fp64_probe_kernel<<<blocks, threads, 0, c->stream>>>(buf, iters, 0.999999, 1e-6);
+        cudaEventRecord(e1, c->stream);
+        c->launches++;
+        cudaError_t e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (e != cudaSuccess) { cudaFree(buf); cudaEventDestroy(e0); cudaEventDestroy(e1); return check_cuda(e, "fp64 probe"); }
+        const double rate = 2.0 * 8.0 * (double)iters * blocks * threads / (ms * 1e-3);
+        if (rep > 0 && rate > best) best = rate;
+    }
+    cudaFree(buf); cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *h_flops_per_s = best;
     return SGW_OK;
 }
 
@@ -173,33 +217,17 @@ extern "C" int sgw_apply_H(sgw_ctx* c, int nvec, const void* d_in, void* d_out) 
         const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
         const cd* i0 = in + (long long)v0 * c->ng;
         cd* o0 = out + (long long)v0 * c->ng;
-        if (c->use_engine) {
-            SGW_TRY(c->use_engine == 2 ? lean_apply_H(c, nv, i0, o0) : eng_apply_H(c, nv, i0, o0));
-            SGW_TRY(kb_apply(c, nv, i0, o0, 0, 1.0));
-            continue;
-        }
-        OpParams p = zero_params();
-        p.out = o0;
-        int rp = run_plane(c, PL_SUM, nv, i0, o0, nullptr, false);
-        if (rp < 0) return rp;
-        if (rp == 1) {
-            p.mul_re = c->kin[0];
-            SGW_TRY(run_pass(c, 0, K_RT_STORE, nv, i0, p));
-            p.mul_re = c->kin[1]; p.acc = o0;
-            SGW_TRY(run_pass(c, 1, K_RT_ACC, nv, i0, p));
-        }
-        p.acc = o0;
+        SGW_TRY(lean_apply_H(c, nv, i0, o0));
         SGW_TRY(kb_apply(c, nv, i0, o0, 0, 1.0));
-        p.mul_re = c->kin[2]; p.vtab = c->vloc;
-        SGW_TRY(run_pass(c, 2, K_RT_HFIN, nv, i0, p));
     }
     return SGW_OK;
 }
 
 extern "C" int sgw_hartree(sgw_ctx* c, int nvec, const void* d_psi, double rho_scale, double* d_vh, double* d_rho) {
     if (!c || nvec < 0 || (nvec > 0 && !d_psi) || !d_vh) return set_error(SGW_EINVAL, "sgw_hartree: bad argument");
-    SGW_TRY(hartree_into(c, nvec, (const cd*)d_psi, rho_scale, d_rho));
-    return check_cuda(cudaMemcpyAsync(d_vh, c->vh, c->ng * sizeof(double), cudaMemcpyDeviceToDevice, c->stream), "copy vh");
+    HartreeOut o;
+    o.vh = d_vh;
+    return hartree_into(c, nvec, (const cd*)d_psi, rho_scale, d_rho, false, o);
 }
 
 namespace {
@@ -211,7 +239,7 @@ int cheb_filter_body(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, 
         scale_kernel<<<blocks_for(ng * nvec, 256), 256, 0, c->stream>>>((cd*)d_psi, h_coeffs[0], ng * nvec);
         return launched(c, "scale");
     }
-    SGW_TRY(ensure_ws(c, c->use_engine ? 2 : 3));
+    SGW_TRY(ensure_ws(c, 2));
     // tables scaled by s = 2/dE so that one pass yields 2*Ht*phi directly (R-1; Eq. 3 mapping to [-1,1])
     for (int a = 0; a < 3; ++a) {
         scale_table_kernel<<<blocks_for(c->dims[a], 128), 128, 0, c->stream>>>(c->kin[a], s, c->cheb_kin[a], c->dims[a]);
@@ -221,52 +249,7 @@ int cheb_filter_body(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, 
     SGW_TRY(launched(c, "vtab"));
     for (int v0 = 0; v0 < nvec; v0 += c->max_nvec) {
         const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
-        cd* X0 = (cd*)d_psi + (long long)v0 * ng;
-        if (c->use_engine) {
-            SGW_TRY(c->use_engine == 2 ? lean_cheb_filter(c, nv, X0, h_coeffs, s, nterms)
-                                       : eng_cheb_filter(c, nv, X0, h_coeffs, s, nterms));
-            continue;
-        }
-        cd *P1 = c->ws[0], *W = c->ws[1], *O = c->ws[2];
-        cd* cur = X0;
-        cd* other = P1;              // receives phi_n; holds phi_{n-2} for n >= 2
-        // series terms not yet added to O: flags for degrees n-2 and n-1 (phi_{n-2}, phi_{n-1}, phi_n are
-        // all in registers in the last pass of term n, so O is touched only every third term)
-        bool pend_m2 = false, pend_m1 = true;  // before n = 1: degree 0 (= n-1) is pending
-        bool series_started = false;
-        for (int n = 1; n < nterms; ++n) {
-            const bool last = (n == nterms - 1);
-            const bool flush = last || pend_m2;
-            const int chunk = (c->l2_chunk > 0 && c->l2_chunk < nv) ? c->l2_chunk : nv;
-            for (int cv = 0; cv < nv; cv += chunk) {          // vector chunks sized so that W stays L2-resident
-                const int nc = (nv - cv < chunk) ? nv - cv : chunk;
-                const long long co = (long long)cv * ng;
-                OpParams p = zero_params();
-                p.out = W;
-                int rp = run_plane(c, PL_SUM, nc, cur + co, W, nullptr, true);
-                if (rp < 0) return rp;
-                if (rp == 1) {
-                    p.mul_re = c->cheb_kin[0];
-                    SGW_TRY(run_pass(c, 0, K_RT_STORE, nc, cur + co, p));
-                    p.mul_re = c->cheb_kin[1]; p.acc = W;
-                    SGW_TRY(run_pass(c, 1, K_RT_ACC, nc, cur + co, p));
-                }
-                p.acc = W;
-                SGW_TRY(kb_apply(c, nc, cur + co, W, 0, s));
-                p.mul_re = c->cheb_kin[2]; p.vtab = c->vtab;
-                p.out = other + co; p.prev = other + co; p.use_prev = (n >= 2);
-                p.hs = (n == 1) ? 0.5 : 1.0;
-                p.flush = flush; p.series = O + co; p.series_init = !series_started;
-                p.c0 = pend_m2 ? h_coeffs[n - 2] : 0.0;
-                p.c1 = pend_m1 ? h_coeffs[n - 1] : 0.0;
-                p.c2 = h_coeffs[n];
-                SGW_TRY(run_pass(c, 2, K_RT_CHEB, nc, cur + co, p));
-            }
-            if (flush) { series_started = true; pend_m2 = false; pend_m1 = false; }
-            else { pend_m2 = pend_m1; pend_m1 = true; }
-            cd* t = cur; cur = other; other = t;
-        }
-        SGW_TRY(check_cuda(cudaMemcpyAsync(X0, O, (size_t)nv * ng * sizeof(cd), cudaMemcpyDeviceToDevice, c->stream), "copy out"));
+        SGW_TRY(lean_cheb_filter(c, nv, (cd*)d_psi + (long long)v0 * ng, h_coeffs, s, nterms));
     }
     return SGW_OK;
 }
@@ -274,15 +257,10 @@ int cheb_filter_body(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, 
 // Small grids are launch-bound (cfg0: 2 MB per array, 256 launches of a few us each): when a call repeats with the
 // same vector block, window and coefficients, its launches are captured on an internal stream, instantiated as a
 // CUDA graph and replayed on the caller's stream from then on (the first call with a key launches plainly).  SGW_GRAPH=0 disables, SGW_GRAPH_BYTES moves
-// the size limit (bytes of one vector block; default 16 MB).
+// the size limit (bytes of one vector block; default 16 MB); both are read when the context is created.
 bool filter_graph_wanted(const sgw_ctx* c, int nvec, int nterms) {
-    if (c->use_engine != 2 || c->prof_on || c->nsphere > 0 || nvec > c->max_nvec || nterms < 3) return false;
-    const char* e = getenv("SGW_GRAPH");
-    if (e && atoi(e) == 0) return false;
-    double limit = 16.0e6;
-    const char* b = getenv("SGW_GRAPH_BYTES");
-    if (b && atof(b) > 0) limit = atof(b);
-    return (double)nvec * (double)c->ng * sizeof(cd) <= limit;
+    if (!c->graph_on || c->prof_on || c->nsphere > 0 || nvec > c->max_nvec || nterms < 3) return false;
+    return (double)nvec * (double)c->ng * sizeof(cd) <= c->graph_bytes;
 }
 }  // namespace
 
@@ -334,97 +312,56 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
     const long long ng = c->ng;
     cd* psi = (cd*)d_psi;
     if (!c->td_kin_valid || c->td_dt != dt) {
+        // exp(-i 1/2 k^2 dt)/N per axis, built on the device from the 1/2 k^2 tables (no host synchronisation)
         for (int a = 0; a < 3; ++a) {
-            const int N = c->dims[a];
-            std::vector<cd> t(N);
-            for (int j = 0; j < N; ++j) {
-                const long double ph = (long double)c->h_kin[a][j] * (long double)dt;
-                t[j] = make_double2((double)(cosl(ph) / N), (double)(-sinl(ph) / N));
-            }
-            SGW_TRY(check_cuda(cudaMemcpyAsync(c->td_kin[a], t.data(), N * sizeof(cd), cudaMemcpyHostToDevice, c->stream), "td table"));
-            SGW_TRY(check_cuda(cudaStreamSynchronize(c->stream), "td table sync"));
+            td_table_kernel<<<blocks_for(c->dims[a], 128), 128, 0, c->stream>>>(c->kin_raw[a], dt, c->td_kin[a], c->dims[a]);
+            SGW_TRY(launched(c, "td_table"));
         }
         c->td_dt = dt; c->td_kin_valid = true;
     }
     const bool kb = c->nsphere > 0;
-    // lean passes without KB: the last pass of a step accumulates the density of its result (atomics), so only
-    // the first step of a call reads the vectors for the density
-    const bool fuse_density = c->hartree_mode && c->use_engine == 2 && !kb;
-    // lean passes without KB: consecutive half-step phases are merged into one table applied on load (R-8)
-    const bool merged = c->use_engine == 2 && !kb;
-    if (merged && !c->vprev) {
-        SGW_TRY(check_cuda(cudaMalloc((void**)&c->vprev, ng * sizeof(double)), "vprev"));
-        SGW_TRY(check_cuda(cudaMalloc((void**)&c->phase_last, ng * sizeof(cd)), "phase_last"));
-    }
+    // without KB: the last pass of a step accumulates the density of its result (atomics), so only the first step of
+    // a call reads the vectors for the density; consecutive half-step phases are merged into one table applied on
+    // load (R-8)
+    const bool fuse_density = c->hartree_mode && !kb;
+    const bool merged = !kb;
+    int chunk = nvec < c->max_nvec ? nvec : c->max_nvec;
+    if (!kb && c->l2_chunk > 0 && c->l2_chunk < chunk) chunk = c->l2_chunk;   // chunks small enough to stay in L2 across the passes
     for (int step = 0; step < nsteps; ++step) {
-        if (c->hartree_mode || step == 0) {
-            const double* vh = nullptr;
-            if (c->hartree_mode) {
-                SGW_TRY(hartree_into(c, nvec, psi, c->rho_scale, nullptr, fuse_density && step > 0, merged));
-                vh = c->vh;
-                if (fuse_density && step + 1 < nsteps)
-                    SGW_TRY(check_cuda(cudaMemsetAsync(c->rho, 0, ng * sizeof(double), c->stream), "rho reset"));
+        const bool last = step + 1 == nsteps;
+        if (c->hartree_mode) {
+            HartreeOut o;
+            if (merged) {
+                o.merge = true; o.first = step == 0 ? 1 : 0; o.half_dt = 0.5 * dt; o.last = last ? c->phase_last : nullptr;
+                o.rho_reset = (fuse_density && !last) ? c->rho : nullptr;
+            } else {
+                o.vh = c->vh;
             }
+            SGW_TRY(hartree_into(c, nvec, psi, c->rho_scale, nullptr, fuse_density && step > 0, o));
             if (!merged) {
-                phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, vh, 0.5 * dt, c->phase, ng);
+                phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, c->vh, 0.5 * dt, c->phase, ng);
                 SGW_TRY(launched(c, "phase"));
             }
-        }
-        const bool last = step + 1 == nsteps;
-        if (merged && (c->hartree_mode || step <= 1 || last)) {
+        } else if (merged) {
             // frozen V: the merged table is exp(-i V dt/2) in step 0 and exp(-i V dt) from step 1 on
-            phase_merge_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, c->hartree_mode ? c->pois : nullptr, c->vprev,
-                                                                            0.5 * dt, step == 0 ? 1 : 0, c->phase,
-                                                                            last ? c->phase_last : nullptr, ng);
-            SGW_TRY(launched(c, "phase_merge"));
+            if (step <= 1 || last) {
+                phase_merge_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, c->vprev, 0.5 * dt, step == 0 ? 1 : 0,
+                                                                                c->phase, last ? c->phase_last : nullptr, ng);
+                SGW_TRY(launched(c, "phase_merge"));
+            }
+        } else if (step == 0) {
+            phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, nullptr, 0.5 * dt, c->phase, ng);
+            SGW_TRY(launched(c, "phase"));
         }
-        const int chunk = (!kb && c->l2_chunk > 0 && c->l2_chunk < nvec) ? c->l2_chunk : nvec;
-        for (int cv = 0; cv < nvec; cv += chunk) {            // chunks small enough to stay in L2 across the 3 passes
+        for (int cv = 0; cv < nvec; cv += chunk) {
             const int nc = (nvec - cv < chunk) ? nvec - cv : chunk;
             cd* ps = psi + (long long)cv * ng;
-            OpParams p = zero_params();
-            p.out = ps;
-            // lean passes with KB: the potential phases stay fused in the passes (on load in x, on store in z); the
-            // KB factors, which sit between them, are conjugated by the phase at their sphere points instead:
+            // with KB: the potential phases stay fused in the passes (on load in x, on store in z); the KB factors,
+            // which sit between them, are conjugated by the phase at their sphere points instead:
             //   P (psi + conj(P) S[P psi]) = P psi + S[P psi]   and   P psi3 + P S[conj(P) (P psi3)] = P (psi3 + S[psi3])
-            const bool kb_fold = kb && c->use_engine == 2;
-            if (kb_fold) {
-                SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, +1));
-            } else if (kb) {
-                dim3 g2(blocks_for(ng, 256), nc);
-                apply_phase_kernel<<<g2, 256, 0, c->stream>>>(ps, c->phase, ng);
-                SGW_TRY(launched(c, "apply_phase"));
-                SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt));
-            } else {
-                p.pro_phase = c->phase;
-            }
-            int rp = 1;
-            if (c->use_engine) {
-                SGW_TRY(c->use_engine == 2 ? lean_td_step(c, nc, ps, kb && !kb_fold, fuse_density && step + 1 < nsteps, merged, last)
-                                           : eng_td_step(c, nc, ps, kb));
-                rp = 2;
-            } else {
-                rp = run_plane(c, PL_TD, nc, ps, ps, p.pro_phase, false);
-            }
-            if (rp < 0) return rp;
-            if (rp == 1) {
-                p.mul_c = c->td_kin[0];
-                SGW_TRY(run_pass(c, 0, K_RT_TD, nc, ps, p));
-                p.pro_phase = nullptr; p.mul_c = c->td_kin[1];
-                SGW_TRY(run_pass(c, 1, K_RT_TD, nc, ps, p));
-            }
-            p.pro_phase = nullptr;
-            p.mul_c = c->td_kin[2];
-            if (!kb) p.epi_phase = c->phase;
-            if (rp != 2) SGW_TRY(run_pass(c, 2, K_RT_TD, nc, ps, p));
-            if (kb_fold) {
-                SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, -1));
-            } else if (kb) {
-                SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt));
-                dim3 g2(blocks_for(ng, 256), nc);
-                apply_phase_kernel<<<g2, 256, 0, c->stream>>>(ps, c->phase, ng);
-                SGW_TRY(launched(c, "apply_phase"));
-            }
+            if (kb) SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, +1));
+            SGW_TRY(lean_td_step(c, nc, ps, false, fuse_density && !last, merged, last));
+            if (kb) SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, -1));
         }
     }
     return SGW_OK;

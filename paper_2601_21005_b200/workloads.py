@@ -274,9 +274,15 @@ def snap_center(grid: Grid):
 
 
 def make_workload(name: str, *, n: int | None = None, nvec: int | None = None,
-                  nterms: int | None = None, td_steps: int | None = None) -> Workload:
-    """Build config ``name`` ('cfg0'..'cfg4'); keyword overrides shrink it for tests."""
+                  nterms: int | None = None, td_steps: int | None = None, subcell: bool = False) -> Workload:
+    """Build config ``name`` ('cfg0'..'cfg4'); keyword overrides shrink it for tests.
+
+    ``subcell=True`` with a smaller ``n``: the central n^3 sub-cell of the config (same spacing, only the atoms whose
+    local Gaussians and KB spheres lie inside it, same spectral window as the full config) -- the bounded sample the
+    CPU oracle is timed on in bench.py.
+    """
     n0, h, nv0, nt0, td0, r2u, use_kb = _CFG[name]
+    full_n = n0
     n = n or n0
     grid = Grid(n, n, n, h, h, h)
     nvec = nvec if nvec is not None else nv0
@@ -291,6 +297,10 @@ def make_workload(name: str, *, n: int | None = None, nvec: int | None = None,
         atoms = "8 Gaussian wells"
     else:
         si_rel, h_rel = diamond_cluster(r2u)
+        if subcell and n < full_n:
+            half = 0.5 * n * h - KB_RADIUS - h
+            si_rel = si_rel[np.max(np.abs(si_rel), axis=1) <= half]
+            h_rel = h_rel[np.max(np.abs(h_rel), axis=1) <= half]
         si, hy = si_rel + c0, h_rel + c0
         centers = np.concatenate([si, hy], axis=0)
         depths = [2.0] * len(si) + [1.0] * len(hy)

@@ -1,5 +1,4 @@
-"""GPU parity at the sizes of BASELINE.json's configs, in the launch configuration bench.py times, for the
-three pass implementations (SGW_ENGINE=2 lean passes, the default; 0 staged kernels; 1 pass engine).
+"""GPU parity at the sizes of BASELINE.json's configs, in the launch configuration bench.py times.
 
 Full-size oracle runs are only feasible for a few applications, so ("Oracle cost and
 parity coverage"): every config shape gets a single H apply compared element by element on a declared
@@ -38,12 +37,10 @@ def relerr(got, want):
     return float(np.max(np.linalg.norm(got - want, axis=1) / np.linalg.norm(want, axis=1)))
 
 
-@pytest.mark.parametrize("engine", ["2", "0", "1"])
-def test_cfg1_bench_configuration_sampled_vectors(api, torch_cuda, oracle, monkeypatch, engine):
+def test_cfg1_bench_configuration_sampled_vectors(api, torch_cuda, oracle, monkeypatch):
     """cfg1 exactly as bench.py runs it (96^3, 64 vectors in one call, max_nvec = 64): the first 33 terms of
     the 512-term coefficient list.  Vectors 0, 37 and 63 of the batch are compared with the oracle."""
     torch = torch_cuda
-    monkeypatch.setenv("SGW_ENGINE", engine)
     w = W.make_workload("cfg1")
     coeffs = w.coeffs[:33]
     ctx = api.context_for(w)
@@ -60,12 +57,10 @@ def test_cfg1_bench_configuration_sampled_vectors(api, torch_cuda, oracle, monke
     ctx.close()
 
 
-@pytest.mark.parametrize("engine", ["2", "0", "1"])
-def test_cfg2_td_hartree_prefix_all_vectors(api, torch_cuda, oracle, monkeypatch, engine):
+def test_cfg2_td_hartree_prefix_all_vectors(api, torch_cuda, oracle, monkeypatch):
     """cfg2 (128^3, 16 vectors): a 9-term filter, then 3 split-operator steps with the Hartree potential
     rebuilt every step from all 16 vectors (prefix of the 2000 steps), every vector compared."""
     torch = torch_cuda
-    monkeypatch.setenv("SGW_ENGINE", engine)
     w = W.make_workload("cfg2", nterms=9)
     ctx = api.context_for(w)
     psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
@@ -85,12 +80,10 @@ def test_cfg2_td_hartree_prefix_all_vectors(api, torch_cuda, oracle, monkeypatch
     ctx.close()
 
 
-@pytest.mark.parametrize("engine", ["2"])
-def test_cfg3_shape_apply_H_and_terms_with_kb(api, torch_cuda, oracle, monkeypatch, engine):
+def test_cfg3_shape_apply_H_and_terms_with_kb(api, torch_cuda, oracle, monkeypatch):
     """cfg3 shape (256^3, Si705H300 local + KB projectors): 2 vectors out of the 256; one H apply and a
     4-term filter (3 applications) compared element by element."""
     torch = torch_cuda
-    monkeypatch.setenv("SGW_ENGINE", engine)
     w = W.make_workload("cfg3", nvec=2, nterms=4)
     assert w.atoms == "Si705H300" and w.kb.nsphere == 705
     ctx = api.context_for(w)
@@ -127,13 +120,10 @@ def test_cfg4_shape_apply_H_and_td_step_with_kb(api, torch_cuda, oracle):
 
 @pytest.mark.parametrize("n,nz,nvec,use_kb", [(32, 32, 4, False), (48, 48, 3, True), (64, 24, 2, True), (24, 12, 5, True),
                                               (12, 12, 2, False)])
-@pytest.mark.parametrize("engine", ["2", "1"])
-def test_engine_path_small_grids(api, torch_cuda, oracle, monkeypatch, n, nz, nvec, use_kb, engine):
-    """The lean passes and the pass engine on cubic grids (one dependent launch), non-cubic grids (one launch per
-    pass) and an axis length that is not a multiple of 8 (4 pencils per tile): H apply, odd and even term
-    counts, TD with and without the Hartree rebuild."""
+def test_lean_passes_small_grids(api, torch_cuda, oracle, monkeypatch, n, nz, nvec, use_kb):
+    """The lean passes on cubic grids, non-cubic grids (three axis launches) and an axis length that is not a
+    multiple of 8 (4 pencils per tile): H apply, odd and even term counts, TD with and without the Hartree rebuild."""
     torch = torch_cuda
-    monkeypatch.setenv("SGW_ENGINE", engine)
     g = W.Grid(n, n, nz, 0.5, 0.5, 0.55)
     rng = np.random.default_rng(7 * n + nz)
     L = np.array(g.box)
@@ -165,13 +155,11 @@ def test_engine_path_small_grids(api, torch_cuda, oracle, monkeypatch, n, nz, nv
     ctx.close()
 
 
-@pytest.mark.parametrize("engine", ["2", "0", "1"])
 @pytest.mark.parametrize("n,nvec", [(32, 80), (48, 40)])
-def test_many_planes_per_cta(api, torch_cuda, oracle, monkeypatch, engine, n, nvec):
+def test_many_planes_per_cta(api, torch_cuda, oracle, monkeypatch, n, nvec):
     """Enough xy planes (2560 / 1920) that every persistent CTA owns several plane groups and every warp group
     many tiles: the regime of the bench workload, at a size the oracle finishes in seconds."""
     torch = torch_cuda
-    monkeypatch.setenv("SGW_ENGINE", engine)
     g = W.Grid(n, n, n, 0.5, 0.5, 0.5)
     rng = np.random.default_rng(n + nvec)
     centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
@@ -223,7 +211,6 @@ def test_lean_plane_kernel_group_and_cta_variants(api, torch_cuda, oracle, monke
     """The lean plane kernel with several planes per CTA-owned group (ragged last group: 5 * 32 planes is not a
     multiple of 3) and with the one-CTA-per-SM (16-warp) variant, against the oracle."""
     torch = torch_cuda
-    monkeypatch.setenv("SGW_ENGINE", "2")
     monkeypatch.setenv("SGW_LEAN_G", G)
     monkeypatch.setenv("SGW_LEAN_CTAS", ctas)
     n, nvec = 32, 5
@@ -253,7 +240,6 @@ def test_lean_plane_cluster_kernel(api, torch_cuda, oracle, monkeypatch, n, nz, 
     on for both families, against the oracle; nvec * nz planes exceed the resident clusters (at most 2 * 148 / size),
     so the plane loop runs a ragged second round."""
     torch = torch_cuda
-    monkeypatch.setenv("SGW_ENGINE", "2")
     monkeypatch.setenv("SGW_LEAN_CLUSTER", "1")
     g = W.Grid(n, n, nz, 0.5, 0.5, 0.5)
     rng = np.random.default_rng(23)
@@ -273,32 +259,6 @@ def test_lean_plane_cluster_kernel(api, torch_cuda, oracle, monkeypatch, n, nz, 
     want = oracle.td_propagate(g, vloc, None, psi, 0.05, 2, 1, 2.0 / (nvec * g.dV) * 0.01, ld=True)
     assert relerr(t.cpu().numpy(), want) < TOL_FULL
     ctx.close()
-
-
-def test_cfg1_full_length_three_implementations_agree(api, torch_cuda, monkeypatch):
-    """cfg1 at full size and full length (64 vectors, all 512 terms), where the oracle would need hours: the three
-    pass implementations are independent formulations of the recurrence (lean and engine accumulate in place with
-    the series updated every second term in the x pass; the staged kernels keep a separate W array and update the
-    series every third term in the z pass), so their agreement to rounding level is a full-length check.  The
-    oracle comparison of the same launch configuration on a 33-term prefix is
-    test_cfg1_bench_configuration_sampled_vectors."""
-    torch = torch_cuda
-    w = W.make_workload("cfg1")
-    res = {}
-    for engine in ("2", "0", "1"):
-        monkeypatch.setenv("SGW_ENGINE", engine)
-        ctx = api.context_for(w)
-        psi = ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec)
-        ctx.sgw_cheb_filter(psi, w.coeffs, w.emin, w.emax)
-        assert ctx.sgw_sync_check() == 0
-        res[engine] = psi
-        ctx.close()
-    ref = res["2"].reshape(w.nvec, -1)
-    nrm = torch.linalg.vector_norm(ref, dim=1)
-    assert float(nrm.min()) > 0
-    for engine in ("0", "1"):
-        d = torch.linalg.vector_norm(res[engine].reshape(w.nvec, -1) - ref, dim=1) / nrm
-        assert float(d.max()) < 1e-10, (engine, float(d.max()))
 
 
 def test_cfg2_full_length_propagation_invariants(api, torch_cuda):

@@ -434,7 +434,7 @@ def test_plane_pass_H_cheb_td(api, torch_cuda, oracle, monkeypatch, n, nz, nvec,
     and the single-plane path."""
     torch = torch_cuda
     if G is not None:
-        monkeypatch.setenv("SGW_PLANE_G", G)
+        monkeypatch.setenv("SGW_LEAN_G", G)
     g, vloc, kb, rng = problem(n, n, nz, seed=n + nz)
     psi = rvec(rng, g, nvec)
     ctx = make_ctx(api, torch, g, vloc, kb, nvec)
