@@ -1,0 +1,355 @@
+// sgw_acc.cuh -- TMA accumulate kernel for sm_100a: acc += c * (T_x + T_y + T_z + vtab) cur + e * v, one launch.
+//
+// Why it exists (profiles/r02_*.md): in the register-operand passes of sgw_lean.cuh every global operand goes through
+// the LSU (and, for the late operands of the first pass, exposes its latency); the x+y plane pass was bound by that
+// path.  Here no consumer thread touches global memory for the vectors at all:
+//   * a LOADER thread brings tiles of B = 8 pencils into a ring of shared-memory slots with bulk asynchronous copies
+//     (cp.async.bulk for the contiguous x tiles, cp.async.bulk.tensor.3d through a tensor map for the strided y / z
+//     tiles), completion on an mbarrier per slot;
+//   * consumer warp groups run the two-stage round trip IN PLACE in the slot: the dense TMA layout is
+//     bank-conflict free for 16-byte elements with the pencils-fastest thread mapping, and every thread reads and
+//     writes the same slots in stage A, so the tile is its own exchange buffer;
+//   * a STORER thread sends the finished tile to the accumulator with bulk REDUCE-ADD operations
+//     (cp.reduce.async.bulk[.tensor].add.f64): the read-modify-write of acc happens in L2, the SM never loads it.
+// Because every direction's contribution is a pure sum into acc, the x, y and z tiles of a term have NO mutual
+// dependency: one launch, no x->y handoff, no barrier between directions; the order of the tiles only decides what
+// stays in L2 (all tiles of a vector together when its arrays fit, else planes then z columns).
+// The Chebyshev recurrence is run in Clenshaw form with sign-folded buffers so that every step is such a sum
+// (sgw_program.cu: acc_cheb_filter; Eq. 3).
+#pragma once
+#include <cuda.h>
+
+#include "sgw_lean.cuh"
+
+namespace sgw {
+
+struct AccArgs {
+    const cd* cur;            // input vectors
+    cd* acc;                  // accumulated into
+    const cd* v;              // second input added with coefficient e in the x tiles (Clenshaw start vector) or NULL
+    const double* vtab;       // N_g real table or NULL
+    const double* kre[3];     // real k tables per axis (include 1/N and any scale)
+    const cd* tw;             // exp(-2 pi i j / N)
+    double c, e;
+    int nvec, nz;             // cubic grids only: nx = ny = nz = N
+    int kinds;                // bit 0: x tiles, bit 1: y tiles, bit 2: z tiles
+    int plane_major;          // 1: x and y tiles interleaved plane by plane (z tiles, if any, after all planes)
+    unsigned ntiles;
+};
+
+template <int N>
+struct AccCfg {
+    static constexpr int B = 8;
+    static constexpr int R1 = Fact2<N>::R1, R2 = Fact2<N>::R2;
+    static constexpr int TG = B * R2;                        // threads of a consumer group
+    static constexpr int GW = (TG + 31) / 32, GT = GW * 32;
+    static constexpr int TASKS = R1 * B, ROUNDS = (TASKS + GT - 1) / GT;
+    static constexpr int XP = N + 1;                         // x tile: row pitch in elements (odd pitch: bank-conflict free)
+    static constexpr int TILE = ((XP * B * 16 + 127) / 128) * 128;   // slot bytes (>= N * B * 16 of the dense y / z tile)
+    static constexpr int TABLES = 2 * N * 16 + 3 * N * 8;
+    static constexpr int NBOX = N <= 256 ? N : N / 2;        // tensor-map box rows (at most 256 per dimension)
+    static constexpr int NOPS = N / NBOX;
+    // consumer groups: bounded by the register file (x[R1] and w[R1] live across the transform: ~160 registers)
+    static constexpr int NG = (GW == 1) ? 8 : (GW == 2 ? 5 : (GW <= 4 ? 2 : 1));
+    static constexpr int T = 64 + NG * GT;                   // loader warp, storer warp, consumers
+    static constexpr int MAXS = 24;
+};
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, unsigned n) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(b)), "r"(n));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* b, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "ACC_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra ACC_DONE;\n"
+        "bra ACC_WAIT;\n"
+        "ACC_DONE:\n"
+        "}\n" ::"r"(smem_u32(b)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_load(void* dst, const void* src, unsigned bytes, uint64_t* b) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst)), "l"(src),
+                 "r"(bytes), "r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void bulk_red_add(void* gdst, const void* ssrc, unsigned bytes) {
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f64 [%0], [%1], %2;\n" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* m, int c0, int c1, int c2, uint64_t* b) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];\n" ::"r"(
+                     smem_u32(dst)), "l"(m), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void tma_red_add_3d(const CUtensorMap* m, const void* src, int c0, int c1, int c2) {
+    asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];\n" ::"l"(m),
+                 "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;\n" ::: "memory"); }
+template <int K>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;\n" ::"n"(K) : "memory"); }
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+
+// Tile sequence of one CTA (tiles blockIdx.x, blockIdx.x + gridDim.x, ...) without per-tile integer divisions.
+//   vector-major: the tiles of a vector are [x tiles | y tiles | z tiles] (kinds present in the launch), vector after vector
+//   plane-major (x and y kinds only): the tiles of a plane are [x tiles | y tiles], plane after plane
+// kind 0 x: rows [j*8, j*8+8) of plane p;  1 y: columns [j*8, ..) of plane p;  2 z: xy points [j*8, ..) of vector v.
+template <int N>
+struct AccIter {
+    static constexpr unsigned TPP = N / 8, TPV = (unsigned)N * N / 8;
+    unsigned t, q, u, period, step;      // u = vector (vector-major) or plane (plane-major), q = offset inside it
+    int kind;
+    unsigned v, p, j;
+    __device__ __forceinline__ void init(const AccArgs& a, unsigned t0, unsigned stride) {
+        const unsigned nk = (unsigned)((a.kinds & 1) + ((a.kinds >> 1) & 1) + ((a.kinds >> 2) & 1));
+        period = a.plane_major ? nk * TPP : nk * TPV;
+        t = t0; step = stride;
+        u = t0 / period; q = t0 - u * period;
+    }
+    __device__ __forceinline__ void decode(const AccArgs& a) {
+        if (a.plane_major) {
+            const unsigned k = q / TPP;
+            kind = (a.kinds & 1) ? (int)k : 1;
+            j = q - k * TPP; p = u; v = 0;
+        } else {
+            const unsigned k = q / TPV, i = q - k * TPV;
+            int kd = 0, seen = 0;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                if ((a.kinds >> d) & 1) { if (seen == (int)k) kd = d; ++seen; }
+            }
+            kind = kd; v = u;
+            if (kd == 2) { j = i; p = 0; }
+            else { const unsigned z = i / TPP; p = u * (unsigned)a.nz + z; j = i - z * TPP; }
+        }
+    }
+    __device__ __forceinline__ void next() {
+        t += step; q += step;
+        while (q >= period) { q -= period; ++u; }
+    }
+};
+
+// the round trip of one tile, in place in its slot.  XK: x tile (rows of pitch XP, lanes along the row) or y / z tile
+// (dense [point][pencil], lanes along the pencils).
+template <int N, bool XK>
+__device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, const cd* vtile, const double* __restrict__ vt, const cd* twA,
+                                                 const cd* twB, const double* ktab, int gt, int bar_id, uint64_t* vempty, uint64_t* vdone) {
+    using C = AccCfg<N>;
+    constexpr int R1 = C::R1, R2 = C::R2, TG = C::TG, GW = C::GW, GT = C::GT, TASKS = C::TASKS, ROUNDS = C::ROUNDS, B = C::B;
+    constexpr bool WCACHE = R2 <= 8;
+    constexpr int SB = XK ? C::XP : 1, SI = XK ? 1 : B;      // element strides of (pencil, point) inside the slot
+    const bool actA = gt < TG;
+    const int n2 = XK ? gt % R2 : gt / B, bA = XK ? gt / R2 : gt % B;
+    cd* eA = tile + bA * SB + n2 * SI;
+    cd x[R1];
+    cd w[XK ? R1 : 1];
+    if (actA) {
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) x[n1] = eA[n1 * R2 * SI];
+        if (XK) {
+            // what the x tiles add besides the transform: (c * vtab) * cur + e * v, kept in registers across the transform
+            const double c = a.c, e = a.e;
+#pragma unroll
+            for (int n1 = 0; n1 < R1; ++n1) {
+                const double cv = vt ? c * __ldg(vt + n1 * R2) : 0.0;
+                w[n1] = make_double2(cv * x[n1].x, cv * x[n1].y);
+            }
+            if (vtile) {
+                const cd* eV = vtile + bA * SB + n2 * SI;
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) { const cd u = eV[n1 * R2 * SI]; w[n1].x += e * u.x; w[n1].y += e * u.y; }
+            }
+        }
+        Dft<R1, -1>::run(x);
+        if (WCACHE) {
+#pragma unroll
+            for (int j = 0; j < R1; ++j) eA[j * R2 * SI] = x[j];
+        } else {
+            eA[0] = x[0];
+#pragma unroll
+            for (int j = 1; j < R1; ++j) eA[j * R2 * SI] = cmul(x[j], twA[j * R2 + n2]);
+        }
+    }
+    lean_sync<GW>(bar_id);
+    // every thread of the group has read the v tile: its slot is free again (its `done` barrier is advanced too, so
+    // that the phase of every barrier of a slot equals the number of times the slot has been used)
+    if (XK && vtile && gt == 0) { mbar_arrive(vdone); mbar_arrive(vempty); }
+#pragma unroll
+    for (int rd = 0; rd < ROUNDS; ++rd) {
+        const int task = gt + rd * GT;
+        if (task < TASKS) {
+            const int bB = task % B, k1 = task / B;
+            cd* eB = tile + bB * SB + k1 * R2 * SI;
+            cd y[R2], wc[WCACHE ? R2 : 1];
+            y[0] = eB[0];
+            if (WCACHE) {
+#pragma unroll
+                for (int m = 1; m < R2; ++m) { wc[m] = twB[m * R1 + k1]; y[m] = cmul(eB[m * SI], wc[m]); }
+            } else {
+#pragma unroll
+                for (int m = 1; m < R2; ++m) y[m] = eB[m * SI];
+            }
+            Dft<R2, -1>::run(y);
+            const double* kt = ktab + k1;
+#pragma unroll
+            for (int k2 = 0; k2 < R2; ++k2) y[k2] = cscale(y[k2], kt[R1 * k2]);
+            Dft<R2, +1>::run(y);
+            eB[0] = y[0];
+#pragma unroll
+            for (int m = 1; m < R2; ++m) eB[m * SI] = cmulc(y[m], WCACHE ? wc[m] : twB[m * R1 + k1]);
+        }
+    }
+    lean_sync<GW>(bar_id);
+    if (actA) {
+#pragma unroll
+        for (int j = 0; j < R1; ++j) x[j] = eA[j * R2 * SI];
+        Dft<R1, +1>::run(x);
+        const double c = a.c;
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) {
+            cd r = cscale(x[n1], c);
+            if (XK) { r.x += w[n1].x; r.y += w[n1].y; }
+            eA[n1 * R2 * SI] = r;
+        }
+        fence_proxy_async_smem();                            // the bulk reduce-add reads the slot through the async proxy
+    }
+    lean_sync<GW>(bar_id);
+}
+
+template <int N>
+__global__ void __launch_bounds__(AccCfg<N>::T, 1)
+acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const __grid_constant__ CUtensorMap cur_z,
+               const __grid_constant__ CUtensorMap acc_y, const __grid_constant__ CUtensorMap acc_z, int nslots) {
+    using C = AccCfg<N>;
+    constexpr int GT = C::GT, NG = C::NG, B = C::B, TILE = C::TILE;
+    constexpr unsigned ROWB = N * 16, YZB = N * B * 16;
+    extern __shared__ __align__(128) char smraw[];
+    char* slots = smraw;                                      // nslots * TILE, 128-byte aligned
+    cd* twA = reinterpret_cast<cd*>(smraw + (size_t)nslots * TILE);
+    cd* twB = twA + N;
+    double* ktab = reinterpret_cast<double*>(twB + N);        // [3][N]
+    uint64_t* full = reinterpret_cast<uint64_t*>(ktab + 3 * N);
+    uint64_t* done = full + C::MAXS;
+    uint64_t* empty = done + C::MAXS;
+    const int tid = threadIdx.x;
+    for (int i = tid; i < N; i += C::T) {
+        twA[i] = a.tw[(i % C::R2) * (i / C::R2)];
+        twB[i] = a.tw[(i / C::R1) * (i % C::R1)];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) ktab[d * N + i] = a.kre[d][i];
+    }
+    if (tid == 0) {
+        for (int s = 0; s < nslots; ++s) { mbar_init(full + s, 1); mbar_init(done + s, 1); mbar_init(empty + s, 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+    const unsigned S = (unsigned)nslots;
+    const bool usev = a.v != nullptr;
+    const long long ng = (long long)N * N * a.nz;
+
+    if (tid < 64) {
+        if (tid == 0) {
+            // ---------------- loader: one slot per tile (two for an x tile with a v operand), in tile order
+            unsigned seq = 0;
+            AccIter<N> tl;
+            for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next()) {
+                tl.decode(a);
+                const int nops = (tl.kind == 0 && usev) ? 2 : 1;
+                for (int op = 0; op < nops; ++op, ++seq) {
+                    const unsigned s = seq % S, round = seq / S;
+                    if (round > 0) mbar_wait(empty + s, (round - 1) & 1);
+                    char* dst = slots + (size_t)s * TILE;
+                    if (tl.kind == 0) {
+                        mbar_expect_tx(full + s, B * ROWB);
+                        const cd* src = (op == 0 ? a.cur : a.v) + (long long)tl.p * (N * N) + (long long)tl.j * (B * N);
+#pragma unroll
+                        for (int b = 0; b < B; ++b) bulk_load(dst + (size_t)b * C::XP * 16, src + b * N, ROWB, full + s);
+                    } else {
+                        mbar_expect_tx(full + s, YZB);
+                        const CUtensorMap* m = tl.kind == 1 ? &cur_y : &cur_z;
+                        const int c2 = tl.kind == 1 ? (int)tl.p : (int)tl.v;
+#pragma unroll
+                        for (int o = 0; o < C::NOPS; ++o)
+                            tma_load_3d(dst + (size_t)o * C::NBOX * B * 16, m, (int)tl.j * 16, o * C::NBOX, c2, full + s);
+                    }
+                }
+            }
+        } else if (tid == 32) {
+            // ---------------- storer: reduce-add of finished tiles, slots released when the engine has read them
+            unsigned seq = 0, pend[2], npend = 0;
+            AccIter<N> tl;
+            for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next()) {
+                tl.decode(a);
+                const unsigned s = seq % S, round = seq / S;
+                seq += (tl.kind == 0 && usev) ? 2 : 1;
+                mbar_wait(done + s, round & 1);
+                const char* src = slots + (size_t)s * TILE;
+                if (tl.kind == 0) {
+                    cd* dst = a.acc + (long long)tl.p * (N * N) + (long long)tl.j * (B * N);
+#pragma unroll
+                    for (int b = 0; b < B; ++b) bulk_red_add(dst + b * N, src + (size_t)b * C::XP * 16, ROWB);
+                } else {
+                    const CUtensorMap* m = tl.kind == 1 ? &acc_y : &acc_z;
+                    const int c2 = tl.kind == 1 ? (int)tl.p : (int)tl.v;
+#pragma unroll
+                    for (int o = 0; o < C::NOPS; ++o) tma_red_add_3d(m, src + (size_t)o * C::NBOX * B * 16, (int)tl.j * 16, o * C::NBOX, c2);
+                }
+                bulk_commit();
+                if (npend == 2) {
+                    bulk_wait_read<2>();                      // all but the two newest groups have been read: tile k-2 is free
+                    mbar_arrive(empty + pend[0]);
+                    pend[0] = pend[1]; npend = 1;
+                }
+                pend[npend++] = s;
+            }
+            asm volatile("cp.async.bulk.wait_group 0;\n" ::: "memory");      // every reduce-add has been performed
+        }
+        return;
+    }
+
+    // ---------------- consumers: group g takes the CTA's tiles g, g + NG, ...
+    const int ct = tid - 64, grp = ct / GT, gt = ct % GT;
+    unsigned seq = 0, i = 0;
+    AccIter<N> tl;
+    for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next(), ++i) {
+        tl.decode(a);
+        const unsigned s = seq % S, round = seq / S;
+        const bool xv = tl.kind == 0 && usev;
+        const unsigned s2 = (seq + 1) % S, round2 = (seq + 1) / S;
+        seq += xv ? 2 : 1;
+        if ((int)(i % NG) != grp) continue;
+        cd* tile = reinterpret_cast<cd*>(slots + (size_t)s * TILE);
+        if (tl.kind == 0) {
+            const int n2 = gt % C::R2, bA = gt / C::R2;
+            const long long g0 = ((long long)tl.p * (N * N) + (long long)tl.j * (B * N)) % ng;
+            const double* vt = a.vtab ? a.vtab + g0 + bA * N + n2 : nullptr;
+            mbar_wait(full + s, round & 1);
+            const cd* vtile = nullptr;
+            if (xv) { mbar_wait(full + s2, round2 & 1); vtile = reinterpret_cast<const cd*>(slots + (size_t)s2 * TILE); }
+            acc_tile_compute<N, true>(a, tile, vtile, vt, twA, twB, ktab, gt, grp, empty + s2, done + s2);
+        } else {
+            mbar_wait(full + s, round & 1);
+            acc_tile_compute<N, false>(a, tile, nullptr, nullptr, twA, twB, ktab + tl.kind * N, gt, grp, nullptr, nullptr);
+        }
+        if (gt == 0) mbar_arrive(done + s);
+    }
+}
+
+struct AccCall {
+    AccArgs args;
+    CUtensorMap cur_y, cur_z, acc_y, acc_z;
+    int num_sms;
+    int* occ;                 // context-owned: [0] = 1 once the kernel attribute is set
+    cudaStream_t stream;
+};
+// returns 0, -(stage*1000 + cudaError) on failure, 1 if this length has no accumulate kernel
+typedef int (*acc_launch_fn)(const AccCall*);
+
+}  // namespace sgw

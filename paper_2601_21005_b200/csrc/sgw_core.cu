@@ -8,7 +8,8 @@
 
 #define SGW_DECL(N)                                             \
     extern "C" int sgw_pass_launch_##N(const sgw::PassCall*);   \
-    extern "C" int sgw_lean_launch_##N(const sgw::LeanCall*, int);
+    extern "C" int sgw_lean_launch_##N(const sgw::LeanCall*, int);  \
+    extern "C" int sgw_acc_launch_##N(const sgw::AccCall*);
 SGW_DECL(8) SGW_DECL(12) SGW_DECL(16) SGW_DECL(24) SGW_DECL(32) SGW_DECL(48) SGW_DECL(64) SGW_DECL(96)
 SGW_DECL(128) SGW_DECL(192) SGW_DECL(256) SGW_DECL(384)
 #undef SGW_DECL
@@ -31,6 +32,14 @@ int check_cuda(cudaError_t e, const char* what) {
 static pass_launch_fn launcher_for(int n) {
     switch (n) {
 #define SGW_CASE(N) case N: return sgw_pass_launch_##N;
+        SGW_SIZES(SGW_CASE)
+#undef SGW_CASE
+        default: return nullptr;
+    }
+}
+static acc_launch_fn acc_launcher_for(int n) {
+    switch (n) {
+#define SGW_CASE(N) case N: return sgw_acc_launch_##N;
         SGW_SIZES(SGW_CASE)
 #undef SGW_CASE
         default: return nullptr;
@@ -196,7 +205,7 @@ extern "C" int sgw_destroy(sgw_ctx* c) {
     cudaFree(c->ws[0]); cudaFree(c->ws[1]);
     cudaFree(c->vloc); cudaFree(c->vtab); cudaFree(c->vk3d); cudaFree(c->sph_ptr); cudaFree(c->sph_idx);
     cudaFree(c->beta); cudaFree(c->D); cudaFree(c->kbc); cudaFree(c->pois); cudaFree(c->rho); cudaFree(c->vh);
-    cudaFree(c->phase); cudaFree(c->phase_last); cudaFree(c->vprev); cudaFree(c->red);
+    cudaFree(c->phase); cudaFree(c->phase_last); cudaFree(c->vprev); cudaFree(c->red); cudaFree(c->team_cnt);
     delete c;
     return SGW_OK;
 }
@@ -232,6 +241,18 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     c->lean_G = env_int("SGW_LEAN_G", 0);
     c->lean_ctas = env_int("SGW_LEAN_CTAS", 0);
     c->lean_cluster = env_int("SGW_LEAN_CLUSTER", -1);
+    c->lean_team = env_int("SGW_LEAN_TEAM", -1);
+    c->use_acc = env_int("SGW_ACC", -1);
+    c->acc_l2_bytes = 1.0e6 * env_int("SGW_ACC_L2_MB", 48);
+    c->acc = (nx == ny && ny == nz && nx >= 32 && nx % 8 == 0) ? acc_launcher_for(nx) : nullptr;
+    {
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &c->tmap_encode, cudaEnableDefault, &qr) != cudaSuccess ||
+            qr != cudaDriverEntryPointSuccess)
+            c->tmap_encode = nullptr;
+    }
+    if (!c->tmap_encode) c->acc = nullptr;
+    c->lean_vminor = env_int("SGW_LEAN_VMINOR", -1);
     c->lean_chunk = env_int("SGW_LEAN_CHUNK", 0);
     c->l2_chunk = env_int("SGW_L2_CHUNK", 0);
     c->pdl = env_int("SGW_PDL", 0) == 1;
@@ -273,6 +294,7 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     if (!rc) rc = dev_alloc(&c->phase_last, c->ng);
     if (!rc) rc = dev_alloc(&c->vprev, c->ng);
     if (!rc) rc = dev_alloc(&c->red, 4);
+    if (!rc) rc = dev_alloc(&c->team_cnt, (size_t)max_nvec * nz);
     if (!rc) {
         const double Lx = nx * hx, Ly = ny * hy, Lz = nz * hz;
         const double Rc = 0.5 * fmin(Lx, fmin(Ly, Lz));

@@ -9,6 +9,7 @@
 #include "../../include/sgw.h"
 #include "sgw_ops.cuh"
 #include "sgw_lean.cuh"
+#include "sgw_acc.cuh"
 
 struct sgw_ctx {
     int nx, ny, nz;
@@ -22,9 +23,17 @@ struct sgw_ctx {
     int leanB;                               // lean passes: pencils per tile (8, or 4 when nx or ny is not a multiple of 8)
     sgw::pass_launch_fn pass[3];             // per-axis launcher of the Poisson passes (x, y, z)
     sgw::lean_launch_fn lean[3];             // per-axis launcher of the lean passes
-    int lean_occ[3][16];                     // occupancy results of the lean kernels, per axis length (filled on first use)
+    sgw::acc_launch_fn acc;                  // TMA accumulate kernel (cubic grids) or NULL
+    int acc_occ[4];
+    int use_acc;                             // real family through the TMA accumulate kernel (SGW_ACC; default: where it is built and measured faster)
+    double acc_l2_bytes;                     // one-launch terms when cur + acc + v of a vector are at most this (SGW_ACC_L2_MB)
+    void* tmap_encode;                       // cuTensorMapEncodeTiled (driver entry point)
+    int lean_occ[3][18];                     // occupancy results of the lean kernels, per axis length (filled on first use)
     int lean_G, lean_ctas;                   // plane kernel: planes per CTA-owned group, CTAs per SM (0 = auto)
     int lean_cluster;                        // -1 auto, 0 / 1 forced (SGW_LEAN_CLUSTER)
+    int lean_team;                           // -1 auto, 0 / 1 forced (SGW_LEAN_TEAM): team-owned planes
+    int lean_vminor;                         // -1 auto, 0 / 1 forced (SGW_LEAN_VMINOR): vectors fastest in the tile order
+    unsigned* team_cnt;                      // max_nvec * nz plane arrival counters of the team plane kernel
     int lean_chunk;                          // filter: vectors per L2-resident chunk (SGW_LEAN_CHUNK; 0 = whole batch)
     int l2_chunk;                            // TD: vectors per L2-resident chunk (SGW_L2_CHUNK; 0 = whole batch)
     int pdl;                                 // programmatic dependent launch (SGW_PDL=1)
@@ -88,6 +97,9 @@ int run_pass(sgw_ctx* c, int axis, int kind, int variant, const cd* in, const Op
 int lean_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out);
 int lean_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* h_coeffs, double s, int nterms);
 int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb, bool accumulate_density, bool merged, bool last);
+// TMA accumulate implementations (sgw_program.cu)
+int acc_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out);
+int acc_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* h_coeffs, double s, int nterms);
 cudaEvent_t prof_begin(sgw_ctx* c, int tag);
 void prof_end(sgw_ctx* c, cudaEvent_t e1);
 int kb_apply(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau, const cd* phase = nullptr,

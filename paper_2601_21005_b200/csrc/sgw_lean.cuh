@@ -66,6 +66,10 @@ struct LeanArgs {
     int nx, ny, nz;
     unsigned ntiles;          // axis kernel: tiles; plane kernel: planes (nz * nvec)
     int G;                    // plane kernel: planes per CTA-owned group
+    int nvec;                 // vectors of the launch
+    int vminor;               // 1: consecutive tiles / planes run over the vectors at one grid location, so the N_g tables
+                              //    (potential, phases) are read from HBM once per launch instead of once per vector
+    unsigned* cnt;            // team plane kernel: one arrival counter per plane (zeroed before the launch)
 };
 
 template <int N, int B, int WPC_ = 8>
@@ -295,26 +299,36 @@ __global__ void __launch_bounds__(LeanCfg<N, B>::T, LeanCfg<N, B>::MINB) axis_le
     if (AXIS == 0) { n2 = gt % R2; bA = gt / R2; e0 = bA * a.nx + n2; estep = R2; }
     else { bA = gt % B; n2 = gt / B; const int sN = (AXIS == 1) ? (CUBE ? N : a.nx) : nxy; e0 = n2 * sN + bA; estep = R2 * sN; }
     const unsigned stride = gridDim.x * NWG;
-    const unsigned rows_per_vec = (unsigned)(a.ny * a.nz), cb_per_plane = (unsigned)(a.nx / B), blk_per_vec = (unsigned)(nxy / B);
-    for (unsigned t = blockIdx.x * NWG + grp; t < a.ntiles; t += stride) {
-        long long base;
-        int g0;
+    const unsigned cb_per_plane = (unsigned)(a.nx / B);
+    const unsigned nvec = (unsigned)a.nvec;
+    // tile -> offset of its first element in the vector arrays (vectors fastest when vminor) and in the N_g tables
+    auto locate = [&](unsigned t, int& g0) -> long long {
+        unsigned v, q;
+        if (a.vminor) { q = t / nvec; v = t - q * nvec; }
+        else { const unsigned tpv = a.ntiles / nvec; v = t / tpv; q = t - v * tpv; }
         if (AXIS == 0) {
-            base = (long long)t * (B * a.nx);
-            g0 = (int)((t * B) % rows_per_vec) * a.nx;
+            g0 = (int)q * (B * a.nx);
         } else if (AXIS == 1) {
-            const unsigned p = t / cb_per_plane, cb = t - p * cb_per_plane;
-            base = (long long)p * nxy + (long long)cb * B;
-            g0 = (int)(p % (unsigned)a.nz) * nxy + (int)cb * B;
+            const unsigned z = q / cb_per_plane, cb = q - z * cb_per_plane;
+            g0 = (int)z * nxy + (int)cb * B;
         } else {
-            const unsigned v = t / blk_per_vec, i = t - v * blk_per_vec;
-            base = (long long)v * ng + (long long)i * B;
-            g0 = (int)i * B;
+            g0 = (int)q * B;
         }
-        const long long o = base + e0;
+        return (long long)v * ng + g0;
+    };
+    for (unsigned t = blockIdx.x * NWG + grp; t < a.ntiles; t += stride) {
+        int g0;
+        const long long o = locate(t, g0) + e0;
         lean_tile<N, B, 8, CPLX, AXIS == 0, H_STREAM, H_STREAM>(a, 0, a.cur + o, a.acc + o, a.series + o, a.vtab + g0 + e0, a.phase + g0 + e0, estep,
                                          xch, twA, twB, ktab, grp, gt, n2, bA);
     }
+}
+
+// k-th plane of a launch -> plane index p = v * nz + z (vminor: consecutive k run over the vectors at one z)
+__device__ __forceinline__ unsigned plane_of(const LeanArgs& a, unsigned k) {
+    if (!a.vminor) return k;
+    const unsigned nvec = (unsigned)a.nvec, z = k / nvec, v = k - z * nvec;
+    return v * (unsigned)a.nz + z;
 }
 
 // x pass then y pass of whole xy planes (nx == ny == N) in one launch.  A CTA owns planes [pg*G, pg*G + G): its
@@ -346,7 +360,7 @@ __global__ void __launch_bounds__(LeanCfg<N, B, WPC>::T, LeanCfg<N, B, WPC>::MIN
     for (unsigned pg = blockIdx.x; pg < ngroups; pg += gridDim.x) {
         const unsigned p0 = pg * G, np = (a.ntiles - p0 < G) ? a.ntiles - p0 : G;
         for (unsigned q = grp; q < np * TPP; q += NWG) {
-            const unsigned p = p0 + q / TPP, rb = q % TPP;
+            const unsigned p = plane_of(a, p0 + q / TPP), rb = q % TPP;
             const long long o = (long long)p * NXY + (long long)rb * (B * N) + e0x;
             const int g = (int)(p % (unsigned)a.nz) * NXY + (int)rb * (B * N) + e0x;
             lean_tile<N, B, WPC, CPLX, true, H_KEEP, H_KEEP>(a, 0, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g, R2, xch, twA, twB,
@@ -354,7 +368,7 @@ __global__ void __launch_bounds__(LeanCfg<N, B, WPC>::T, LeanCfg<N, B, WPC>::MIN
         }
         __syncthreads();                                     // every row tile of the group is stored (to L2)
         for (unsigned q = grp; q < np * TPP; q += NWG) {
-            const unsigned p = p0 + q / TPP, cb = q % TPP;
+            const unsigned p = plane_of(a, p0 + q / TPP), cb = q % TPP;
             const long long o = (long long)p * NXY + (long long)cb * B + e0y;
             const int g = (int)(p % (unsigned)a.nz) * NXY + (int)cb * B + e0y;
             // the y pass reads what the x pass left in acc; for the complex family cur == acc
@@ -392,7 +406,8 @@ __global__ void __launch_bounds__(LeanCfg<N, B, 8>::T, LeanCfg<N, B, 8>::MINB) p
     const int n2x = gt % R2, bAx = gt / R2, e0x = bAx * N + n2x;                 // x: lanes along n
     const int bAy = gt % B, n2y = gt / B, e0y = n2y * N + bAy;                   // y: lanes along b
     const unsigned me = crank * NWG + grp, gsz = CS * NWG;
-    for (unsigned p = cid; p < a.ntiles; p += ncl) {
+    for (unsigned k = cid; k < a.ntiles; k += ncl) {
+        const unsigned p = plane_of(a, k);
         const int gp = (int)(p % (unsigned)a.nz) * NXY;
         for (unsigned q = me; q < TPP; q += gsz) {
             const long long o = (long long)p * NXY + (long long)q * (B * N) + e0x;
@@ -410,16 +425,73 @@ __global__ void __launch_bounds__(LeanCfg<N, B, 8>::T, LeanCfg<N, B, 8>::MINB) p
     }
 }
 
+// Team variant of the plane kernel, for planes too large for CTA- or cluster-owned transposes through L2 (256^2,
+// 384^2): a TEAM of TPP = N/B warp groups (on as many SMs as that takes: 24 SMs for 384^2) owns one plane at a
+// time, one row tile and one column tile per group, so only (groups / TPP) planes are in flight and the x->y
+// transpose of a 2.4 MB plane stays in L2.  The teams are software constructs: the x->y handoff is one arrival
+// counter per plane in global memory (release: group barrier, fence, atomic; acquire: one lane polls, group barrier),
+// software-pipelined so that a group does its row tile of plane k+1 before it waits for plane k.  All CTAs must be
+// co-resident: the launcher uses a cooperative launch sized by the occupancy query.
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+template <int N, int B, bool CPLX>
+__global__ void __launch_bounds__(LeanCfg<N, B, 8>::T, LeanCfg<N, B, 8>::MINB) plane_team_kernel(const LeanArgs a) {
+    using C = LeanCfg<N, B, 8>;
+    constexpr int R2 = C::R2, GT = C::GT, NWG = C::NWG, GW = C::GW;
+    constexpr unsigned TPP = N / B;
+    constexpr int NXY = N * N;
+    extern __shared__ __align__(16) char smraw[];
+    cd* twA = reinterpret_cast<cd*>(smraw);
+    cd* twB = twA + N;
+    char* ktab = reinterpret_cast<char*>(twB + N);
+    const int tid = threadIdx.x, grp = tid / GT, gt = tid % GT;
+    cd* xch = reinterpret_cast<cd*>(ktab + 2 * N * (CPLX ? 16 : 8)) + grp * C::XCH;
+    lean_tables<N, B, 8, CPLX>(a, twA, twB, ktab);
+    const char* ktab_y = ktab + N * (CPLX ? 16 : 8);
+    const int n2x = gt % R2, bAx = gt / R2, e0x = bAx * N + n2x;                 // x: lanes along n
+    const int bAy = gt % B, n2y = gt / B, e0y = n2y * N + bAy;                   // y: lanes along b
+    const unsigned gid = blockIdx.x * NWG + grp, nteams = (gridDim.x * NWG) / TPP;
+    const unsigned team = gid / TPP, slot = gid - team * TPP;
+    if (team >= nteams) return;                                                // left-over groups
+    long long prev = -1;
+    for (unsigned k = team;; k += nteams) {
+        const bool have = k < a.ntiles;
+        if (have) {
+            const unsigned p = plane_of(a, k);
+            const long long o = (long long)p * NXY + (long long)slot * (B * N) + e0x;
+            const int g = (int)(p % (unsigned)a.nz) * NXY + (int)slot * (B * N) + e0x;
+            lean_tile<N, B, 8, CPLX, true, H_KEEP, H_KEEP>(a, 0, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g, R2, xch,
+                                                           twA, twB, ktab, grp, gt, n2x, bAx);
+            // lean_tile ends with a group barrier: every store of the tile precedes this release
+            if (gt == 0) { __threadfence(); atomicAdd(a.cnt + k, 1u); }
+        }
+        if (prev >= 0) {
+            if (gt == 0) { while (ld_acquire_u32(a.cnt + prev) < TPP) __nanosleep(64); }
+            lean_sync<GW>(grp);
+            const unsigned p = plane_of(a, (unsigned)prev);
+            const long long o = (long long)p * NXY + (long long)slot * B + e0y;
+            const int g = (int)(p % (unsigned)a.nz) * NXY + (int)slot * B + e0y;
+            lean_tile<N, B, 8, CPLX, false, H_STREAM, H_STREAM>(a, 1, a.cur + o, a.acc + o, a.series + o, a.vtab + g, a.phase + g,
+                                                                R2 * N, xch, twA, twB, ktab_y, grp, gt, n2y, bAy);
+        }
+        if (!have) break;
+        prev = k;
+    }
+}
+
 struct LeanCall {
     LeanArgs args;
     int cplx;
     int kind;                 // 0..2: axis pass along x, y, z; 3: plane pass (x then y); 4 / 5: z / y pass on a cubic grid
     int ctas_per_sm;          // 0 = as many as fit
     int wpc;                  // plane kernel: warps per CTA, 8 (two CTAs per SM) or 16 (one)
-    int cluster;              // plane kernel: 1 = cluster-owned planes (plane_cluster_kernel), 0 = CTA-owned
+    int cluster;              // plane kernel: 1 = cluster-owned planes (plane_cluster_kernel), 2 = team-owned, 0 = CTA-owned
     int pdl;                  // 1 = programmatic dependent launch (SGW_PDL=1)
     int num_sms;              // of the context's device
-    int* occ;                 // context-owned cache of occupancy results for this axis length, 16 ints, zero-initialised
+    int* occ;                 // context-owned cache of occupancy results for this axis length, 18 ints, zero-initialised
     cudaStream_t stream;
 };
 // returns 0, -(stage*1000 + cudaError) on failure, or 1 if this (N, B) is not instantiated

@@ -4,6 +4,7 @@
 
 #include "sgw_ops.cuh"
 #include "sgw_lean.cuh"
+#include "sgw_acc.cuh"
 
 #ifndef SGW_N
 #error "compile with -DSGW_N=<axis length>"
@@ -102,12 +103,44 @@ static int launch_plane_cluster(const LeanCall* c) {
     return e == cudaSuccess ? 0 : -(4000 + (int)e);
 }
 
+// team-owned planes (plane_team_kernel): cooperative launch of as many CTAs as are co-resident
+template <int B, bool CPLX>
+static int launch_plane_team(const LeanCall* c) {
+    constexpr int N = SGW_N;
+    if (N % B) return 1;
+    using Cfg = LeanCfg<N, B, 8>;
+    const size_t smem = CPLX ? Cfg::SMEM_CPLX : Cfg::SMEM_REAL;
+    auto kern = plane_team_kernel<N, B, CPLX>;
+    int& per_sm = c->occ[CPLX ? 17 : 16];
+    if (!per_sm) {
+        cudaError_t e = smem > 48 * 1024 ? cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) : cudaSuccess;
+        if (e != cudaSuccess) return -(1000 + (int)e);
+        int n = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, Cfg::T, smem);
+        if (e != cudaSuccess) return -(2000 + (int)e);
+        if (n < 1) return 1;
+        per_sm = n;
+    }
+    int ctas = per_sm;
+    if (c->ctas_per_sm > 0 && c->ctas_per_sm < ctas) ctas = c->ctas_per_sm;
+    const long long grid = (long long)ctas * c->num_sms;
+    if (grid * Cfg::NWG < N / B) return 1;        // not even one team
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(Cfg::T); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, c->args);
+    return e == cudaSuccess ? 0 : -(4000 + (int)e);
+}
+
 template <int B, bool CPLX>
 static int launch_lean_b(const LeanCall* c) {
     constexpr int N = SGW_N;
     using Cfg = LeanCfg<N, B>;
     const size_t smem = CPLX ? Cfg::SMEM_CPLX : Cfg::SMEM_REAL;
-    int* occ = c->occ + (CPLX ? 9 : 0);          // per context and axis length: [0..6] real kinds, [7], [8] clusters, [9..15] complex kinds
+    int* occ = c->occ + (CPLX ? 9 : 0);          // per context and axis length: [0..6] real kinds, [7], [8] clusters, [9..15] complex kinds, [16], [17] teams
     const long long tiles_ctas = ((long long)c->args.ntiles + Cfg::NWG - 1) / Cfg::NWG;
     switch (c->kind) {
         case 0: return lean_launch_kernel(axis_lean_kernel<N, B, CPLX, 0, false>, Cfg::T, smem, tiles_ctas, c, &occ[0]);
@@ -117,6 +150,7 @@ static int launch_lean_b(const LeanCall* c) {
         case 4: return lean_launch_kernel(axis_lean_kernel<N, B, CPLX, 2, true>, Cfg::T, smem, tiles_ctas, c, &occ[4]);
         case 3: {
             if (N % B) return 1;
+            if (c->cluster == 2) return launch_plane_team<B, CPLX>(c);
             if (c->cluster) { const int rc = launch_plane_cluster<B, CPLX>(c); if (rc != 1) return rc; }
             const long long ngroups = ((long long)c->args.ntiles + c->args.G - 1) / c->args.G;
             if (c->wpc == 16) {
@@ -131,6 +165,34 @@ static int launch_lean_b(const LeanCall* c) {
         }
     }
     return -1;
+}
+
+// ---- TMA accumulate kernel (sgw_acc.cuh): one persistent CTA per SM ---------------------------------
+static int launch_acc(const AccCall* c) {
+#if SGW_N >= 32 && SGW_N % 8 == 0
+    constexpr int N = SGW_N;
+    using Cfg = AccCfg<N>;
+    auto kern = acc_tma_kernel<N>;
+    const int fixed = Cfg::TABLES + 3 * Cfg::MAXS * 8 + 128;
+    int nslots = (227 * 1024 - fixed) / Cfg::TILE;
+    if (nslots > Cfg::MAXS) nslots = Cfg::MAXS;
+    if (nslots < 4) return 1;
+    const size_t smem = (size_t)nslots * Cfg::TILE + fixed;
+    if (!c->occ[0]) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return -(1000 + (int)e);
+        c->occ[0] = 1;
+    }
+    long long grid = c->num_sms;
+    if (grid > (long long)c->args.ntiles) grid = c->args.ntiles;
+    if (grid <= 0) return 0;
+    kern<<<(unsigned)grid, Cfg::T, smem, c->stream>>>(c->args, c->cur_y, c->cur_z, c->acc_y, c->acc_z, nslots);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? 0 : -(4000 + (int)e);
+#else
+    (void)c;
+    return 1;
+#endif
 }
 
 }  // namespace sgw
@@ -157,3 +219,6 @@ extern "C" int SGW_CAT(sgw_lean_launch_, SGW_N)(const sgw::LeanCall* c, int B) {
     if (B == 4) return c->cplx ? launch_lean_b<4, true>(c) : launch_lean_b<4, false>(c);
     return 1;
 }
+
+// TMA accumulate kernel: acc += c (T + vtab) cur + e v on a cubic grid of this axis length.  Returns 1 if not built.
+extern "C" int SGW_CAT(sgw_acc_launch_, SGW_N)(const sgw::AccCall* c) { return sgw::launch_acc(c); }

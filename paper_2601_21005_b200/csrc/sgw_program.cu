@@ -25,6 +25,16 @@ __global__ void cheb_tail_kernel(cd* out, const cd* P, const cd* Q, const cd* O,
     out[i] = r;
 }
 
+int Fact2_R2(int n) {
+    switch (n) {
+        case 8: case 12: case 16: case 24: case 32: case 48: return 4;
+        case 64: case 96: case 128: return 8;
+        case 192: case 256: return 16;
+        case 384: return 24;
+    }
+    return 8;
+}
+
 struct LeanOp {
     const cd* cur; cd* acc; cd* series;
     const double* vtab; const cd* phase; const cd* phase_z;
@@ -78,6 +88,16 @@ bool lean_use_plane(const sgw_ctx* c, bool cplx, int* G, int* ctas, int* wpc, in
     // overrides.
     int use_cluster = (!cplx && (n == 128 || n == 256)) ? 1 : 0;
     if (c->lean_cluster >= 0) use_cluster = c->lean_cluster ? 1 : 0;
+    // Team-owned planes (plane_team_kernel: N/B warp groups on several SMs own a plane at a time, software-pipelined
+    // arrival counters): the way 256^2 and 384^2 planes transpose through L2 (a 384^2 plane of two arrays is 4.7 MB).
+    int use_team = (n >= 256) ? 1 : 0;
+    if (c->lean_team >= 0) use_team = c->lean_team ? 1 : 0;
+    if (c->lean_cluster == 1) use_team = 0;
+    const int gw = (B * Fact2_R2(n) + 31) / 32, groups_per_cta = 8 / gw > 0 ? 8 / gw : 1;
+    if (use_team && c->num_sms * groups_per_cta >= n / B) {           // at least one team even at one CTA per SM
+        *cluster = 2; *G = 1; *ctas = 0; *wpc = 8;
+        return true;
+    }
     *cluster = use_cluster;
     if (use_cluster && (n == 256 || n == 384)) { *G = 1; *ctas = 2; *wpc = 8; return true; }
     if (use_cluster) { *G = 1; *ctas = 2; *wpc = 8; return true; }
@@ -100,6 +120,12 @@ int lean_apply(sgw_ctx* c, int nv, const LeanOp& op, int kind_tag, bool allow_pl
     a.rho = op.rho; a.dens_scale = op.dens_scale;
     a.hs = op.hs; a.c0 = op.c0; a.c1 = op.c1;
     a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+    a.nvec = nv;
+    // vectors fastest in the tile order when an N_g table is read and does not stay in L2 by itself
+    const bool table = op.cplx ? (op.phase != nullptr) : (op.vtab != nullptr);
+    a.vminor = (table && nv > 1 && (double)c->ng * (op.cplx ? 16.0 : 8.0) > 24.0e6) ? 1 : 0;
+    if (c->lean_vminor >= 0) a.vminor = (c->lean_vminor && nv > 1) ? 1 : 0;
+    a.cnt = c->team_cnt;
     int G = 1, ctas = 0, wpc = 8, cluster = 0;
     if (allow_plane && lean_use_plane(c, op.cplx, &G, &ctas, &wpc, &cluster)) {
         a.tw = c->tw[0];
@@ -107,6 +133,8 @@ int lean_apply(sgw_ctx* c, int nv, const LeanOp& op, int kind_tag, bool allow_pl
         a.flags[0] = op.fx; a.alpha[0] = op.ax; a.flags[1] = op.fy; a.alpha[1] = op.ay;
         a.ntiles = (unsigned)((long long)nv * c->nz);
         a.G = G;
+        if (cluster == 2)
+            SGW_TRY(check_cuda(cudaMemsetAsync(c->team_cnt, 0, (size_t)a.ntiles * sizeof(unsigned), c->stream), "team counters"));
         SGW_TRY(lean_launch(c, 0, 3, a, op.cplx, ctas, 1 * K_NKINDS + (op.cplx ? K_RT_TD : K_RT_ACC), wpc, cluster));
     } else {
         a.tw = c->tw[0];
@@ -206,6 +234,136 @@ int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb, bool accumulate_density
     op.cplx = true;
     for (int a = 0; a < 3; ++a) op.kc[a] = c->td_kin[a];
     return lean_apply(c, nvec, op, K_RT_TD);
+}
+
+}  // namespace sgw
+
+// =====================================================================================================
+// TMA accumulate kernel (sgw_acc.cuh): acc += c (T + vtab) cur + e v
+// =====================================================================================================
+namespace {
+
+typedef CUresult (*tmap_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// tensor maps of one vector array (nv vectors of a cubic N^3 grid, interleaved complex = pairs of doubles) for the
+// strided tiles: y tiles (8 x-adjacent pencils along y of one plane) and z tiles (8 xy-adjacent pencils along z)
+int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap* mz) {
+    const cuuint64_t N = (cuuint64_t)c->nx;
+    tmap_encode_fn enc = (tmap_encode_fn)c->tmap_encode;
+    const cuuint32_t nbox = (cuuint32_t)(N <= 256 ? N : N / 2);
+    const cuuint32_t box[3] = {16, nbox, 1}, es[3] = {1, 1, 1};
+    const cuuint64_t dy[3] = {2 * N, N, N * (cuuint64_t)nv}, sy[2] = {N * 16, N * N * 16};
+    const cuuint64_t dz[3] = {2 * N * N, N, (cuuint64_t)nv}, sz[2] = {N * N * 16, N * N * N * 16};
+    CUresult r = enc(my, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dy, sy, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r == CUDA_SUCCESS)
+        r = enc(mz, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dz, sz, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return set_error(SGW_ECUDA, "cuTensorMapEncodeTiled failed: " + std::to_string((int)r));
+    return 0;
+}
+
+struct AccOp {
+    const cd* cur; cd* acc; const cd* v;
+    const double* vtab;
+    const double* kre[3];
+    double c, e;
+};
+
+int acc_launch_one(sgw_ctx* c, int nv, const AccOp& op, const AccCall& maps, int kinds, int plane_major, int prof_tag) {
+    AccCall call = maps;
+    AccArgs& a = call.args;
+    memset(&a, 0, sizeof(a));
+    a.cur = op.cur; a.acc = op.acc; a.v = op.v; a.vtab = op.vtab;
+    for (int d = 0; d < 3; ++d) a.kre[d] = op.kre[d];
+    a.tw = c->tw[0];
+    a.c = op.c; a.e = op.e;
+    a.nvec = nv; a.nz = c->nz;
+    a.kinds = kinds; a.plane_major = plane_major;
+    const long long n = c->nx, tpv = n * n / 8, nk = (kinds & 1) + ((kinds >> 1) & 1) + ((kinds >> 2) & 1);
+    const long long ntiles = plane_major ? nk * (n / 8) * c->nz * nv : nk * tpv * nv;
+    if (ntiles > 0xffffffffLL - 1024) return set_error(SGW_EINVAL, "too many tiles for one launch");
+    a.ntiles = (unsigned)ntiles;
+    call.num_sms = c->num_sms;
+    call.occ = c->acc_occ;
+    call.stream = c->stream;
+    cudaEvent_t e1 = prof_begin(c, prof_tag);
+    const int rc = c->acc(&call);
+    if (rc != 0)
+        return set_error(rc < 0 ? SGW_ECUDA : SGW_ESIZE, "accumulate kernel launch failed: stage " + std::to_string((-rc) / 1000) + ": " +
+                                                             cudaGetErrorString((cudaError_t)((-rc) % 1000)));
+    prof_end(c, e1);
+    c->launches++;
+    return 0;
+}
+
+// acc += c (T + vtab) cur + e v over nv vectors.  One launch when the arrays of a vector stay in L2 together (all
+// x, y and z tiles of a vector are then adjacent in the tile order: cur is read from HBM once, acc read and written
+// once); otherwise the x and y tiles plane by plane, then the z tiles in a second launch.
+int acc_apply(sgw_ctx* c, int nv, const AccOp& op, int z_tag) {
+    AccCall maps;
+    memset(&maps, 0, sizeof(maps));
+    SGW_TRY(acc_maps(c, op.cur, nv, &maps.cur_y, &maps.cur_z));
+    SGW_TRY(acc_maps(c, op.acc, nv, &maps.acc_y, &maps.acc_z));
+    const double per_vec = 16.0 * (double)c->ng * (op.v ? 3.0 : 2.0);
+    if (per_vec <= c->acc_l2_bytes) return acc_launch_one(c, nv, op, maps, 7, 0, 1 * K_NKINDS + K_RT_ACC);
+    SGW_TRY(acc_launch_one(c, nv, op, maps, 3, 1, 1 * K_NKINDS + K_RT_ACC));
+    return acc_launch_one(c, nv, op, maps, 4, 0, 2 * K_NKINDS + z_tag);
+}
+
+__global__ void scaled_copy_kernel(cd* out, const cd* in, double a, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = cscale(in[i], a);
+}
+
+}  // namespace
+
+namespace sgw {
+
+// out = (Tx + Ty + Tz + V_loc) in (the KB term is added by the caller)
+int acc_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out) {
+    SGW_TRY(check_cuda(cudaMemsetAsync(out, 0, (size_t)nv * c->ng * sizeof(cd), c->stream), "clear output"));
+    AccOp op;
+    memset(&op, 0, sizeof(op));
+    op.cur = in; op.acc = out; op.v = nullptr; op.vtab = c->vloc;
+    for (int d = 0; d < 3; ++d) op.kre[d] = c->kin[d];
+    op.c = 1.0; op.e = 0.0;
+    return acc_apply(c, nv, op, K_RT_HFIN);
+}
+
+// Chebyshev series sum_n a_n T_n(Ht) v (Eq. 3; R-1) by the Clenshaw recurrence
+//     b_k = a_k v + 2 Ht b_{k+1} - b_{k+2}   (k = L .. 1, b_{L+1} = b_{L+2} = 0),   result = a_0 v + Ht b_1 - b_2,
+// which needs the same L = nterms - 1 applications of H as the forward recurrence but only READS v every step
+// instead of reading and writing a series array.  Stored are Q_k = t_k b_k with signs t = + + - - + + ... (t_k t_{k+2}
+// = -1), which turns every step into a pure accumulation into the buffer that holds Q_{k+2}:
+//     Q_k = Q_{k+2} + (t_k t_{k+1}) 2 Ht Q_{k+1} + (t_k a_k) v ,      result = Q_2 + (t_1 / 2) 2 Ht Q_1 + a_0 v   (t_2 = -1)
+// -- the form the accumulate kernel computes.  Tables are scaled so that (T + vtab) = 2 Ht (sgw_cheb_filter).
+int acc_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* a, double s, int nterms) {
+    const long long ng = c->ng, n = (long long)nvec * ng;
+    SGW_TRY(ensure_ws(c, 2));
+    const bool kb = c->nsphere > 0;
+    const int L = nterms - 1;
+    auto t = [](int k) { return ((k & 3) < 2) ? 1.0 : -1.0; };
+    cd *A = c->ws[0], *Bf = c->ws[1];
+    scaled_copy_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(A, psi, t(L) * a[L], n);      // Q_L
+    c->launches++;
+    SGW_TRY(check_cuda(cudaGetLastError(), "scaled_copy"));
+    SGW_TRY(check_cuda(cudaMemsetAsync(Bf, 0, (size_t)n * sizeof(cd), c->stream), "clear"));            // Q_{L+1}
+    AccOp op;
+    memset(&op, 0, sizeof(op));
+    op.v = psi; op.vtab = c->vtab;
+    for (int d = 0; d < 3; ++d) op.kre[d] = c->cheb_kin[d];
+    for (int k = L - 1; k >= 0; --k) {
+        op.cur = A; op.acc = Bf;
+        op.c = k > 0 ? t(k) * t(k + 1) : 0.5 * t(1);
+        op.e = k > 0 ? t(k) * a[k] : a[0];
+        SGW_TRY(acc_apply(c, nvec, op, K_RT_CHEB));
+        if (kb) SGW_TRY(kb_apply(c, nvec, A, Bf, 0, s * op.c));
+        cd* tmp = A; A = Bf; Bf = tmp;                       // A = Q_k, Bf = Q_{k+1}
+    }
+    return check_cuda(cudaMemcpyAsync(psi, A, (size_t)n * sizeof(cd), cudaMemcpyDeviceToDevice, c->stream), "copy result");
 }
 
 }  // namespace sgw

@@ -19,6 +19,14 @@ inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) /
         if (rc_ != 0) return rc_; \
     } while (0)
 
+// the real family (H apply, Chebyshev filter) runs through the TMA accumulate kernel where it is built (cubic grids,
+// axis length a multiple of 8) and enabled (SGW_ACC=0/1; default: on for 64..128 points per axis)
+bool acc_enabled(const sgw_ctx* c) {
+    if (!c->acc) return false;
+    if (c->use_acc >= 0) return c->use_acc != 0;
+    return c->nx >= 64 && c->nx <= 128;
+}
+
 int launched(sgw_ctx* c, const char* what) {
     c->launches++;
     return check_cuda(cudaGetLastError(), what);
@@ -217,7 +225,7 @@ extern "C" int sgw_apply_H(sgw_ctx* c, int nvec, const void* d_in, void* d_out) 
         const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
         const cd* i0 = in + (long long)v0 * c->ng;
         cd* o0 = out + (long long)v0 * c->ng;
-        SGW_TRY(lean_apply_H(c, nv, i0, o0));
+        SGW_TRY(acc_enabled(c) ? acc_apply_H(c, nv, i0, o0) : lean_apply_H(c, nv, i0, o0));
         SGW_TRY(kb_apply(c, nv, i0, o0, 0, 1.0));
     }
     return SGW_OK;
@@ -249,7 +257,8 @@ int cheb_filter_body(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, 
     SGW_TRY(launched(c, "vtab"));
     for (int v0 = 0; v0 < nvec; v0 += c->max_nvec) {
         const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
-        SGW_TRY(lean_cheb_filter(c, nv, (cd*)d_psi + (long long)v0 * ng, h_coeffs, s, nterms));
+        cd* X0 = (cd*)d_psi + (long long)v0 * ng;
+        SGW_TRY(acc_enabled(c) ? acc_cheb_filter(c, nv, X0, h_coeffs, s, nterms) : lean_cheb_filter(c, nv, X0, h_coeffs, s, nterms));
     }
     return SGW_OK;
 }

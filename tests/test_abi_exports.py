@@ -12,7 +12,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def _declared():
     src = open(os.path.join(ROOT, "include", "sgw.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(sgw_[a-z_A-Z]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(sgw_[a-z_A-Z0-9]+)\s*\(", src)))
 
 
 def test_library_exports_every_declared_symbol():
@@ -62,7 +62,7 @@ def _prototypes():
     src = open(os.path.join(ROOT, "include", "sgw.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     protos = {}
-    for m in re.finditer(r"([A-Za-z_0-9 ]+?[ *]+)(sgw_[A-Za-z_]+)\s*\(([^)]*)\)\s*;", src):
+    for m in re.finditer(r"([A-Za-z_0-9 ]+?[ *]+)(sgw_[A-Za-z_0-9]+)\s*\(([^)]*)\)\s*;", src):
         args = [a.strip() for a in m.group(3).split(",")] if m.group(3).strip() != "void" else []
         protos[m.group(2)] = (m.group(1).strip(), args)
     return protos

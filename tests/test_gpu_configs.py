@@ -261,6 +261,104 @@ def test_lean_plane_cluster_kernel(api, torch_cuda, oracle, monkeypatch, n, nz, 
     ctx.close()
 
 
+@pytest.mark.parametrize("n,nz,nvec,vminor", [(32, 24, 7, "1"), (64, 16, 5, "0"), (96, 8, 6, "1"), (256, 8, 3, "1")])
+def test_lean_plane_team_kernel_and_vector_minor_order(api, torch_cuda, oracle, monkeypatch, n, nz, nvec, vminor):
+    """The team-owned plane kernel (N/8 warp groups per plane, arrival counter per plane, software-pipelined row and
+    column tiles; default for 256^2 and 384^2 planes), forced on for small planes so that many teams run several
+    rounds with a ragged last round, with the tile order running over the vectors first (vminor) or last; both
+    operator families, against the oracle."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_LEAN_TEAM", "1")
+    monkeypatch.setenv("SGW_LEAN_VMINOR", vminor)
+    g = W.Grid(n, n, nz, 0.5, 0.5, 0.5)
+    rng = np.random.default_rng(29 + n)
+    centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    psi = rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    got = ctx.sgw_apply_H(torch.from_numpy(psi).cuda()).cpu().numpy()
+    assert relerr(got, oracle.apply_H(g, vloc, None, psi, ld=True)) < TOL_H
+    emin, emax = W.spectral_bounds(g, vloc, False)
+    coeffs = rng.standard_normal(6)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+    assert relerr(t.cpu().numpy(), oracle.cheb_filter(g, vloc, None, psi, coeffs, emin, emax, ld=True)) < TOL_FULL
+    rs = 2.0 / (nvec * g.dV) * 0.01
+    ctx.sgw_set_td(1, rs)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_td_propagate(t, 0.05, 3)
+    assert relerr(t.cpu().numpy(), oracle.td_propagate(g, vloc, None, psi, 0.05, 3, 1, rs, ld=True)) < TOL_FULL
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
+
+
+@pytest.mark.parametrize("shape", [(32, 48, 24), (64, 32, 16)])
+def test_vector_minor_order_on_axis_passes(api, torch_cuda, oracle, monkeypatch, shape):
+    """Non-square planes take three axis passes; with the tile order running over the vectors first (the order used
+    when the potential / phase table does not fit L2) the results are those of the oracle, with KB projectors."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_LEAN_VMINOR", "1")
+    nx, ny, nz = shape
+    nvec = 5
+    g = W.Grid(nx, ny, nz, 0.5, 0.45, 0.55)
+    rng = np.random.default_rng(nx + ny)
+    centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    kb = W.kb_projectors(g, centers[:2], radius=1.8, sigma=0.7)
+    psi = rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                         torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+    emin, emax = W.spectral_bounds(g, vloc, True)
+    coeffs = rng.standard_normal(7)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+    assert relerr(t.cpu().numpy(), oracle.cheb_filter(g, vloc, kb, psi, coeffs, emin, emax, ld=True)) < TOL_FULL
+    rs = 2.0 / (nvec * g.dV) * 0.01
+    ctx.sgw_set_td(1, rs)
+    t = torch.from_numpy(psi).cuda()
+    ctx.sgw_td_propagate(t, 0.05, 3)
+    assert relerr(t.cpu().numpy(), oracle.td_propagate(g, vloc, kb, psi, 0.05, 3, 1, rs, ld=True)) < TOL_FULL
+    ctx.close()
+
+
+@pytest.mark.parametrize("n,nvec,use_kb,l2mb", [(32, 5, True, None), (48, 3, False, "0"), (64, 4, True, "0"), (96, 3, False, None),
+                                                 (128, 2, True, None), (96, 5, True, "0")])
+def test_tma_accumulate_kernel_apply_H_and_clenshaw_filter(api, torch_cuda, oracle, monkeypatch, n, nvec, use_kb, l2mb):
+    """The TMA accumulate kernel (sgw_acc.cuh: bulk / tensor-map loads into a shared-memory ring, in-place round trip,
+    bulk reduce-add into the accumulator) forced on for every cubic size it is built for: H apply and the Clenshaw
+    form of the Chebyshev series for 1..10 coefficients against the oracle's forward recurrence, in the one-launch
+    (vector-major) order and, with SGW_ACC_L2_MB=0, in the two-launch (planes, then z columns) order."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_ACC", "1")
+    if l2mb is not None:
+        monkeypatch.setenv("SGW_ACC_L2_MB", l2mb)
+    g = W.Grid(n, n, n, 0.5, 0.45, 0.55)
+    rng = np.random.default_rng(41 + n)
+    centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    kb = W.kb_projectors(g, centers[:2], radius=1.8, sigma=0.7) if use_kb else W.KB.empty()
+    kbo = kb if kb.nsphere else None
+    psi = rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    if kb.nsphere:
+        ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                             torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+    got = ctx.sgw_apply_H(torch.from_numpy(psi).cuda()).cpu().numpy()
+    assert relerr(got, oracle.apply_H(g, vloc, kbo, psi, ld=True)) < TOL_H
+    emin, emax = W.spectral_bounds(g, vloc, True)
+    for nterms in (1, 2, 3, 4, 5, 10):
+        coeffs = rng.standard_normal(nterms)
+        t = torch.from_numpy(psi).cuda()
+        ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+        assert relerr(t.cpu().numpy(), oracle.cheb_filter(g, vloc, kbo, psi, coeffs, emin, emax, ld=True)) < TOL_FULL, nterms
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
+
+
 def test_cfg2_full_length_propagation_invariants(api, torch_cuda):
     """cfg2 at full size and full length (16 vectors, 2000 steps, dt = 0.05): properties that hold at any length.
     With the Hartree term rebuilt every step the propagator stays unitary (norms conserved); with a frozen potential
