@@ -49,8 +49,8 @@ struct AccCfg {
     static constexpr int TABLES = 2 * N * 16 + 3 * N * 8;
     static constexpr int NBOX = N <= 256 ? N : N / 2;        // tensor-map box rows (at most 256 per dimension)
     static constexpr int NOPS = N / NBOX;
-    // consumer groups: bounded by the register file (x[R1] and w[R1] live across the transform: ~160 registers)
-    static constexpr int NG = (GW == 1) ? 8 : (GW == 2 ? 5 : (GW <= 4 ? 2 : 1));
+    // consumer groups: as many as leave each thread ~128-146 registers
+    static constexpr int NG = (GW == 1) ? 8 : (GW == 2 ? 7 : (GW <= 4 ? 3 : 2));
     static constexpr int T = 64 + NG * GT;                   // loader warp, storer warp, consumers
     static constexpr int MAXS = 24;
 };
@@ -75,6 +75,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity) {
         "bra ACC_WAIT;\n"
         "ACC_DONE:\n"
         "}\n" ::"r"(smem_u32(b)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ bool mbar_test(uint64_t* b, unsigned parity) {
+    unsigned ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+    return ok != 0;
 }
 __device__ __forceinline__ void bulk_load(void* dst, const void* src, unsigned bytes, uint64_t* b) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst)), "l"(src),
@@ -104,15 +114,20 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 template <int N>
 struct AccIter {
     static constexpr unsigned TPP = N / 8, TPV = (unsigned)N * N / 8;
-    unsigned t, q, u, period, step;      // u = vector (vector-major) or plane (plane-major), q = offset inside it
+    unsigned t, q, u, period, step, seg; // u = vector (vector-major) or plane (plane-major), q = offset inside it
+    bool hasx;
     int kind;
     unsigned v, p, j;
     __device__ __forceinline__ void init(const AccArgs& a, unsigned t0, unsigned stride) {
         const unsigned nk = (unsigned)((a.kinds & 1) + ((a.kinds >> 1) & 1) + ((a.kinds >> 2) & 1));
-        period = a.plane_major ? nk * TPP : nk * TPV;
+        seg = a.plane_major ? TPP : TPV;
+        hasx = a.kinds & 1;
+        period = nk * seg;
         t = t0; step = stride;
         u = t0 / period; q = t0 - u * period;
     }
+    // x tiles are the first segment of a period when the launch has any
+    __device__ __forceinline__ bool is_x() const { return hasx && q < seg; }
     __device__ __forceinline__ void decode(const AccArgs& a) {
         if (a.plane_major) {
             const unsigned k = q / TPP;
@@ -138,9 +153,12 @@ struct AccIter {
 
 // the round trip of one tile, in place in its slot.  XK: x tile (rows of pitch XP, lanes along the row) or y / z tile
 // (dense [point][pencil], lanes along the pencils).
+//   wtile (x tiles): second slot of the tile.  On entry it holds the v tile (hasv) or nothing; the thread replaces its
+//   elements by w = (c * vtab) * cur + e * v, what the x tiles add besides the transform, and reads them back after the
+//   inverse stage, so that w costs no registers across the transform.
 template <int N, bool XK>
-__device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, const cd* vtile, const double* __restrict__ vt, const cd* twA,
-                                                 const cd* twB, const double* ktab, int gt, int bar_id, uint64_t* vempty, uint64_t* vdone) {
+__device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, cd* wtile, bool hasv, const double* __restrict__ vt, const cd* twA,
+                                                 const cd* twB, const double* ktab, int gt, int bar_id) {
     using C = AccCfg<N>;
     constexpr int R1 = C::R1, R2 = C::R2, TG = C::TG, GW = C::GW, GT = C::GT, TASKS = C::TASKS, ROUNDS = C::ROUNDS, B = C::B;
     constexpr bool WCACHE = R2 <= 8;
@@ -149,22 +167,18 @@ __device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, con
     const int n2 = XK ? gt % R2 : gt / B, bA = XK ? gt / R2 : gt % B;
     cd* eA = tile + bA * SB + n2 * SI;
     cd x[R1];
-    cd w[XK ? R1 : 1];
+    cd* eW = XK ? wtile + bA * SB + n2 * SI : nullptr;
     if (actA) {
 #pragma unroll
         for (int n1 = 0; n1 < R1; ++n1) x[n1] = eA[n1 * R2 * SI];
         if (XK) {
-            // what the x tiles add besides the transform: (c * vtab) * cur + e * v, kept in registers across the transform
             const double c = a.c, e = a.e;
 #pragma unroll
             for (int n1 = 0; n1 < R1; ++n1) {
                 const double cv = vt ? c * __ldg(vt + n1 * R2) : 0.0;
-                w[n1] = make_double2(cv * x[n1].x, cv * x[n1].y);
-            }
-            if (vtile) {
-                const cd* eV = vtile + bA * SB + n2 * SI;
-#pragma unroll
-                for (int n1 = 0; n1 < R1; ++n1) { const cd u = eV[n1 * R2 * SI]; w[n1].x += e * u.x; w[n1].y += e * u.y; }
+                cd w = make_double2(cv * x[n1].x, cv * x[n1].y);
+                if (hasv) { const cd u = eW[n1 * R2 * SI]; w.x += e * u.x; w.y += e * u.y; }
+                eW[n1 * R2 * SI] = w;
             }
         }
         Dft<R1, -1>::run(x);
@@ -178,9 +192,6 @@ __device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, con
         }
     }
     lean_sync<GW>(bar_id);
-    // every thread of the group has read the v tile: its slot is free again (its `done` barrier is advanced too, so
-    // that the phase of every barrier of a slot equals the number of times the slot has been used)
-    if (XK && vtile && gt == 0) { mbar_arrive(vdone); mbar_arrive(vempty); }
 #pragma unroll
     for (int rd = 0; rd < ROUNDS; ++rd) {
         const int task = gt + rd * GT;
@@ -215,7 +226,7 @@ __device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, con
 #pragma unroll
         for (int n1 = 0; n1 < R1; ++n1) {
             cd r = cscale(x[n1], c);
-            if (XK) { r.x += w[n1].x; r.y += w[n1].y; }
+            if (XK) { const cd w = eW[n1 * R2 * SI]; r.x += w.x; r.y += w.y; }
             eA[n1 * R2 * SI] = r;
         }
         fence_proxy_async_smem();                            // the bulk reduce-add reads the slot through the async proxy
@@ -261,11 +272,12 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
             AccIter<N> tl;
             for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next()) {
                 tl.decode(a);
-                const int nops = (tl.kind == 0 && usev) ? 2 : 1;
+                const int nops = tl.kind == 0 ? 2 : 1;          // an x tile takes a second slot: the v tile, then scratch
                 for (int op = 0; op < nops; ++op, ++seq) {
                     const unsigned s = seq % S, round = seq / S;
                     if (round > 0) mbar_wait(empty + s, (round - 1) & 1);
                     char* dst = slots + (size_t)s * TILE;
+                    if (op == 1 && !usev) { mbar_arrive(full + s); continue; }
                     if (tl.kind == 0) {
                         mbar_expect_tx(full + s, B * ROWB);
                         const cd* src = (op == 0 ? a.cur : a.v) + (long long)tl.p * (N * N) + (long long)tl.j * (B * N);
@@ -288,8 +300,17 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
             for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next()) {
                 tl.decode(a);
                 const unsigned s = seq % S, round = seq / S;
-                seq += (tl.kind == 0 && usev) ? 2 : 1;
-                mbar_wait(done + s, round & 1);
+                seq += tl.kind == 0 ? 2 : 1;
+                if (!mbar_test(done + s, round & 1)) {
+                    // about to block: first hand back every slot whose reduce-add has been issued (with few slots the
+                    // loader may need exactly those to bring in the tile this thread waits for)
+                    if (npend) {
+                        bulk_wait_read<0>();
+                        for (unsigned k = 0; k < npend; ++k) mbar_arrive(empty + pend[k]);
+                        npend = 0;
+                    }
+                    mbar_wait(done + s, round & 1);
+                }
                 const char* src = slots + (size_t)s * TILE;
                 if (tl.kind == 0) {
                     cd* dst = a.acc + (long long)tl.p * (N * N) + (long long)tl.j * (B * N);
@@ -319,24 +340,26 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
     unsigned seq = 0, i = 0;
     AccIter<N> tl;
     for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next(), ++i) {
-        tl.decode(a);
+        const bool isx = tl.is_x();
         const unsigned s = seq % S, round = seq / S;
-        const bool xv = tl.kind == 0 && usev;
         const unsigned s2 = (seq + 1) % S, round2 = (seq + 1) / S;
-        seq += xv ? 2 : 1;
+        seq += isx ? 2 : 1;
         if ((int)(i % NG) != grp) continue;
+        tl.decode(a);
         cd* tile = reinterpret_cast<cd*>(slots + (size_t)s * TILE);
         if (tl.kind == 0) {
             const int n2 = gt % C::R2, bA = gt / C::R2;
-            const long long g0 = ((long long)tl.p * (N * N) + (long long)tl.j * (B * N)) % ng;
+            const long long g0 = (long long)(tl.p % (unsigned)a.nz) * (N * N) + (long long)tl.j * (B * N);
             const double* vt = a.vtab ? a.vtab + g0 + bA * N + n2 : nullptr;
             mbar_wait(full + s, round & 1);
-            const cd* vtile = nullptr;
-            if (xv) { mbar_wait(full + s2, round2 & 1); vtile = reinterpret_cast<const cd*>(slots + (size_t)s2 * TILE); }
-            acc_tile_compute<N, true>(a, tile, vtile, vt, twA, twB, ktab, gt, grp, empty + s2, done + s2);
+            mbar_wait(full + s2, round2 & 1);
+            acc_tile_compute<N, true>(a, tile, reinterpret_cast<cd*>(slots + (size_t)s2 * TILE), usev, vt, twA, twB, ktab, gt, grp);
+            // the second slot is free again (its `done` barrier is advanced too: the phase of every barrier of a slot is
+            // the number of times the slot has been used)
+            if (gt == 0) { mbar_arrive(done + s2); mbar_arrive(empty + s2); }
         } else {
             mbar_wait(full + s, round & 1);
-            acc_tile_compute<N, false>(a, tile, nullptr, nullptr, twA, twB, ktab + tl.kind * N, gt, grp, nullptr, nullptr);
+            acc_tile_compute<N, false>(a, tile, nullptr, false, nullptr, twA, twB, ktab + tl.kind * N, gt, grp);
         }
         if (gt == 0) mbar_arrive(done + s);
     }
