@@ -180,16 +180,20 @@ def collect_passes(ctx):
 
 
 def pass_model(passes, nvec, n, kb_frac):
-    """Algorithmic bytes per grid-pt*vector of each profiled launch kind and a display name."""
-    plane_f = "x_store" not in passes            # filter: fused x+y plane pass (no separate x launch)
+    """Algorithmic bytes per grid-pt*vector of each profiled launch kind and a display name.
+    Filter launches: 'y_acc' + 'z_cheb' = accumulate kernel in two launches (planes: w, x, y tiles; then z tiles),
+    'y_acc' alone = accumulate kernel in one launch, 'x_store' present = three register-operand axis passes."""
+    acc2 = "x_store" not in passes and "z_cheb" in passes
+    acc1 = "x_store" not in passes and "z_cheb" not in passes
     plane_t = "x_td" not in passes
     m = {
         "x_store": (48.0 + 16.0 + 8.0 / nvec, f"axis_lean_kernel<{n},8,real,x> (x round trip, potential, recurrence, series every 2nd term)"),
-        "y_acc": ((48.0 + 16.0 + 8.0 / nvec, f"plane_lean/plane_cluster kernel<{n},8,real> (x and y round trips of whole planes)") if plane_f
-                  else (48.0, f"axis_lean_kernel<{n},8,real,y> (y round trip, accumulate)")),
-        "z_cheb": (48.0, f"axis_lean_kernel<{n},8,real,z> (z round trip, accumulate)"),
+        "y_acc": ((64.0 + 8.0 / nvec, f"acc_tma_kernel<{n}> (x and y tiles of whole planes: TMA loads, in-place round trips, bulk reduce-add; Clenshaw v read)") if acc2
+                  else ((64.0 + 8.0 / nvec, f"acc_tma_kernel<{n}> (x, y and z tiles of whole vectors in one launch)") if acc1
+                        else (48.0, f"axis_lean_kernel<{n},8,real,y> (y round trip, accumulate)"))),
+        "z_cheb": (48.0, f"acc_tma_kernel<{n}> (z tiles: TMA tensor loads, bulk reduce-add)" if acc2 else f"axis_lean_kernel<{n},8,real,z> (z round trip, accumulate)"),
         "x_td": (32.0 + 16.0 / nvec, f"axis_lean_kernel<{n},8,complex,x> (x factor of exp(-iT dt), phase on load)"),
-        "y_td": ((32.0 + 16.0 / nvec, f"plane_lean kernel<{n},8,complex> (x and y factors of exp(-iT dt))") if plane_t
+        "y_td": ((32.0 + 16.0 / nvec, f"plane kernel<{n},8,complex> (x and y factors of exp(-iT dt), team- or CTA-owned planes)") if plane_t
                  else (32.0, f"axis_lean_kernel<{n},8,complex,y> (y factor of exp(-iT dt))")),
         "z_td": (32.0 + 16.0 / nvec, f"axis_lean_kernel<{n},8,complex,z> (z factor, phase / density on store)"),
         "kb_project": (16.0 * kb_frac + 32.0 * kb_frac / nvec, "kb_project_kernel<4> (gather-dot over sphere points)"),
@@ -503,7 +507,13 @@ def write_traffic(csv_path, source):
     scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
 
     def key_of(name):
-        fam = "td" if ("true" in name.split("<")[1].split(">")[0].split(",")[2:3] or ", true" in name) and "lean" in name else None
+        if "acc_tma" in name:
+            return "acc"
+        cplx = False
+        if "<" in name:
+            args_ = name.split("<")[1].split(">")[0].replace(" ", "").replace("(bool)", "").replace("(int)", "").split(",")
+            cplx = len(args_) > 2 and args_[2] in ("true", "1")
+        fam = "td" if cplx else None
         if "kb_project" in name:
             return "kb_project"
         if "kb_scatter" in name:
@@ -513,18 +523,20 @@ def write_traffic(csv_path, source):
         if "plane" in name:
             return "y_td" if fam else "y_acc"
         if "axis_lean" in name:
-            args_ = name.split("<")[1].split(">")[0].replace(" ", "").split(",")
             axis = {"0": "x", "1": "y", "2": "z"}[args_[3]]
-            cplx = args_[2] in ("true", "1")
             if cplx:
                 return f"{axis}_td"
             return {"x": "x_store", "y": "y_acc", "z": "z_cheb"}[axis]
         return None
     acc = {}
+    nacc = 0
     for r in rows[2:]:
         k = key_of(r[nm])
         if not k:
             continue
+        if k == "acc":                      # two launches per term: planes (y_acc), then z columns (z_cheb)
+            k = "y_acc" if nacc % 2 == 0 else "z_cheb"
+            nacc += 1
         b = float(r[rd].replace(",", "")) * scale.get(units[rd], 1.0) + float(r[wr].replace(",", "")) * scale.get(units[wr], 1.0)
         e = acc.setdefault(k, {"launches": 0, "bytes": 0.0, "kernel": r[nm][:120]})
         e["launches"] += 1

@@ -27,10 +27,17 @@
  *    nvec > max_nvec are processed in sub-batches of max_nvec (vectors are independent in the
  *    filter; in the TD step the density is accumulated over all sub-batches first).
  *  - Run-time switches, all read ONCE in sgw_init_grid (defaults are the measured best):
+ *      SGW_ACC=0|1           H apply / Chebyshev filter through the TMA accumulate kernel (bulk-tensor loads, in-place
+ *                            round trip in shared memory, bulk reduce-add; cubic grids with N a multiple of 8): default
+ *                            on for N >= 64, else the register-operand passes below
+ *      SGW_ACC_L2_MB=m       accumulate kernel: one launch per term while cur + acc + v of a vector are at most m MB
+ *                            (default 48), else planes (x, y tiles) then z columns in two launches
  *      SGW_LEAN_B=4|8        pencils per tile of the fused passes (default 8 when nx and ny are multiples of 8)
  *      SGW_LEAN_G=n          plane kernel: planes per CTA-owned group (default 1)
  *      SGW_LEAN_CTAS=1|2     plane kernel: one 16-warp or two 8-warp CTAs per SM (default: by L2 footprint)
- *      SGW_LEAN_CLUSTER=0|1  plane kernel: cluster-owned planes off / on (default: on for real 128^2, 256^2 planes)
+ *      SGW_LEAN_CLUSTER=0|1  plane kernel: cluster-owned planes off / on (default: on for real 128^2 planes)
+ *      SGW_LEAN_TEAM=0|1     plane kernel: team-owned planes (arrival counter per plane) off / on (default: on from 256^2)
+ *      SGW_LEAN_VMINOR=0|1   tile order runs over the vectors first (default: when an N_g table exceeds 24 MB)
  *      SGW_LEAN_CHUNK=n      filter: n vectors at a time through all terms (default: all vectors per term)
  *      SGW_L2_CHUNK=n        propagation: n vectors at a time through a step (default: all vectors)
  *      SGW_PDL=1             programmatic dependent launch of the passes (default off)

@@ -53,6 +53,10 @@ struct AccCfg {
     static constexpr int NG = (GW == 1) ? 8 : (GW == 2 ? 7 : (GW <= 4 ? 3 : 2));
     static constexpr int T = 64 + NG * GT;                   // loader warp, storer warp, consumers
     static constexpr int MAXS = 24;
+    // x tiles: the pointwise part w = (c vtab) cur + e v either goes through a second slot of the tile (v is brought in
+    // by the loader) or, where a slot is too precious (few, large slots), is read from global memory after the inverse
+    // stage (cur is an L2 hit then)
+    static constexpr bool LATEW = N > 256;
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -158,7 +162,8 @@ struct AccIter {
 //   inverse stage, so that w costs no registers across the transform.
 template <int N, bool XK>
 __device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, cd* wtile, bool hasv, const double* __restrict__ vt, const cd* twA,
-                                                 const cd* twB, const double* ktab, int gt, int bar_id) {
+                                                 const cd* twB, const double* ktab, int gt, int bar_id, const cd* __restrict__ gcur = nullptr,
+                                                 const cd* __restrict__ gv = nullptr) {
     using C = AccCfg<N>;
     constexpr int R1 = C::R1, R2 = C::R2, TG = C::TG, GW = C::GW, GT = C::GT, TASKS = C::TASKS, ROUNDS = C::ROUNDS, B = C::B;
     constexpr bool WCACHE = R2 <= 8;
@@ -167,11 +172,12 @@ __device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, cd*
     const int n2 = XK ? gt % R2 : gt / B, bA = XK ? gt / R2 : gt % B;
     cd* eA = tile + bA * SB + n2 * SI;
     cd x[R1];
-    cd* eW = XK ? wtile + bA * SB + n2 * SI : nullptr;
+    constexpr bool LATEW = C::LATEW;
+    cd* eW = (XK && !LATEW) ? wtile + bA * SB + n2 * SI : nullptr;
     if (actA) {
 #pragma unroll
         for (int n1 = 0; n1 < R1; ++n1) x[n1] = eA[n1 * R2 * SI];
-        if (XK) {
+        if (XK && !LATEW) {
             const double c = a.c, e = a.e;
 #pragma unroll
             for (int n1 = 0; n1 < R1; ++n1) {
@@ -223,11 +229,34 @@ __device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, cd*
         for (int j = 0; j < R1; ++j) x[j] = eA[j * R2 * SI];
         Dft<R1, +1>::run(x);
         const double c = a.c;
+        if (XK && LATEW) {
+            const double e = a.e;
+            constexpr int CH = (R1 % 4 == 0) ? 4 : ((R1 % 3 == 0) ? 3 : 1);
 #pragma unroll
-        for (int n1 = 0; n1 < R1; ++n1) {
-            cd r = cscale(x[n1], c);
-            if (XK) { const cd w = eW[n1 * R2 * SI]; r.x += w.x; r.y += w.y; }
-            eA[n1 * R2 * SI] = r;
+            for (int c0 = 0; c0 < R1; c0 += CH) {
+                cd cu[CH], vv[CH];
+                double tv[CH];
+#pragma unroll
+                for (int q = 0; q < CH; ++q) {
+                    const int o = (c0 + q) * R2;
+                    tv[q] = vt ? __ldg(vt + o) : 0.0;
+                    cu[q] = vt ? __ldg(gcur + o) : make_double2(0.0, 0.0);
+                    vv[q] = hasv ? __ldg(gv + o) : make_double2(0.0, 0.0);
+                }
+#pragma unroll
+                for (int q = 0; q < CH; ++q) {
+                    const int n1 = c0 + q;
+                    const double cv = c * tv[q];
+                    eA[n1 * R2 * SI] = make_double2(c * x[n1].x + cv * cu[q].x + e * vv[q].x, c * x[n1].y + cv * cu[q].y + e * vv[q].y);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int n1 = 0; n1 < R1; ++n1) {
+                cd r = cscale(x[n1], c);
+                if (XK) { const cd w = eW[n1 * R2 * SI]; r.x += w.x; r.y += w.y; }
+                eA[n1 * R2 * SI] = r;
+            }
         }
         fence_proxy_async_smem();                            // the bulk reduce-add reads the slot through the async proxy
     }
@@ -272,7 +301,7 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
             AccIter<N> tl;
             for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next()) {
                 tl.decode(a);
-                const int nops = tl.kind == 0 ? 2 : 1;          // an x tile takes a second slot: the v tile, then scratch
+                const int nops = (tl.kind == 0 && !C::LATEW) ? 2 : 1;   // an x tile takes a second slot: the v tile, then scratch
                 for (int op = 0; op < nops; ++op, ++seq) {
                     const unsigned s = seq % S, round = seq / S;
                     if (round > 0) mbar_wait(empty + s, (round - 1) & 1);
@@ -300,7 +329,7 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
             for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next()) {
                 tl.decode(a);
                 const unsigned s = seq % S, round = seq / S;
-                seq += tl.kind == 0 ? 2 : 1;
+                seq += (tl.kind == 0 && !C::LATEW) ? 2 : 1;
                 if (!mbar_test(done + s, round & 1)) {
                     // about to block: first hand back every slot whose reduce-add has been issued (with few slots the
                     // loader may need exactly those to bring in the tile this thread waits for)
@@ -340,7 +369,7 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
     unsigned seq = 0, i = 0;
     AccIter<N> tl;
     for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next(), ++i) {
-        const bool isx = tl.is_x();
+        const bool isx = !C::LATEW && tl.is_x();
         const unsigned s = seq % S, round = seq / S;
         const unsigned s2 = (seq + 1) % S, round2 = (seq + 1) / S;
         seq += isx ? 2 : 1;
@@ -352,11 +381,16 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
             const long long g0 = (long long)(tl.p % (unsigned)a.nz) * (N * N) + (long long)tl.j * (B * N);
             const double* vt = a.vtab ? a.vtab + g0 + bA * N + n2 : nullptr;
             mbar_wait(full + s, round & 1);
-            mbar_wait(full + s2, round2 & 1);
-            acc_tile_compute<N, true>(a, tile, reinterpret_cast<cd*>(slots + (size_t)s2 * TILE), usev, vt, twA, twB, ktab, gt, grp);
-            // the second slot is free again (its `done` barrier is advanced too: the phase of every barrier of a slot is
-            // the number of times the slot has been used)
-            if (gt == 0) { mbar_arrive(done + s2); mbar_arrive(empty + s2); }
+            if (C::LATEW) {
+                const long long o = (long long)tl.p * (N * N) + (long long)tl.j * (B * N) + bA * N + n2;
+                acc_tile_compute<N, true>(a, tile, nullptr, usev, vt, twA, twB, ktab, gt, grp, a.cur + o, usev ? a.v + o : nullptr);
+            } else {
+                mbar_wait(full + s2, round2 & 1);
+                acc_tile_compute<N, true>(a, tile, reinterpret_cast<cd*>(slots + (size_t)s2 * TILE), usev, vt, twA, twB, ktab, gt, grp);
+                // the second slot is free again (its `done` barrier is advanced too: the phase of every barrier of a slot
+                // is the number of times the slot has been used)
+                if (gt == 0) { mbar_arrive(done + s2); mbar_arrive(empty + s2); }
+            }
         } else {
             mbar_wait(full + s, round & 1);
             acc_tile_compute<N, false>(a, tile, nullptr, false, nullptr, twA, twB, ktab + tl.kind * N, gt, grp);

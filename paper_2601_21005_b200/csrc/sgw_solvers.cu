@@ -20,11 +20,12 @@ inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) /
     } while (0)
 
 // the real family (H apply, Chebyshev filter) runs through the TMA accumulate kernel where it is built (cubic grids,
-// axis length a multiple of 8) and enabled (SGW_ACC=0/1; default: on for 64..128 points per axis)
+// axis length a multiple of 8) and enabled (SGW_ACC=0/1; default: on from 64 points per axis; smaller grids are
+// launch-bound and keep the register-operand passes with their cached graph)
 bool acc_enabled(const sgw_ctx* c) {
     if (!c->acc) return false;
     if (c->use_acc >= 0) return c->use_acc != 0;
-    return c->nx >= 64 && c->nx <= 128;
+    return c->nx >= 64;
 }
 
 int launched(sgw_ctx* c, const char* what) {
