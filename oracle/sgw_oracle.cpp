@@ -130,6 +130,16 @@ void kvals(int N, double h, std::vector<T>& k) {
 }
 
 struct Grid { int nx, ny, nz; double hx, hy, hz; };
+
+// Kinetic-energy cutoff ("apply an energy cutoff of 28 Hartrees to the kinetic energy operator"; a cutoff
+// bounds the spectral width and with it N_chb; R-14): when g_ecut > 0 the kinetic operator is diagonal in k
+// with values min(1/2 |k|^2, E_cut) instead of 1/2 |k|^2, in H and in the propagator.  0 = no cutoff (the configs).
+double g_ecut = 0.0;
+template <class T>
+inline T kinetic(T k2) {
+    const T t = (T)0.5 * k2;
+    return (g_ecut > 0.0 && t > (T)g_ecut) ? (T)g_ecut : t;
+}
 struct KBList {
     int nsphere, nproj;
     const int64_t* ptr; const int32_t* idx; const double* beta; const double* D;
@@ -149,7 +159,7 @@ void apply_H_one(const Grid& g, const double* vloc, const KBList& kb, const C<T>
         for (int iy = 0; iy < g.ny; ++iy)
             for (int ix = 0; ix < g.nx; ++ix) {
                 T k2 = kx[ix] * kx[ix] + ky[iy] * ky[iy] + kz[iz] * kz[iz];
-                t[ix + (size_t)g.nx * (iy + (size_t)g.ny * iz)] *= (T)0.5 * k2;
+                t[ix + (size_t)g.nx * (iy + (size_t)g.ny * iz)] *= kinetic<T>(k2);
             }
     fft3<T>(g.nx, g.ny, g.nz, +1, t.data());
     const T inv = (T)1 / (T)ng;
@@ -309,7 +319,7 @@ void td_batch(const Grid& g, const double* vloc, const KBList& kb, int nvec, dou
             for (int iz = 0; iz < g.nz; ++iz)
                 for (int iy = 0; iy < g.ny; ++iy)
                     for (int ix = 0; ix < g.nx; ++ix) {
-                        T ph = (T)0.5 * (kx[ix] * kx[ix] + ky[iy] * ky[iy] + kz[iz] * kz[iz]) * (T)dt;
+                        T ph = kinetic<T>(kx[ix] * kx[ix] + ky[iy] * ky[iy] + kz[iz] * kz[iz]) * (T)dt;
                         a[ix + (size_t)g.nx * (iy + (size_t)g.ny * iz)] *= C<T>(std::cos(ph), -std::sin(ph));
                     }
             fft3<T>(g.nx, g.ny, g.nz, +1, a.data());
@@ -368,6 +378,7 @@ void spectral_bounds(const Grid& g, const double* vloc, const KBList& kb, int ni
 }
 
 extern "C" {
+void sgwo_set_kinetic_cutoff(double ecut) { g_ecut = ecut > 0.0 ? ecut : 0.0; }
 
 uint64_t sgwo_splitmix64_next(uint64_t* state) {   // the standard generator: state += gamma; mix
     uint64_t s = *state;

@@ -60,6 +60,11 @@ def _vec(a):
     return np.ascontiguousarray(a, dtype=np.complex128)
 
 
+def set_kinetic_cutoff(ecut: float):
+    """Kinetic operator min(1/2 k^2, ecut) in H and the propagator (0 = off, the default)."""
+    lib().sgwo_set_kinetic_cutoff(C.c_double(ecut))
+
+
 def set_threads(n: int):
     lib().sgwo_set_threads(C.c_int(n))
 

@@ -21,11 +21,13 @@ def kgrid(g):
     return kx, ky, kz
 
 
-def dense_H(g, vloc, kb):
+def dense_H(g, vloc, kb, ecut=0.0):
     """H as a dense matrix, built with numpy.fft and outer products (independent of the oracle)."""
     ng = g.ng
     kx, ky, kz = kgrid(g)
     k2 = 0.5 * (kx ** 2 + ky ** 2 + kz ** 2)
+    if ecut > 0:
+        k2 = np.minimum(k2, ecut)
     eye = np.eye(ng, dtype=np.complex128).reshape((ng,) + g.shape)
     T = np.fft.ifftn(k2[None] * np.fft.fftn(eye, axes=(1, 2, 3)), axes=(1, 2, 3)).reshape(ng, ng).T
     H = T + np.diag(vloc.ravel())
@@ -363,3 +365,53 @@ def test_power_iteration_bounds_converge_to_dense_extreme_eigenvalues(oracle):
     a = oracle.spectral_bounds(g, vloc, kb, 50, 99)
     b = oracle.spectral_bounds(g, vloc, kb, 50, 99, ld=True)
     assert np.allclose(a, b, rtol=1e-12, atol=1e-12)
+
+
+# ------------------------------------------------------------------ NEXT-3: kinetic-energy cutoff
+def test_kinetic_cutoff_plane_waves_dense_matrix_spectrum_and_propagator(oracle):
+    """With the cutoff the kinetic operator is min(1/2 k^2, E_cut), diagonal in k ("an energy cutoff ... to the
+    kinetic energy operator"): closed-form eigenvalues for plane waves below and above the cutoff, a dense matrix built
+    here with numpy, the spectrum bounded by E_cut + max V (the point of the cutoff), and the V = 0 propagator
+    exp(-i min(1/2 k^2, E_cut) t) in closed form."""
+    ecut = 6.0
+    g = W.Grid(8, 6, 12, 0.5, 0.6, 0.45)
+    z, y, x = np.meshgrid(np.arange(g.nz), np.arange(g.ny), np.arange(g.nx), indexing="ij")
+    try:
+        oracle.set_kinetic_cutoff(ecut)
+        seen_above = seen_below = False
+        for (mx, my, mz) in [(0, 0, 0), (1, 0, 0), (1, -2, 3), (-4, 3, -6), (3, 2, 5), (0, -3, 0)]:
+            k = 2 * np.pi * np.array([mx / (g.nx * g.hx), my / (g.ny * g.hy), mz / (g.nz * g.hz)])
+            e = min(0.5 * float(k @ k), ecut)
+            seen_above |= 0.5 * float(k @ k) > ecut
+            seen_below |= 0.5 * float(k @ k) < ecut
+            pw = np.exp(2j * np.pi * (mx * x / g.nx + my * y / g.ny + mz * z / g.nz))[None]
+            for ld in (False, True):
+                out = oracle.apply_H(g, np.full(g.shape, 0.3), None, pw, ld=ld)
+                assert np.max(np.abs(out - (e + 0.3) * pw)) < 1e-11
+            t = 0.7
+            prop = oracle.td_propagate(g, None, None, pw, t / 7, 7, 0, 0.0, ld=True)
+            assert np.max(np.abs(prop - np.exp(-1j * e * t) * pw)) < 1e-11
+        assert seen_above and seen_below
+        g2, vloc, kb, rng = small_problem(8, 0.7, True)
+        H = dense_H(g2, vloc, kb, ecut=ecut)
+        psi = rvec(rng, g2, 2)
+        want = (H @ psi.reshape(2, -1).T).T.reshape(psi.shape)
+        assert np.max(np.abs(oracle.apply_H(g2, vloc, kb, psi, ld=True) - want)) < 1e-11
+        ev = np.linalg.eigvalsh(H)
+        assert ev[-1] <= ecut + vloc.max() + np.abs(kb.D).max() * 1.01 + 1e-9
+        assert np.linalg.eigvalsh(dense_H(g2, vloc, kb))[-1] > ev[-1] + 5.0      # the cutoff did shrink the spectrum
+        # a filter on the narrower window: polynomial of the cut-off H by dense diagonalisation
+        emin, emax = ev[0] - 0.5, ev[-1] + 0.5
+        co = rng.standard_normal(12)
+        w_, U = np.linalg.eigh(H)
+        xs = (w_ - 0.5 * (emax + emin)) / (0.5 * (emax - emin))
+        pol = np.polynomial.chebyshev.chebval(xs, co)
+        want = ((U * pol) @ (U.conj().T @ psi.reshape(2, -1).T)).T.reshape(psi.shape)
+        got = oracle.cheb_filter(g2, vloc, kb, psi, co, emin, emax, ld=True)
+        assert np.max(np.abs(got - want)) < 1e-10
+    finally:
+        oracle.set_kinetic_cutoff(0.0)
+    # and off again: the plain operator
+    pw = np.exp(2j * np.pi * (3 * x / g.nx))[None]
+    k = 2 * np.pi * 3 / (g.nx * g.hx)
+    assert np.max(np.abs(oracle.apply_H(g, None, None, pw, ld=True) - 0.5 * k * k * pw)) < 1e-11
