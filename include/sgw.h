@@ -15,7 +15,7 @@
  *    [nvec][nz][ny][nx] with x fastest; flat grid index g = ix + nx*(iy + ny*iz) (packed
  *    (N_g x n) multi-index arrays).  Real fields (V_loc, rho, V_H) are [nz][ny][nx] doubles.
  *  - All work is enqueued on the CUDA stream given to sgw_init_grid and is asynchronous with respect to the
- *    host.  The calls that block the host are: sgw_init_grid, sgw_set_vloc, sgw_set_nonlocal, sgw_destroy (setup;
+ *    host.  The calls that block the host are: sgw_init_grid, sgw_set_vloc, sgw_set_nonlocal, sgw_set_kinetic_cutoff, sgw_destroy (setup;
  *    they allocate and synchronise the stream), sgw_sync_check, sgw_profile_get / _reset / _enable(0),
  *    sgw_spectral_bounds and sgw_probe_fp64 (they return host values), the FIRST sgw_cheb_filter / sgw_spectral_bounds call on a context
  *    (it allocates the two workspace arrays of max_nvec vectors: cudaMalloc), and error paths.  sgw_random_vectors,
@@ -125,6 +125,14 @@ int sgw_set_td(sgw_ctx* ctx, int hartree_mode, double rho_scale);
  * NL(tau) psi = psi + sum_{s,p} beta_sp (e^{-i D_sp tau} - 1) dV <beta_sp|psi>.
  * dt may be negative (reverse-time propagation). */
 int sgw_td_propagate(sgw_ctx* ctx, int nvec, void* d_psi, double dt, int nsteps);
+
+/* Kinetic-energy cutoff ("apply an energy cutoff of 28 Hartrees to the kinetic energy operator"; it bounds
+ * the spectral width and with it the number of Chebyshev terms; R-14).  ecut > 0 (Ha): from now on the kinetic operator
+ * of sgw_apply_H, sgw_cheb_filter, sgw_td_propagate and sgw_spectral_bounds is F^-1 min(1/2 |k|^2, ecut) F.  That
+ * operator is not separable, so these calls then take a five-pass full-3D-transform route (about 7 array sweeps per
+ * application instead of 2-3).  ecut <= 0 restores the plain 1/2 |k|^2 (the default, and what BASELINE.json's configs
+ * use).  Setup call: allocates N_g doubles + N_g complex + max_nvec vectors of scratch and synchronises the stream. */
+int sgw_set_kinetic_cutoff(sgw_ctx* ctx, double ecut);
 
 /* Spectral bounds of H by shifted power iteration ("the upper and lower spectral bounds of the Kohn-Sham
  * Hamiltonian ... a shifted power iteration"; R-20).  power(shift, x0): x = x0/|x0|; niter times: y = H x - shift x,

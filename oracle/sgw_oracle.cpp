@@ -331,6 +331,56 @@ void td_batch(const Grid& g, const double* vloc, const KBList& kb, int nvec, dou
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// NEXT-2: perturbed / unperturbed pair propagation and the sparse stochastic projection of the retarded response
+// ("create a perturbed copy of each eta (eta^lambda) and propagate both perturbed and unperturbed copies in time
+// under the action of the time-dependent Hamiltonian ... accumulate the causal response function u^R(r,t) as the
+// difference of the perturbed and unperturbed time-dependent potentials"; "projecting u^R(r,t) onto a set of N_xi
+// randomly chosen functions xi on short, fragmented segments of the spatial grid"; "(N_xi x N_g f_g) and
+// (N_g f_g x 2) ... each xi function is processed in segments of length L = 32").  Readings R-21..R-23:
+//   * the caller supplies both copies (the perturbed one is exp(-i lambda v_pert(r)) eta, sgwo_apply_kick);
+//   * each copy is propagated with the split-operator step of td_batch under ITS OWN Hartree potential
+//     V_loc + V_H[rho_copy(t_n)];
+//   * xi_m (m < nxi) lives on nfrag fragments of L = 32 consecutive grid points; fragment f starts at grid index
+//     32 * (h(seed, 2m, f) mod (N_g / 32)) and carries the signs (top bit of h(seed, 2m+1, 32 f + j) ? -1 : +1);
+//   * at the start of step n: out[n][m][copy] = dV * sum_{f,j} sign * V_H[rho_copy(t_n)](point), copy 0 = unperturbed,
+//     1 = perturbed; the coefficients of u^R are (out[..][1] - out[..][0]) / lambda.
+// ---------------------------------------------------------------------------------------------
+constexpr int XI_L = 32;
+
+template <class T>
+void xi_project(const Grid& g, const std::vector<T>& field, uint64_t seed, int nxi, int nfrag, double* out, int stride) {
+    const size_t ng = (size_t)g.nx * g.ny * g.nz;
+    const uint64_t nblocks = ng / XI_L;
+    const T dV = (T)g.hx * (T)g.hy * (T)g.hz;
+    for (int m = 0; m < nxi; ++m) {
+        T acc = 0;
+        for (int f = 0; f < nfrag; ++f) {
+            const uint64_t b = keyed_hash(seed, 2 * (uint64_t)m, (uint64_t)f) % nblocks;
+            for (int j = 0; j < XI_L; ++j) {
+                const T sg = (keyed_hash(seed, 2 * (uint64_t)m + 1, (uint64_t)f * XI_L + j) >> 63) ? (T)-1 : (T)1;
+                acc += sg * field[b * XI_L + j];
+            }
+        }
+        out[(size_t)m * stride] = (double)(acc * dV);
+    }
+}
+
+template <class T>
+void td_pair(const Grid& g, const double* vloc, const KBList& kb, int nvec, double* psi, double* psi_lam, double dt, int nsteps,
+             double rho_scale, uint64_t xi_seed, int nxi, int nfrag, double* out) {
+    std::vector<T> rho, vh;
+    for (int n = 0; n < nsteps; ++n) {
+        for (int copy = 0; copy < 2; ++copy) {
+            density<T>(g, nvec, copy ? psi_lam : psi, rho_scale, rho);
+            poisson<T>(g, rho, vh);
+            xi_project<T>(g, vh, xi_seed, nxi, nfrag, out + ((size_t)n * nxi) * 2 + copy, 2);
+        }
+        td_batch<T>(g, vloc, kb, nvec, psi, dt, 1, 1, rho_scale);
+        td_batch<T>(g, vloc, kb, nvec, psi_lam, dt, 1, 1, rho_scale);
+    }
+}
+
 }  // namespace
 
 // =============================================================================================
@@ -473,6 +523,25 @@ void sgwo_td_propagate(GRID_ARGS, const double* vloc, KB_ARGS, int nvec, double*
     MK
     if (use_ld) td_batch<long double>(g, vloc, kb, nvec, psi, dt, nsteps, hartree_mode, rho_scale);
     else td_batch<double>(g, vloc, kb, nvec, psi, dt, nsteps, hartree_mode, rho_scale);
+}
+
+// psi <- exp(-i lambda v_pert(r)) psi for nvec vectors (the perturbed copy of P:57; R-21)
+void sgwo_apply_kick(int64_t ng, int nvec, double* psi, const double* vpert, double lambda) {
+    for (int v = 0; v < nvec; ++v)
+        for (int64_t i = 0; i < ng; ++i) {
+            const long double ph = (long double)lambda * (long double)vpert[i];
+            const std::complex<long double> z((long double)psi[2 * (ng * v + i)], (long double)psi[2 * (ng * v + i) + 1]);
+            const std::complex<long double> r = z * std::complex<long double>(std::cos(ph), -std::sin(ph));
+            psi[2 * (ng * v + i)] = (double)r.real();
+            psi[2 * (ng * v + i) + 1] = (double)r.imag();
+        }
+}
+
+void sgwo_td_pair(GRID_ARGS, const double* vloc, KB_ARGS, int nvec, double* psi, double* psi_lam, double dt, int nsteps,
+                  double rho_scale, uint64_t xi_seed, int nxi, int nfrag, double* out, int use_ld) {
+    MK
+    if (use_ld) td_pair<long double>(g, vloc, kb, nvec, psi, psi_lam, dt, nsteps, rho_scale, xi_seed, nxi, nfrag, out);
+    else td_pair<double>(g, vloc, kb, nvec, psi, psi_lam, dt, nsteps, rho_scale, xi_seed, nxi, nfrag, out);
 }
 
 void sgwo_spectral_bounds(GRID_ARGS, const double* vloc, KB_ARGS, int niter, uint64_t seed, double* emin, double* emax,

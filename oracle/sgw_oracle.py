@@ -163,3 +163,23 @@ def norms(psi):
     ng = psi[0].size
     lib().sgwo_norms(C.c_int64(ng), C.c_int(psi.shape[0]), _p(psi), _p(out))
     return out
+
+
+def apply_kick(psi, vpert, lam):
+    """Perturbed copy exp(-i lam v_pert) psi (R-21)."""
+    psi = _vec(psi).copy()
+    vp = np.ascontiguousarray(vpert, np.float64)
+    lib().sgwo_apply_kick(C.c_int64(psi[0].size), C.c_int(psi.shape[0]), _p(psi), _p(vp), C.c_double(lam))
+    return psi
+
+
+def td_pair(grid, vloc, kb, psi, psi_lam, dt, nsteps, rho_scale, xi_seed, nxi, nfrag, ld: bool = False):
+    """Pair propagation with the xi projections of both Hartree potentials at the start of every step
+    (R-21..R-23).  Returns (psi, psi_lam, out[nsteps, nxi, 2])."""
+    a, b = _vec(psi).copy(), _vec(psi_lam).copy()
+    kba, keep = _kb_args(kb)
+    v = None if vloc is None else np.ascontiguousarray(vloc, np.float64)
+    out = np.zeros((nsteps, nxi, 2), np.float64)
+    lib().sgwo_td_pair(*_grid_args(grid), _p(v), *kba, C.c_int(a.shape[0]), _p(a), _p(b), C.c_double(dt), C.c_int(nsteps),
+                       C.c_double(rho_scale), C.c_uint64(xi_seed), C.c_int(nxi), C.c_int(nfrag), _p(out), C.c_int(int(ld)))
+    return a, b, out

@@ -20,7 +20,7 @@ ERRORS = {-1: "SGW_EINVAL", -2: "SGW_ESIZE", -3: "SGW_ENOMEM", -4: "SGW_ECUDA"}
 EXPORTS = ["sgw_init_grid", "sgw_destroy", "sgw_set_vloc", "sgw_set_nonlocal", "sgw_random_vectors",
            "sgw_apply_H", "sgw_cheb_filter", "sgw_hartree", "sgw_set_td", "sgw_td_propagate", "sgw_norms",
            "sgw_launch_count", "sgw_last_error", "sgw_sync_check", "sgw_spectral_bounds", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get",
-           "sgw_probe_fp64"]
+           "sgw_probe_fp64", "sgw_set_kinetic_cutoff"]
 
 
 class SGWError(RuntimeError):
@@ -57,6 +57,7 @@ def load():
         lib.sgw_profile_reset.argtypes = [vp]
         lib.sgw_profile_get.argtypes = [vp, i, i, C.POINTER(i64), C.POINTER(d)]
         lib.sgw_probe_fp64.argtypes = [vp, C.POINTER(d)]
+        lib.sgw_set_kinetic_cutoff.argtypes = [vp, d]
         _lib = lib
     return _lib
 
@@ -176,6 +177,9 @@ class Context:
         n, ms = C.c_int64(), C.c_double()
         _check(self.lib.sgw_profile_get(self._h, axis, kind, C.byref(n), C.byref(ms)))
         return n.value, ms.value
+
+    def sgw_set_kinetic_cutoff(self, ecut):
+        _check(self.lib.sgw_set_kinetic_cutoff(self._h, float(ecut)))
 
     def sgw_probe_fp64(self):
         r = C.c_double()

@@ -92,11 +92,11 @@ PassGeom geom_for_axis(const sgw_ctx* c, int axis, int nvec, long long* ntiles) 
     return g;
 }
 
-int run_pass(sgw_ctx* c, int axis, int kind, int variant, const cd* in, const OpParams& p) {
+int run_pass(sgw_ctx* c, int axis, int kind, int variant, const cd* in, const OpParams& p, int nvec) {
     PassCall call;
     call.kind = kind;
     call.variant = variant;
-    call.gm = geom_for_axis(c, axis, 1, &call.ntiles);
+    call.gm = geom_for_axis(c, axis, nvec, &call.ntiles);
     call.in = in;
     call.tw = c->tw[axis];
     call.p = p;
@@ -205,7 +205,7 @@ extern "C" int sgw_destroy(sgw_ctx* c) {
     cudaFree(c->ws[0]); cudaFree(c->ws[1]);
     cudaFree(c->vloc); cudaFree(c->vtab); cudaFree(c->vk3d); cudaFree(c->sph_ptr); cudaFree(c->sph_idx);
     cudaFree(c->beta); cudaFree(c->D); cudaFree(c->kbc); cudaFree(c->pois); cudaFree(c->rho); cudaFree(c->vh);
-    cudaFree(c->phase); cudaFree(c->phase_last); cudaFree(c->vprev); cudaFree(c->red); cudaFree(c->team_cnt);
+    cudaFree(c->phase); cudaFree(c->phase_last); cudaFree(c->vprev); cudaFree(c->red); cudaFree(c->team_cnt); cudaFree(c->kin3d); cudaFree(c->td_kin3d); cudaFree(c->wcut);
     delete c;
     return SGW_OK;
 }

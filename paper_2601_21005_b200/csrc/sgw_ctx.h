@@ -66,6 +66,13 @@ struct sgw_ctx {
     sgw::cd* phase;                          // exp(-i V dt/2), N_g (merged table of two half steps without KB)
     sgw::cd* phase_last;                     // closing exp(-i V dt/2) of the last step of a call
     double* vprev;                           // total potential of the previous step
+    // kinetic-energy cutoff (sgw_set_kinetic_cutoff): non-separable kinetic operator min(1/2 k^2, E_cut)
+    double ecut;                             // 0 = off
+    double* kin3d;                           // min(1/2 |k|^2, E_cut) / N_g on the grid's k layout
+    sgw::cd* td_kin3d;                       // exp(-i min(1/2 |k|^2, E_cut) dt) / N_g (rebuilt when dt changes)
+    double td3d_dt;
+    bool td3d_valid;
+    sgw::cd* wcut;                           // max_nvec vectors of scratch for the five-pass route
     double* red;                             // 4 doubles: reductions of sgw_spectral_bounds
     int hartree_mode;
     double rho_scale;
@@ -92,7 +99,11 @@ int set_error(int code, const std::string& msg);
 int check_cuda(cudaError_t e, const char* what);
 PassGeom geom_for_axis(const sgw_ctx* c, int axis, int nvec, long long* ntiles);
 // one Poisson pass on a single N_g array (variant: see PassCall)
-int run_pass(sgw_ctx* c, int axis, int kind, int variant, const cd* in, const OpParams& p);
+int run_pass(sgw_ctx* c, int axis, int kind, int variant, const cd* in, const OpParams& p, int nvec = 1);
+// non-separable kinetic operator (sgw_cut.cu)
+int cut_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out);
+int cut_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* h_coeffs, double s, int nterms);
+int cut_td_propagate(sgw_ctx* c, int nvec, cd* psi, double dt, int nsteps);
 // lean-pass implementations (sgw_program.cu)
 int lean_apply_H(sgw_ctx* c, int nv, const cd* in, cd* out);
 int lean_cheb_filter(sgw_ctx* c, int nvec, cd* psi, const double* h_coeffs, double s, int nterms);

@@ -144,7 +144,7 @@ struct PassGeom {
 enum { MODE_RT = 0, MODE_FWD = 1, MODE_INV = 2 };
 
 // One CTA = B pencils of length N.  Op supplies (sgw_ops.cuh):
-//   cd   load(const cd* in, long long off)                  input element
+//   cd   load(const cd* in, long long off, long long g)     input element (off: in the vector arrays, g: on the grid)
 //   cd   mult(cd X, int k, long long gk)                    k-space multiply (RT only)
 //   void epi(cd r, long long off, long long g)              store
 template <int N, int MODE, class Op>
@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(256) pass_kernel(PassGeom gm, const cd* __rest
 #pragma unroll
             for (int n1 = 0; n1 < R1; ++n1) {
                 const long long o = (long long)(n1 * R2 + n2) * gm.sN + (long long)bA * gm.sB;
-                x[n1] = op.load(in, base + o);
+                x[n1] = op.load(in, base + o, g0 + o);
             }
             Dft<R1, -1>::run(x);
 #pragma unroll
@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(256) pass_kernel(PassGeom gm, const cd* __rest
 #pragma unroll
                 for (int k2 = 0; k2 < R2; ++k2) {
                     const long long o = (long long)(k1 + R1 * k2) * gm.sN + (long long)bB * gm.sB;
-                    y[k2] = op.load(in, base + o);
+                    y[k2] = op.load(in, base + o, g0 + o);
                 }
             }
             Dft<R2, +1>::run(y);

@@ -34,11 +34,19 @@ struct OpParams {
     double* vh_out;          // Re(result) or NULL
     double half_dt;
     int first;
+    // non-separable kinetic operator (sgw_set_kinetic_cutoff): passes over nvec vectors
+    const cd* src;           // the operator's input vectors (epilogues that add V * src)
+    cd* acc;                 // Chebyshev: phi_{n-1} in, phi_{n+1} out
+    const double* vtab;      // N_g real table multiplying src in the epilogue
+    const cd* phase;         // N_g complex table applied on load (K_FWD variant 3) or on store (K_INV variant 5)
+    const cd* mul3c;         // complex N_g k-space table
+    double kscale, hs, alpha;
 };
 
 struct PassCall {
     int kind;                // PassKind
-    int variant;             // K_FWD: 1 = real input (rin);  K_INV: 1 = merged phase epilogue, 2 = real output (vh_out)
+    int variant;             // K_FWD: 1 = real input (rin), 3 = phase on load;  K_RT_MUL3D: 1 = complex table;
+                             // K_INV: 1 = merged phase epilogue, 2 = real output (vh_out), 3 = + vtab * src, 4 = Chebyshev step, 5 = phase on store
     PassGeom gm;
     long long ntiles;
     const cd* in;
@@ -50,18 +58,18 @@ struct PassCall {
 typedef int (*pass_launch_fn)(const PassCall*);
 
 // ---- functors -------------------------------------------------------------------------------
-//   cd   load(const cd* in, long long off)                  input element
+//   cd   load(const cd* in, long long off, long long g)     input element
 //   cd   mult(cd X, int k, long long gk)                    k-space multiply (RT only)
 //   void epi(cd r, long long off, long long g)              store
 struct OpStore {
     OpParams p;
-    __device__ __forceinline__ cd load(const cd* in, long long off) const { return in[off]; }
+    __device__ __forceinline__ cd load(const cd* in, long long off, long long) const { return in[off]; }
     __device__ __forceinline__ cd mult(cd X, int, long long) const { return X; }
     __device__ __forceinline__ void epi(cd r, long long off, long long) const { p.out[off] = r; }
 };
 // forward pass straight from the real density (replaces a separate real -> complex copy)
 struct OpFromReal : OpStore {
-    __device__ __forceinline__ cd load(const cd*, long long off) const { return make_double2(p.rin[off], 0.0); }
+    __device__ __forceinline__ cd load(const cd*, long long off, long long) const { return make_double2(p.rin[off], 0.0); }
 };
 struct OpMul3D : OpStore {
     __device__ __forceinline__ cd mult(cd X, int, long long gk) const { return cscale(X, __ldg(p.mul3d + gk)); }
@@ -85,6 +93,36 @@ struct OpPhaseMerge : OpStore {
         }
         if (p.rho_reset) p.rho_reset[off] = 0.0;
     }
+};
+
+// ---- non-separable kinetic operator min(1/2 k^2, E_cut) (R-14): full 3D transform in five passes ----------
+struct OpPhaseLoad : OpStore {                // forward x pass of a split-operator step: psi * phase on load
+    __device__ __forceinline__ cd load(const cd* in, long long off, long long g) const { return cmul(in[off], __ldg(p.phase + g)); }
+};
+struct OpMul3DScaled : OpStore {              // z round trip with kscale * table (filter: table scaled by 2 / dE)
+    __device__ __forceinline__ cd mult(cd X, int, long long gk) const { return cscale(X, p.kscale * __ldg(p.mul3d + gk)); }
+};
+struct OpMul3DC : OpStore {                   // z round trip with a complex table: exp(-i T dt) / N_g
+    __device__ __forceinline__ cd mult(cd X, int, long long gk) const { return cmul(X, __ldg(p.mul3c + gk)); }
+};
+struct OpInvAddV : OpStore {                  // last inverse pass of H apply: out = T src + vtab * src
+    __device__ __forceinline__ void epi(cd r, long long off, long long g) const {
+        const cd u = p.src[off];
+        const double v = p.vtab ? __ldg(p.vtab + g) : 0.0;
+        p.out[off] = make_double2(r.x + v * u.x, r.y + v * u.y);
+    }
+};
+struct OpInvCheb : OpStore {                  // last inverse pass of a Chebyshev step: acc <- hs (T + vtab) src + alpha acc
+    __device__ __forceinline__ void epi(cd r, long long off, long long g) const {
+        const cd u = p.src[off];
+        const double v = __ldg(p.vtab + g);
+        cd n = make_double2(p.hs * (r.x + v * u.x), p.hs * (r.y + v * u.y));
+        if (p.alpha != 0.0) { const cd o = p.acc[off]; n.x += p.alpha * o.x; n.y += p.alpha * o.y; }
+        p.acc[off] = n;
+    }
+};
+struct OpInvPhase : OpStore {                 // last inverse pass of a split-operator step: result * phase on store
+    __device__ __forceinline__ void epi(cd r, long long off, long long g) const { p.out[off] = cmul(r, __ldg(p.phase + g)); }
 };
 
 }  // namespace sgw

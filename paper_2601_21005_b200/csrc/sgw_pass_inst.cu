@@ -203,11 +203,19 @@ static int launch_acc(const AccCall* c) {
 extern "C" int SGW_CAT(sgw_pass_launch_, SGW_N)(const sgw::PassCall* c) {
     using namespace sgw;
     switch (c->kind) {
-        case K_RT_MUL3D: return launch<MODE_RT, OpMul3D>(c);
-        case K_FWD: return c->variant == 1 ? launch<MODE_FWD, OpFromReal>(c) : launch<MODE_FWD, OpStore>(c);
+        case K_RT_MUL3D:
+            return c->variant == 1 ? launch<MODE_RT, OpMul3DC>(c) : (c->variant == 2 ? launch<MODE_RT, OpMul3DScaled>(c) : launch<MODE_RT, OpMul3D>(c));
+        case K_FWD:
+            return c->variant == 1 ? launch<MODE_FWD, OpFromReal>(c) : (c->variant == 3 ? launch<MODE_FWD, OpPhaseLoad>(c) : launch<MODE_FWD, OpStore>(c));
         case K_INV:
-            return c->variant == 1 ? launch<MODE_INV, OpPhaseMerge>(c)
-                                   : (c->variant == 2 ? launch<MODE_INV, OpToReal>(c) : launch<MODE_INV, OpStore>(c));
+            switch (c->variant) {
+                case 1: return launch<MODE_INV, OpPhaseMerge>(c);
+                case 2: return launch<MODE_INV, OpToReal>(c);
+                case 3: return launch<MODE_INV, OpInvAddV>(c);
+                case 4: return launch<MODE_INV, OpInvCheb>(c);
+                case 5: return launch<MODE_INV, OpInvPhase>(c);
+                default: return launch<MODE_INV, OpStore>(c);
+            }
         default: return -1;
     }
 }

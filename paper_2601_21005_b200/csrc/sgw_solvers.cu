@@ -226,7 +226,8 @@ extern "C" int sgw_apply_H(sgw_ctx* c, int nvec, const void* d_in, void* d_out) 
         const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
         const cd* i0 = in + (long long)v0 * c->ng;
         cd* o0 = out + (long long)v0 * c->ng;
-        SGW_TRY(acc_enabled(c) ? acc_apply_H(c, nv, i0, o0) : lean_apply_H(c, nv, i0, o0));
+        if (c->ecut > 0.0) SGW_TRY(cut_apply_H(c, nv, i0, o0));
+        else SGW_TRY(acc_enabled(c) ? acc_apply_H(c, nv, i0, o0) : lean_apply_H(c, nv, i0, o0));
         SGW_TRY(kb_apply(c, nv, i0, o0, 0, 1.0));
     }
     return SGW_OK;
@@ -259,7 +260,8 @@ int cheb_filter_body(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, 
     for (int v0 = 0; v0 < nvec; v0 += c->max_nvec) {
         const int nv = (nvec - v0 < c->max_nvec) ? nvec - v0 : c->max_nvec;
         cd* X0 = (cd*)d_psi + (long long)v0 * ng;
-        SGW_TRY(acc_enabled(c) ? acc_cheb_filter(c, nv, X0, h_coeffs, s, nterms) : lean_cheb_filter(c, nv, X0, h_coeffs, s, nterms));
+        if (c->ecut > 0.0) SGW_TRY(cut_cheb_filter(c, nv, X0, h_coeffs, s, nterms));
+        else SGW_TRY(acc_enabled(c) ? acc_cheb_filter(c, nv, X0, h_coeffs, s, nterms) : lean_cheb_filter(c, nv, X0, h_coeffs, s, nterms));
     }
     return SGW_OK;
 }
@@ -269,7 +271,7 @@ int cheb_filter_body(sgw_ctx* c, int nvec, void* d_psi, const double* h_coeffs, 
 // CUDA graph and replayed on the caller's stream from then on (the first call with a key launches plainly).  SGW_GRAPH=0 disables, SGW_GRAPH_BYTES moves
 // the size limit (bytes of one vector block; default 16 MB); both are read when the context is created.
 bool filter_graph_wanted(const sgw_ctx* c, int nvec, int nterms) {
-    if (!c->graph_on || c->prof_on || c->nsphere > 0 || nvec > c->max_nvec || nterms < 3) return false;
+    if (!c->graph_on || c->prof_on || c->nsphere > 0 || nvec > c->max_nvec || nterms < 3 || c->ecut > 0.0) return false;
     return (double)nvec * (double)c->ng * sizeof(cd) <= c->graph_bytes;
 }
 }  // namespace
@@ -321,6 +323,7 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
     if (nvec == 0 || nsteps == 0) return SGW_OK;
     const long long ng = c->ng;
     cd* psi = (cd*)d_psi;
+    if (c->ecut > 0.0) return cut_td_propagate(c, nvec, psi, dt, nsteps);
     if (!c->td_kin_valid || c->td_dt != dt) {
         // exp(-i 1/2 k^2 dt)/N per axis, built on the device from the 1/2 k^2 tables (no host synchronisation)
         for (int a = 0; a < 3; ++a) {

@@ -41,6 +41,8 @@ int main(void) {
     CHECK(sgw_profile_enable(NULL, 1) == SGW_EINVAL);
     CHECK(sgw_profile_reset(NULL) == SGW_EINVAL);
     CHECK(sgw_profile_get(NULL, 0, 0, &cnt, &ms) == SGW_EINVAL);
+    CHECK(sgw_set_kinetic_cutoff(NULL, 28.0) == SGW_EINVAL);
+    CHECK(sgw_probe_fp64(NULL, &ms) == SGW_EINVAL);
     CHECK(sgw_sync_check(NULL) == SGW_EINVAL);
     CHECK(sgw_launch_count(NULL) == 0);
     CHECK(sgw_destroy(NULL) == SGW_OK);
@@ -74,6 +76,12 @@ int main(void) {
     CHECK(sgw_apply_H(ctx, 1, psi, out) == SGW_OK);
     CHECK(sgw_profile_get(ctx, 2, 2, &cnt, &ms) == SGW_OK && cnt == 1);
     CHECK(sgw_profile_enable(ctx, 0) == SGW_OK);
+    CHECK(sgw_set_kinetic_cutoff(ctx, 5.0) == SGW_OK);
+    CHECK(sgw_apply_H(ctx, 2, psi, out) == SGW_OK);
+    CHECK(sgw_cheb_filter(ctx, 2, psi, coeffs, -1.0, 20.0, 3) == SGW_OK);
+    CHECK(sgw_td_propagate(ctx, 2, psi, 0.05, 2) == SGW_OK);
+    CHECK(sgw_set_kinetic_cutoff(ctx, 0.0) == SGW_OK);
+    CHECK(sgw_probe_fp64(ctx, &ms) == SGW_OK && ms > 1e11);
     CHECK(sgw_sync_check(ctx) == SGW_OK);
     double h[2] = {0, 0};
     CHECK(cudaMemcpy(h, nrm, 16, cudaMemcpyDeviceToHost) == cudaSuccess);

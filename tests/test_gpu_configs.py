@@ -359,6 +359,56 @@ def test_tma_accumulate_kernel_apply_H_and_clenshaw_filter(api, torch_cuda, orac
     ctx.close()
 
 
+@pytest.mark.parametrize("shape,nvec,use_kb", [((32, 32, 32), 3, True), ((24, 32, 16), 2, False), ((64, 64, 64), 2, True)])
+def test_kinetic_cutoff_five_pass_route(api, torch_cuda, oracle, shape, nvec, use_kb):
+    """NEXT-3: with sgw_set_kinetic_cutoff the kinetic operator is min(1/2 k^2, E_cut), which is not
+    separable; H apply, the Chebyshev filter and the split-operator step then take the five-pass full-3D-transform route.
+    Against the oracle with the same cutoff (cubic and non-cubic grids, with and without KB and the Hartree rebuild),
+    and back to the separable operator after sgw_set_kinetic_cutoff(0)."""
+    torch = torch_cuda
+    nx, ny, nz = shape
+    ecut = 9.0
+    g = W.Grid(nx, ny, nz, 0.5, 0.45, 0.55)
+    rng = np.random.default_rng(nx + nz)
+    centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    kb = W.kb_projectors(g, centers[:2], radius=1.8, sigma=0.7) if use_kb else W.KB.empty()
+    kbo = kb if kb.nsphere else None
+    psi = rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    if kb.nsphere:
+        ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                             torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+    plain = ctx.sgw_apply_H(torch.from_numpy(psi).cuda()).cpu().numpy()
+    ctx.sgw_set_kinetic_cutoff(ecut)
+    try:
+        oracle.set_kinetic_cutoff(ecut)
+        got = ctx.sgw_apply_H(torch.from_numpy(psi).cuda()).cpu().numpy()
+        want = oracle.apply_H(g, vloc, kbo, psi, ld=True)
+        assert relerr(got, want) < TOL_H
+        assert relerr(plain, want) > 1e-3                     # the cutoff changes the operator on this grid
+        emin, emax = float(vloc.min()) - 2.0, ecut + float(vloc.max()) + 2.0      # the narrower window the cutoff buys (P:88)
+        for nterms in (2, 5, 8):
+            coeffs = rng.standard_normal(nterms)
+            t = torch.from_numpy(psi).cuda()
+            ctx.sgw_cheb_filter(t, coeffs, emin, emax)
+            assert relerr(t.cpu().numpy(), oracle.cheb_filter(g, vloc, kbo, psi, coeffs, emin, emax, ld=True)) < TOL_FULL
+        rs = 2.0 / (nvec * g.dV) * 0.01
+        for mode in (0, 1):
+            ctx.sgw_set_td(mode, rs)
+            t = torch.from_numpy(psi).cuda()
+            ctx.sgw_td_propagate(t, 0.05, 3)
+            assert relerr(t.cpu().numpy(), oracle.td_propagate(g, vloc, kbo, psi, 0.05, 3, mode, rs, ld=True)) < TOL_FULL
+    finally:
+        oracle.set_kinetic_cutoff(0.0)
+    ctx.sgw_set_kinetic_cutoff(0.0)
+    again = ctx.sgw_apply_H(torch.from_numpy(psi).cuda()).cpu().numpy()
+    assert relerr(again, plain) < 1e-14
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
+
+
 def test_cfg2_full_length_propagation_invariants(api, torch_cuda):
     """cfg2 at full size and full length (16 vectors, 2000 steps, dt = 0.05): properties that hold at any length.
     With the Hartree term rebuilt every step the propagator stays unitary (norms conserved); with a frozen potential

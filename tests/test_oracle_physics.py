@@ -415,3 +415,76 @@ def test_kinetic_cutoff_plane_waves_dense_matrix_spectrum_and_propagator(oracle)
     pw = np.exp(2j * np.pi * (3 * x / g.nx))[None]
     k = 2 * np.pi * 3 / (g.nx * g.hx)
     assert np.max(np.abs(oracle.apply_H(g, None, None, pw, ld=True) - 0.5 * k * k * pw)) < 1e-11
+
+
+# ------------------------------------------------------------------ NEXT-2: pair propagation and xi projection
+def _xi_dense(g, seed, nxi, nfrag):
+    """xi_m as dense +-1 / 0 arrays from a big-int restatement of the keyed hash (workloads._sm64): R-23."""
+    L = 32
+    xi = np.zeros((nxi, g.ng))
+    for m in range(nxi):
+        for f in range(nfrag):
+            kb_ = W._sm64(W._sm64(seed) ^ (2 * m))
+            b = W._sm64(kb_ ^ f) % (g.ng // L)
+            ks = W._sm64(W._sm64(seed) ^ (2 * m + 1))
+            for j in range(L):
+                sg = -1.0 if (W._sm64(ks ^ (f * L + j)) >> 63) else 1.0
+                xi[m, b * L + j] += sg                    # overlapping fragments add up, as in the oracle's loop
+    return xi
+
+
+def test_pair_propagation_and_xi_projection(oracle):
+    """(i) the xi projections are those of a brute-force dense xi built here from the hash definition; (ii) both copies
+    follow td_propagate applied to each separately; (iii) a pure phase kick leaves the density unchanged, so the
+    projections of the two copies agree at t = 0; (iv) lambda = 0 gives identical copies at every step; (v) the u^R
+    coefficients (difference / lambda) are linear in lambda to first order; (vi) at short times they are those of the
+    continuity equation: rho^lambda - rho = lambda t div(rho grad v_pert) + O(t^2) for real start orbitals, i.e.
+    u^R(t) = t V_H[div(rho grad v)] with the Hartree solve of the erf pin -- sign and scale of the response."""
+    g = W.Grid(16, 16, 16, 0.6, 0.6, 0.6)
+    rng = np.random.default_rng(17)
+    L = np.array(g.box)
+    z, y, x = np.meshgrid(np.arange(g.nz) * g.hz, np.arange(g.ny) * g.hy, np.arange(g.nx) * g.hx, indexing="ij")
+
+    def gauss(c, s):
+        d = [np.minimum(np.abs(a - ci), Li - np.abs(a - ci)) for a, ci, Li in zip((x, y, z), c, L)]
+        return np.exp(-(d[0] ** 2 + d[1] ** 2 + d[2] ** 2) / (2 * s * s))
+    vloc = -1.0 * gauss(L / 2, 1.5)
+    psi = np.stack([gauss(L / 2 + [0.7, 0, 0], 1.6), gauss(L / 2 - [0, 0.9, 0.3], 1.9)]).astype(np.complex128)   # real orbitals
+    vpert = 0.3 * np.cos(2 * np.pi * x / L[0]) + 0.2 * np.sin(2 * np.pi * (y / L[1] + z / L[2]))                 # smooth, periodic
+    rs = 2.0 / (2 * g.dV) * 0.05
+    seed, nxi, nfrag, dt, nsteps = 99, 6, 5, 0.01, 4
+    lam = 1e-3
+    kick = oracle.apply_kick(psi, vpert, lam)
+    assert np.max(np.abs(kick - np.exp(-1j * lam * vpert)[None] * psi)) < 1e-15
+    a, b, out = oracle.td_pair(g, vloc, None, psi, kick, dt, nsteps, rs, seed, nxi, nfrag, ld=True)
+    # (i) brute-force projection at step 0 and (ii) trajectories
+    xi = _xi_dense(g, seed, nxi, nfrag)
+    vh0, _ = oracle.hartree(g, psi, rs, ld=True)
+    assert np.max(np.abs(out[0, :, 0] - g.dV * xi @ vh0.ravel())) < 1e-12 * np.max(np.abs(out[0]))
+    assert np.max(np.abs(a - oracle.td_propagate(g, vloc, None, psi, dt, nsteps, 1, rs, ld=True))) < 1e-13
+    assert np.max(np.abs(b - oracle.td_propagate(g, vloc, None, kick, dt, nsteps, 1, rs, ld=True))) < 1e-13
+    # (iii) no response at t = 0
+    assert np.max(np.abs(out[0, :, 1] - out[0, :, 0])) < 1e-13 * np.max(np.abs(out[0]))
+    # (iv) lambda = 0
+    _, _, out0 = oracle.td_pair(g, vloc, None, psi, psi, dt, nsteps, rs, seed, nxi, nfrag, ld=True)
+    assert np.array_equal(out0[:, :, 0], out0[:, :, 1])
+    # (v) linear in lambda
+    ur = (out[:, :, 1] - out[:, :, 0]) / lam
+    kick2 = oracle.apply_kick(psi, vpert, lam / 2)
+    _, _, outh = oracle.td_pair(g, vloc, None, psi, kick2, dt, nsteps, rs, seed, nxi, nfrag, ld=True)
+    urh = (outh[:, :, 1] - outh[:, :, 0]) / (lam / 2)
+    assert np.max(np.abs(ur[1:] - urh[1:])) < 2e-3 * np.max(np.abs(ur[1:]))
+    # (vi) continuity equation at first order in t, spectral derivatives with numpy
+    kx, ky, kz = kgrid(g)
+    rho = rs * np.sum(np.abs(psi) ** 2, axis=0)
+
+    def grad(f):
+        F = np.fft.fftn(f)
+        return [np.fft.ifftn(1j * k * F).real for k in (kx, ky, kz)]
+    gv = grad(vpert)
+    div = sum(np.fft.ifftn(1j * k * np.fft.fftn(rho * gi)).real for k, gi in zip((kx, ky, kz), gv))
+    resp = oracle.poisson(g, div, ld=True)                  # V_H[div(rho grad v)]
+    want1 = g.dV * xi @ resp.ravel()                        # d u^R / dt at t = 0, projected
+    for n in (1, 2):
+        t = n * dt
+        assert np.max(np.abs(ur[n] - t * want1)) < 0.08 * np.max(np.abs(t * want1)), (n, ur[n], t * want1)
