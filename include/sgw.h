@@ -126,6 +126,24 @@ int sgw_set_td(sgw_ctx* ctx, int hartree_mode, double rho_scale);
  * dt may be negative (reverse-time propagation). */
 int sgw_td_propagate(sgw_ctx* ctx, int nvec, void* d_psi, double dt, int nsteps);
 
+/* d_psi <- exp(-i lambda v_pert(r)) d_psi for nvec vectors: the perturbed copy eta^lambda of P:57 ("we create a perturbed
+ * copy of each eta"; R-21: the perturbing potential and its strength are the caller's).  d_vpert: N_g device doubles. */
+int sgw_apply_kick(sgw_ctx* ctx, int nvec, void* d_psi, const double* d_vpert, double lambda);
+
+/* Pair propagation with the sparse stochastic projection of the retarded response ("propagate both perturbed and
+ * unperturbed copies in time under the action of the time-dependent Hamiltonian ... accumulate the causal response
+ * function u^R(r,t) as the difference of the perturbed and unperturbed time-dependent potentials"; projected
+ * on the fly onto N_xi random functions xi on short, fragmented segments of the grid, in segments of L = 32; R-21..R-23).
+ * d_psi (unperturbed) and d_psi_lambda (perturbed) hold nvec vectors each and are both propagated nsteps split-operator
+ * steps in place, each under V_loc + V_H[rho of ITS OWN copy at the start of the step] with the rho_scale of sgw_set_td
+ * (the Hartree rebuild is always on here).  xi_m (m < nxi) consists of nfrag fragments of 32 consecutive grid points;
+ * fragment f starts at grid index 32 * (h(seed, 2m, f) mod N_g/32) and carries the signs (top bit of h(seed, 2m+1, 32 f + j)
+ * ? -1 : +1), h the keyed hash of sgw_random_vectors.  d_out[nsteps][nxi][2] (device doubles) receives, at the start of
+ * step n, dV <xi_m | V_H[rho_copy(t_n)]> for copy 0 (unperturbed) and 1 (perturbed); the coefficients of u^R are
+ * (out[..][1] - out[..][0]) / lambda.  N_g must be a multiple of 32.  nvec <= max_nvec vectors are processed at a time. */
+int sgw_td_propagate_pair(sgw_ctx* ctx, int nvec, void* d_psi, void* d_psi_lambda, double dt, int nsteps, uint64_t xi_seed,
+                          int nxi, int nfrag, double* d_out);
+
 /* Kinetic-energy cutoff ("apply an energy cutoff of 28 Hartrees to the kinetic energy operator"; it bounds
  * the spectral width and with it the number of Chebyshev terms; R-14).  ecut > 0 (Ha): from now on the kinetic operator
  * of sgw_apply_H, sgw_cheb_filter, sgw_td_propagate and sgw_spectral_bounds is F^-1 min(1/2 |k|^2, ecut) F.  That

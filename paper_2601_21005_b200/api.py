@@ -20,7 +20,8 @@ ERRORS = {-1: "SGW_EINVAL", -2: "SGW_ESIZE", -3: "SGW_ENOMEM", -4: "SGW_ECUDA"}
 EXPORTS = ["sgw_init_grid", "sgw_destroy", "sgw_set_vloc", "sgw_set_nonlocal", "sgw_random_vectors",
            "sgw_apply_H", "sgw_cheb_filter", "sgw_hartree", "sgw_set_td", "sgw_td_propagate", "sgw_norms",
            "sgw_launch_count", "sgw_last_error", "sgw_sync_check", "sgw_spectral_bounds", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get",
-           "sgw_probe_fp64", "sgw_set_kinetic_cutoff"]
+           "sgw_probe_fp64", "sgw_set_kinetic_cutoff", "sgw_apply_kick",
+           "sgw_td_propagate_pair"]
 
 
 class SGWError(RuntimeError):
@@ -58,6 +59,8 @@ def load():
         lib.sgw_profile_get.argtypes = [vp, i, i, C.POINTER(i64), C.POINTER(d)]
         lib.sgw_probe_fp64.argtypes = [vp, C.POINTER(d)]
         lib.sgw_set_kinetic_cutoff.argtypes = [vp, d]
+        lib.sgw_apply_kick.argtypes = [vp, i, vp, vp, d]
+        lib.sgw_td_propagate_pair.argtypes = [vp, i, vp, vp, d, i, u64, i, i, vp]
         _lib = lib
     return _lib
 
@@ -177,6 +180,20 @@ class Context:
         n, ms = C.c_int64(), C.c_double()
         _check(self.lib.sgw_profile_get(self._h, axis, kind, C.byref(n), C.byref(ms)))
         return n.value, ms.value
+
+    def sgw_apply_kick(self, psi, vpert, lam):
+        nvec = _cvec(psi, self.ng)
+        _real(vpert, self.ng)
+        _check(self.lib.sgw_apply_kick(self._h, nvec, _ptr(psi), _ptr(vpert), float(lam)))
+        return psi
+
+    def sgw_td_propagate_pair(self, psi, psi_lam, dt, nsteps, xi_seed, nxi, nfrag):
+        nvec = _cvec(psi, self.ng)
+        assert _cvec(psi_lam, self.ng) == nvec
+        out = torch.empty((nsteps, nxi, 2), dtype=torch.float64, device=self.device)
+        _check(self.lib.sgw_td_propagate_pair(self._h, nvec, _ptr(psi), _ptr(psi_lam), float(dt), int(nsteps), int(xi_seed),
+                                              int(nxi), int(nfrag), _ptr(out)))
+        return out
 
     def sgw_set_kinetic_cutoff(self, ecut):
         _check(self.lib.sgw_set_kinetic_cutoff(self._h, float(ecut)))

@@ -161,6 +161,36 @@ static __global__ void power_scale_kernel(cd* __restrict__ x, const cd* __restri
     if (i < n) x[i] = cscale(y[i], inv);
 }
 
+// ---- NEXT-2: perturbed copy and sparse stochastic projection (R-21..R-23) -------------------------
+// psi[v][g] *= exp(-i lambda vpert[g])
+static __global__ void kick_kernel(cd* __restrict__ psi, const double* __restrict__ vpert, double lambda, long long ng) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ng) return;
+    double s, c;
+    sincos(lambda * vpert[i], &s, &c);
+    cd* p = psi + (long long)blockIdx.y * ng;
+    p[i] = cmul(p[i], make_double2(c, -s));
+}
+
+// out[m * stride] = dV * sum over the nfrag fragments of xi_m (32 consecutive grid points each, start 32 * (h(seed, 2m, f)
+// mod N_g/32), signs from the top bit of h(seed, 2m+1, 32 f + j)) of sign * field.  One warp per fragment (a coalesced
+// 256-byte read), a shuffle sum per segment of L = 32 and one atomic add per segment ("each xi function is
+// processed in segments of length L = 32"; one atomic add per segment).  grid (nxi), out zeroed by the caller.
+static __global__ void __launch_bounds__(256) xi_project_kernel(const double* __restrict__ field, long long ng, uint64_t seed_mixed, int nfrag,
+                                                                 double dV, double* __restrict__ out, int stride) {
+    const int m = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const uint64_t kpos = sm64(seed_mixed ^ (uint64_t)(2 * m)), ksgn = sm64(seed_mixed ^ (uint64_t)(2 * m + 1));
+    const uint64_t nblocks = (uint64_t)(ng / 32);
+    for (int f = warp; f < nfrag; f += nwarps) {
+        const uint64_t b = sm64(kpos ^ (uint64_t)f) % nblocks;
+        const double sg = (sm64(ksgn ^ ((uint64_t)f * 32 + lane)) >> 63) ? -1.0 : 1.0;
+        double a = sg * field[b * 32 + lane];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) a += __shfl_down_sync(0xffffffffu, a, o);
+        if (lane == 0) atomicAdd(out + (long long)m * stride, a * dV);
+    }
+}
+
 // ---- a6: Kleinman-Bylander gather-dot (R-12) --------------------------------------------
 // grid (nsphere, nvec), 128 threads: c[v][s][p] = dV * sum_j beta[j][p] * psi_v[idx[j]]
 template <int NP>

@@ -379,3 +379,68 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
     }
     return SGW_OK;
 }
+
+// =====================================================================================================
+// NEXT-2: perturbed / unperturbed pair propagation with the xi projection of both Hartree potentials
+// =====================================================================================================
+extern "C" int sgw_apply_kick(sgw_ctx* c, int nvec, void* d_psi, const double* d_vpert, double lambda) {
+    if (!c || nvec < 0 || (nvec > 0 && (!d_psi || !d_vpert))) return set_error(SGW_EINVAL, "sgw_apply_kick: bad argument");
+    if (nvec == 0) return SGW_OK;
+    dim3 grid(blocks_for(c->ng, 256), nvec);
+    kick_kernel<<<grid, 256, 0, c->stream>>>((cd*)d_psi, d_vpert, lambda, c->ng);
+    return launched(c, "kick_kernel");
+}
+
+namespace {
+// one split-operator step of one copy with the Hartree potential already in c->vh (potential half steps on load in x and
+// on store in z, KB factors conjugated by the phase: the same step as sgw_td_propagate, without the merged tables)
+int pair_step(sgw_ctx* c, int nvec, cd* psi, double dt) {
+    const long long ng = c->ng;
+    const bool kb = c->nsphere > 0;
+    phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, c->vh, 0.5 * dt, c->phase, ng);
+    SGW_TRY(launched(c, "phase"));
+    const int chunk = nvec < c->max_nvec ? nvec : c->max_nvec;
+    for (int cv = 0; cv < nvec; cv += chunk) {
+        const int nc = (nvec - cv < chunk) ? nvec - cv : chunk;
+        cd* ps = psi + (long long)cv * ng;
+        if (kb) SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, +1));
+        SGW_TRY(lean_td_step(c, nc, ps, false, false, false, false));     // phase on load in x, on store in z
+        if (kb) SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, -1));
+    }
+    return SGW_OK;
+}
+}  // namespace
+
+extern "C" int sgw_td_propagate_pair(sgw_ctx* c, int nvec, void* d_psi, void* d_psi_lambda, double dt, int nsteps, uint64_t xi_seed,
+                                     int nxi, int nfrag, double* d_out) {
+    if (!c || nvec < 0 || nsteps < 0 || nxi < 0 || nfrag < 0 || (nvec > 0 && (!d_psi || !d_psi_lambda)) || d_psi == d_psi_lambda ||
+        (nxi > 0 && nsteps > 0 && !d_out))
+        return set_error(SGW_EINVAL, "sgw_td_propagate_pair: bad argument");
+    if (c->ng % 32) return set_error(SGW_ESIZE, "sgw_td_propagate_pair: N_g must be a multiple of the segment length 32");
+    if (c->ecut > 0.0) return set_error(SGW_EINVAL, "sgw_td_propagate_pair: not available with a kinetic-energy cutoff");
+    if (nvec == 0 || nsteps == 0) return SGW_OK;
+    if (!c->td_kin_valid || c->td_dt != dt) {
+        for (int a = 0; a < 3; ++a) {
+            td_table_kernel<<<blocks_for(c->dims[a], 128), 128, 0, c->stream>>>(c->kin_raw[a], dt, c->td_kin[a], c->dims[a]);
+            SGW_TRY(launched(c, "td_table"));
+        }
+        c->td_dt = dt; c->td_kin_valid = true;
+    }
+    const double dV = c->hx * c->hy * c->hz;
+    if (nxi > 0) SGW_TRY(check_cuda(cudaMemsetAsync(d_out, 0, (size_t)nsteps * nxi * 2 * sizeof(double), c->stream), "clear projections"));
+    cd* copy[2] = {(cd*)d_psi, (cd*)d_psi_lambda};
+    for (int n = 0; n < nsteps; ++n) {
+        for (int k = 0; k < 2; ++k) {
+            // V_H[rho_copy(t_n)] -> c->vh, its xi projections, then the step of this copy under V_loc + that potential
+            HartreeOut o;
+            o.vh = c->vh;
+            SGW_TRY(hartree_into(c, nvec, copy[k], c->rho_scale, nullptr, false, o));
+            if (nxi > 0) {
+                xi_project_kernel<<<nxi, 256, 0, c->stream>>>(c->vh, c->ng, sm64(xi_seed), nfrag, dV, d_out + ((size_t)n * nxi) * 2 + k, 2);
+                SGW_TRY(launched(c, "xi_project"));
+            }
+            SGW_TRY(pair_step(c, nvec, copy[k], dt));
+        }
+    }
+    return SGW_OK;
+}

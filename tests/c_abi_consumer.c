@@ -42,6 +42,8 @@ int main(void) {
     CHECK(sgw_profile_reset(NULL) == SGW_EINVAL);
     CHECK(sgw_profile_get(NULL, 0, 0, &cnt, &ms) == SGW_EINVAL);
     CHECK(sgw_set_kinetic_cutoff(NULL, 28.0) == SGW_EINVAL);
+    CHECK(sgw_apply_kick(NULL, 1, NULL, NULL, 0.1) == SGW_EINVAL);
+    CHECK(sgw_td_propagate_pair(NULL, 1, NULL, NULL, 0.05, 1, 1, 1, 1, NULL) == SGW_EINVAL);
     CHECK(sgw_probe_fp64(NULL, &ms) == SGW_EINVAL);
     CHECK(sgw_sync_check(NULL) == SGW_EINVAL);
     CHECK(sgw_launch_count(NULL) == 0);
@@ -59,7 +61,7 @@ int main(void) {
     double *vloc = NULL, *vh = NULL, *nrm = NULL;
     CHECK(cudaMalloc(&psi, 2 * ng * 16) == cudaSuccess && cudaMalloc(&out, 2 * ng * 16) == cudaSuccess);
     CHECK(cudaMalloc((void**)&vloc, ng * 8) == cudaSuccess && cudaMalloc((void**)&vh, ng * 8) == cudaSuccess);
-    CHECK(cudaMalloc((void**)&nrm, 2 * 8) == cudaSuccess);
+    CHECK(cudaMalloc((void**)&nrm, 4 * 8) == cudaSuccess);
     CHECK(cudaMemset(vloc, 0, ng * 8) == cudaSuccess);
     CHECK(sgw_set_vloc(ctx, vloc) == SGW_OK);
     CHECK(sgw_set_nonlocal(ctx, 0, NULL, NULL, 4, NULL, NULL) == SGW_OK);
@@ -76,6 +78,8 @@ int main(void) {
     CHECK(sgw_apply_H(ctx, 1, psi, out) == SGW_OK);
     CHECK(sgw_profile_get(ctx, 2, 2, &cnt, &ms) == SGW_OK && cnt == 1);
     CHECK(sgw_profile_enable(ctx, 0) == SGW_OK);
+    CHECK(sgw_apply_kick(ctx, 2, out, vloc, 0.01) == SGW_OK);
+    CHECK(sgw_td_propagate_pair(ctx, 2, psi, out, 0.05, 2, 7, 1, 3, nrm) == SGW_OK);    /* nrm: 2 steps x 1 xi x 2 = 4 doubles */
     CHECK(sgw_set_kinetic_cutoff(ctx, 5.0) == SGW_OK);
     CHECK(sgw_apply_H(ctx, 2, psi, out) == SGW_OK);
     CHECK(sgw_cheb_filter(ctx, 2, psi, coeffs, -1.0, 20.0, 3) == SGW_OK);

@@ -409,6 +409,46 @@ def test_kinetic_cutoff_five_pass_route(api, torch_cuda, oracle, shape, nvec, us
     ctx.close()
 
 
+@pytest.mark.parametrize("n,nvec,use_kb", [(32, 3, False), (48, 2, True), (64, 2, False)])
+def test_pair_propagation_with_xi_projection(api, torch_cuda, oracle, n, nvec, use_kb):
+    """NEXT-2: perturbed copy exp(-i lambda v) eta, both copies propagated under their own
+    Hartree potentials, and the xi projections of both potentials at every step, against the oracle: the kick bit for
+    bit up to rounding, both trajectories to 1e-8, the projections to 1e-10 of their scale, and the u^R coefficients
+    (difference / lambda) to 1e-6 of theirs (they are a small difference of the projections)."""
+    torch = torch_cuda
+    g = W.Grid(n, n, n, 0.5, 0.5, 0.5)
+    rng = np.random.default_rng(3 * n)
+    centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    kb = W.kb_projectors(g, centers[:2], radius=1.8, sigma=0.7) if use_kb else W.KB.empty()
+    kbo = kb if kb.nsphere else None
+    vpert = W.gaussian_vloc(g, centers[1:2], [0.7], [1.5]) + 0.1
+    psi = rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+    lam, dt, nsteps, seed, nxi, nfrag = 1e-2, 0.05, 4, 77, 9, 6
+    rs = 2.0 / (nvec * g.dV) * 0.01
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    if kb.nsphere:
+        ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                             torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+    ctx.sgw_set_td(1, rs)
+    a = torch.from_numpy(psi).cuda()
+    b = a.clone()
+    ctx.sgw_apply_kick(b, torch.from_numpy(vpert).cuda(), lam)
+    kick = oracle.apply_kick(psi, vpert, lam)
+    assert relerr(b.cpu().numpy(), kick) < 1e-14
+    out = ctx.sgw_td_propagate_pair(a, b, dt, nsteps, seed, nxi, nfrag).cpu().numpy()
+    ra, rb, rout = oracle.td_pair(g, vloc, kbo, psi, kick, dt, nsteps, rs, seed, nxi, nfrag, ld=True)
+    assert relerr(a.cpu().numpy(), ra) < TOL_FULL and relerr(b.cpu().numpy(), rb) < TOL_FULL
+    scale = np.max(np.abs(rout))
+    assert np.max(np.abs(out - rout)) < 1e-10 * scale
+    ur, rur = (out[:, :, 1] - out[:, :, 0]) / lam, (rout[:, :, 1] - rout[:, :, 0]) / lam
+    assert np.max(np.abs(ur[0])) < 1e-9 * scale / lam                    # no response at t = 0 (a pure phase kick)
+    assert np.max(np.abs(ur - rur)) < 1e-6 * np.max(np.abs(rur))
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
+
+
 def test_cfg2_full_length_propagation_invariants(api, torch_cuda):
     """cfg2 at full size and full length (16 vectors, 2000 steps, dt = 0.05): properties that hold at any length.
     With the Hartree term rebuilt every step the propagator stays unitary (norms conserved); with a frozen potential
