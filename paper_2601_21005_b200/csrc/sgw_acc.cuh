@@ -399,6 +399,223 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
     }
 }
 
+// =====================================================================================================================
+// Split-operator factors through the same slot ring: psi <- [phase] F^-1 exp(-i T_axis dt) F [phase] psi for
+// one axis per launch, in place: TMA load of a tile, round trip with the complex k table in the slot, plain bulk store
+// back to where it came from.  The potential phases (an N_g table shared by all vectors) are read from global memory by
+// the thread that owns the element; the tiles run over the vectors first, so the table comes from HBM once per launch.
+// =====================================================================================================================
+enum { KX = 0, KY = 1, KZ = 2 };          // tile kinds = axes
+
+struct TdArgs {
+    cd* psi;
+    const cd* phase;          // N_g table applied on load (F_PRO) or on store (F_EPI)
+    double* rho;              // F_DENS: rho[g] += dens_scale * |result|^2
+    double dens_scale;
+    const cd* kc;             // complex k table of the axis: exp(-i 1/2 k^2 dt) / N
+    const cd* tw;
+    int kind;                 // KX, KY or KZ
+    int flags;                // F_PRO / F_EPI / F_DENS
+    int nvec, nz;
+    unsigned ntiles;          // nvec * N * N / 8
+};
+
+template <int N, bool XK>
+__device__ __forceinline__ void td_tile_compute(const TdArgs& a, cd* tile, const cd* __restrict__ ph, double* __restrict__ rp, int gstep,
+                                                const cd* twA, const cd* twB, const cd* ktab, int gt, int bar_id) {
+    using C = AccCfg<N>;
+    constexpr int R1 = C::R1, R2 = C::R2, TG = C::TG, GW = C::GW, GT = C::GT, TASKS = C::TASKS, ROUNDS = C::ROUNDS, B = C::B;
+    constexpr bool WCACHE = R2 <= 8;
+    constexpr int SB = XK ? C::XP : 1, SI = XK ? 1 : B;
+    const bool actA = gt < TG;
+    const int n2 = XK ? gt % R2 : gt / B, bA = XK ? gt / R2 : gt % B;
+    cd* eA = tile + bA * SB + n2 * SI;
+    cd x[R1];
+    if (actA) {
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) x[n1] = eA[n1 * R2 * SI];
+        if (a.flags & F_PRO) {
+#pragma unroll
+            for (int n1 = 0; n1 < R1; ++n1) x[n1] = cmul(x[n1], __ldg(ph + (long long)n1 * gstep));
+        }
+        Dft<R1, -1>::run(x);
+        if (WCACHE) {
+#pragma unroll
+            for (int j = 0; j < R1; ++j) eA[j * R2 * SI] = x[j];
+        } else {
+            eA[0] = x[0];
+#pragma unroll
+            for (int j = 1; j < R1; ++j) eA[j * R2 * SI] = cmul(x[j], twA[j * R2 + n2]);
+        }
+    }
+    lean_sync<GW>(bar_id);
+#pragma unroll
+    for (int rd = 0; rd < ROUNDS; ++rd) {
+        const int task = gt + rd * GT;
+        if (task < TASKS) {
+            const int bB = task % B, k1 = task / B;
+            cd* eB = tile + bB * SB + k1 * R2 * SI;
+            cd y[R2], wc[WCACHE ? R2 : 1];
+            y[0] = eB[0];
+            if (WCACHE) {
+#pragma unroll
+                for (int m = 1; m < R2; ++m) { wc[m] = twB[m * R1 + k1]; y[m] = cmul(eB[m * SI], wc[m]); }
+            } else {
+#pragma unroll
+                for (int m = 1; m < R2; ++m) y[m] = eB[m * SI];
+            }
+            Dft<R2, -1>::run(y);
+            const cd* kt = ktab + k1;
+#pragma unroll
+            for (int k2 = 0; k2 < R2; ++k2) y[k2] = cmul(y[k2], kt[R1 * k2]);
+            Dft<R2, +1>::run(y);
+            eB[0] = y[0];
+#pragma unroll
+            for (int m = 1; m < R2; ++m) eB[m * SI] = cmulc(y[m], WCACHE ? wc[m] : twB[m * R1 + k1]);
+        }
+    }
+    lean_sync<GW>(bar_id);
+    if (actA) {
+#pragma unroll
+        for (int j = 0; j < R1; ++j) x[j] = eA[j * R2 * SI];
+        Dft<R1, +1>::run(x);
+        if (a.flags & F_EPI) {
+#pragma unroll
+            for (int n1 = 0; n1 < R1; ++n1) x[n1] = cmul(x[n1], __ldg(ph + (long long)n1 * gstep));
+        }
+        if (a.flags & F_DENS) {
+            const double ds = a.dens_scale;
+#pragma unroll
+            for (int n1 = 0; n1 < R1; ++n1) atomicAdd(rp + (long long)n1 * gstep, ds * (x[n1].x * x[n1].x + x[n1].y * x[n1].y));
+        }
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) eA[n1 * R2 * SI] = x[n1];
+        fence_proxy_async_smem();
+    }
+    lean_sync<GW>(bar_id);
+}
+
+__device__ __forceinline__ void bulk_store(void* gdst, const void* ssrc, unsigned bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, const void* src, int c0, int c1, int c2) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];\n" ::"l"(m), "r"(smem_u32(src)),
+                 "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+template <int N>
+__global__ void __launch_bounds__(AccCfg<N>::T, 1)
+td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_z, int nslots) {
+    using C = AccCfg<N>;
+    constexpr int GT = C::GT, NG = C::NG, B = C::B, TILE = C::TILE;
+    constexpr unsigned ROWB = N * 16, TILEB = N * B * 16, TPV = (unsigned)N * N / 8;
+    extern __shared__ __align__(128) char smraw[];
+    char* slots = smraw;
+    cd* twA = reinterpret_cast<cd*>(smraw + (size_t)nslots * TILE);
+    cd* twB = twA + N;
+    cd* ktab = twB + N;
+    uint64_t* full = reinterpret_cast<uint64_t*>(ktab + N);
+    uint64_t* done = full + C::MAXS;
+    uint64_t* empty = done + C::MAXS;
+    const int tid = threadIdx.x;
+    for (int i = tid; i < N; i += C::T) {
+        twA[i] = a.tw[(i % C::R2) * (i / C::R2)];
+        twB[i] = a.tw[(i / C::R1) * (i % C::R1)];
+        ktab[i] = a.kc[i];
+    }
+    if (tid == 0) {
+        for (int s = 0; s < nslots; ++s) { mbar_init(full + s, 1); mbar_init(done + s, 1); mbar_init(empty + s, 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+    const unsigned S = (unsigned)nslots, nvec = (unsigned)a.nvec;
+    // tile t -> block q of the vector's N*N/8 blocks (x: 8 rows; y: plane z = q / (N/8), 8 columns; z: 8 xy points), vector v;
+    // vectors fastest, so that consecutive tiles read the same part of the phase table
+    if (tid < 64) {
+        if (tid == 0) {
+            unsigned seq = 0;
+            for (unsigned t = blockIdx.x; t < a.ntiles; t += gridDim.x, ++seq) {
+                const unsigned q = t / nvec, v = t - q * nvec, s = seq % S, round = seq / S;
+                if (round > 0) mbar_wait(empty + s, (round - 1) & 1);
+                char* dst = slots + (size_t)s * TILE;
+                mbar_expect_tx(full + s, TILEB);
+                if (a.kind == KX) {
+                    const cd* row0 = a.psi + ((long long)v * a.nz * N + (long long)q * B) * N;
+#pragma unroll
+                    for (int b = 0; b < B; ++b) bulk_load(dst + (size_t)b * C::XP * 16, row0 + b * N, ROWB, full + s);
+                } else {
+                    const CUtensorMap* m = a.kind == KY ? &map_y : &map_z;
+                    const unsigned tpp = N / 8;
+                    const int c0 = a.kind == KY ? (int)(q % tpp) * 16 : (int)q * 16;
+                    const int c2 = a.kind == KY ? (int)(v * (unsigned)a.nz + q / tpp) : (int)v;
+#pragma unroll
+                    for (int o = 0; o < C::NOPS; ++o) tma_load_3d(dst + (size_t)o * C::NBOX * B * 16, m, c0, o * C::NBOX, c2, full + s);
+                }
+            }
+        } else if (tid == 32) {
+            unsigned seq = 0, pend[2], npend = 0;
+            for (unsigned t = blockIdx.x; t < a.ntiles; t += gridDim.x, ++seq) {
+                const unsigned q = t / nvec, v = t - q * nvec, s = seq % S, round = seq / S;
+                if (!mbar_test(done + s, round & 1)) {
+                    if (npend) {
+                        bulk_wait_read<0>();
+                        for (unsigned k = 0; k < npend; ++k) mbar_arrive(empty + pend[k]);
+                        npend = 0;
+                    }
+                    mbar_wait(done + s, round & 1);
+                }
+                const char* src = slots + (size_t)s * TILE;
+                if (a.kind == KX) {
+                    cd* row0 = a.psi + ((long long)v * a.nz * N + (long long)q * B) * N;
+#pragma unroll
+                    for (int b = 0; b < B; ++b) bulk_store(row0 + b * N, src + (size_t)b * C::XP * 16, ROWB);
+                } else {
+                    const CUtensorMap* m = a.kind == KY ? &map_y : &map_z;
+                    const unsigned tpp = N / 8;
+                    const int c0 = a.kind == KY ? (int)(q % tpp) * 16 : (int)q * 16;
+                    const int c2 = a.kind == KY ? (int)(v * (unsigned)a.nz + q / tpp) : (int)v;
+#pragma unroll
+                    for (int o = 0; o < C::NOPS; ++o) tma_store_3d(m, src + (size_t)o * C::NBOX * B * 16, c0, o * C::NBOX, c2);
+                }
+                bulk_commit();
+                if (npend == 2) {
+                    bulk_wait_read<2>();
+                    mbar_arrive(empty + pend[0]);
+                    pend[0] = pend[1]; npend = 1;
+                }
+                pend[npend++] = s;
+            }
+            asm volatile("cp.async.bulk.wait_group 0;\n" ::: "memory");
+        }
+        return;
+    }
+    const int ct = tid - 64, grp = ct / GT, gt = ct % GT;
+    unsigned seq = (unsigned)grp;
+    for (unsigned t = blockIdx.x + (unsigned)grp * gridDim.x; t < a.ntiles; t += NG * gridDim.x, seq += NG) {
+        const unsigned q = t / nvec, s = seq % S, round = seq / S;
+        cd* tile = reinterpret_cast<cd*>(slots + (size_t)s * TILE);
+        // grid index of this thread's first element and the step between its elements (phase table, density)
+        long long g0;
+        int gstep;
+        if (a.kind == KX) { g0 = (long long)q * (B * N) + (gt / C::R2) * N + gt % C::R2; gstep = C::R2; }
+        else if (a.kind == KY) { const unsigned tpp = N / 8, z = q / tpp, cb = q - z * tpp; g0 = (long long)z * (N * N) + cb * B + gt % B + (long long)(gt / B) * N; gstep = C::R2 * N; }
+        else { g0 = (long long)q * B + gt % B + (long long)(gt / B) * (N * N); gstep = C::R2 * N * N; }
+        mbar_wait(full + s, round & 1);
+        if (a.kind == KX) td_tile_compute<N, true>(a, tile, a.phase + g0, a.rho + g0, gstep, twA, twB, ktab, gt, grp);
+        else td_tile_compute<N, false>(a, tile, a.phase + g0, a.rho + g0, gstep, twA, twB, ktab, gt, grp);
+        if (gt == 0) mbar_arrive(done + s);
+    }
+}
+
+struct TdCall {
+    TdArgs args;
+    CUtensorMap map_y, map_z;
+    int num_sms;
+    int* occ;                 // context-owned: [1] = 1 once the kernel attribute is set
+    cudaStream_t stream;
+};
+typedef int (*td_launch_fn)(const TdCall*);
+
 struct AccCall {
     AccArgs args;
     CUtensorMap cur_y, cur_z, acc_y, acc_z;

@@ -9,7 +9,8 @@
 #define SGW_DECL(N)                                             \
     extern "C" int sgw_pass_launch_##N(const sgw::PassCall*);   \
     extern "C" int sgw_lean_launch_##N(const sgw::LeanCall*, int);  \
-    extern "C" int sgw_acc_launch_##N(const sgw::AccCall*);
+    extern "C" int sgw_acc_launch_##N(const sgw::AccCall*);         \
+    extern "C" int sgw_td_launch_##N(const sgw::TdCall*);
 SGW_DECL(8) SGW_DECL(12) SGW_DECL(16) SGW_DECL(24) SGW_DECL(32) SGW_DECL(48) SGW_DECL(64) SGW_DECL(96)
 SGW_DECL(128) SGW_DECL(192) SGW_DECL(256) SGW_DECL(384)
 #undef SGW_DECL
@@ -40,6 +41,14 @@ static pass_launch_fn launcher_for(int n) {
 static acc_launch_fn acc_launcher_for(int n) {
     switch (n) {
 #define SGW_CASE(N) case N: return sgw_acc_launch_##N;
+        SGW_SIZES(SGW_CASE)
+#undef SGW_CASE
+        default: return nullptr;
+    }
+}
+static td_launch_fn td_launcher_for(int n) {
+    switch (n) {
+#define SGW_CASE(N) case N: return sgw_td_launch_##N;
         SGW_SIZES(SGW_CASE)
 #undef SGW_CASE
         default: return nullptr;
@@ -252,6 +261,8 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
             c->tmap_encode = nullptr;
     }
     if (!c->tmap_encode) c->acc = nullptr;
+    c->tdk = c->acc ? td_launcher_for(nx) : nullptr;
+    c->use_acc_td = env_int("SGW_ACC_TD", -1);
     c->lean_vminor = env_int("SGW_LEAN_VMINOR", -1);
     c->lean_chunk = env_int("SGW_LEAN_CHUNK", 0);
     c->l2_chunk = env_int("SGW_L2_CHUNK", 0);

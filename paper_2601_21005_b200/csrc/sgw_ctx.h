@@ -24,6 +24,8 @@ struct sgw_ctx {
     sgw::pass_launch_fn pass[3];             // per-axis launcher of the Poisson passes (x, y, z)
     sgw::lean_launch_fn lean[3];             // per-axis launcher of the lean passes
     sgw::acc_launch_fn acc;                  // TMA accumulate kernel (cubic grids) or NULL
+    sgw::td_launch_fn tdk;                   // TMA split-operator kernel (cubic grids) or NULL
+    int use_acc_td;                          // complex family through it (SGW_ACC_TD; default: from 256 points per axis)
     int acc_occ[4];
     int use_acc;                             // real family through the TMA accumulate kernel (SGW_ACC; default: where it is built and measured faster)
     double acc_l2_bytes;                     // one-launch terms when cur + acc + v of a vector are at most this (SGW_ACC_L2_MB)

@@ -195,6 +195,33 @@ static int launch_acc(const AccCall* c) {
 #endif
 }
 
+static int launch_td(const TdCall* c) {
+#if SGW_N >= 32 && SGW_N % 8 == 0
+    constexpr int N = SGW_N;
+    using Cfg = AccCfg<N>;
+    auto kern = td_tma_kernel<N>;
+    const int fixed = 3 * N * 16 + 3 * Cfg::MAXS * 8 + 128;
+    int nslots = (227 * 1024 - fixed) / Cfg::TILE;
+    if (nslots > Cfg::MAXS) nslots = Cfg::MAXS;
+    if (nslots < 3) return 1;
+    const size_t smem = (size_t)nslots * Cfg::TILE + fixed;
+    if (!c->occ[1]) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return -(1000 + (int)e);
+        c->occ[1] = 1;
+    }
+    long long grid = c->num_sms;
+    if (grid > (long long)c->args.ntiles) grid = c->args.ntiles;
+    if (grid <= 0) return 0;
+    kern<<<(unsigned)grid, Cfg::T, smem, c->stream>>>(c->args, c->map_y, c->map_z, nslots);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? 0 : -(4000 + (int)e);
+#else
+    (void)c;
+    return 1;
+#endif
+}
+
 }  // namespace sgw
 
 #define SGW_CAT_(a, b) a##b
@@ -230,3 +257,6 @@ extern "C" int SGW_CAT(sgw_lean_launch_, SGW_N)(const sgw::LeanCall* c, int B) {
 
 // TMA accumulate kernel: acc += c (T + vtab) cur + e v on a cubic grid of this axis length.  Returns 1 if not built.
 extern "C" int SGW_CAT(sgw_acc_launch_, SGW_N)(const sgw::AccCall* c) { return sgw::launch_acc(c); }
+
+// TMA split-operator factor along one axis of a cubic grid of this axis length, in place.  Returns 1 if not built.
+extern "C" int SGW_CAT(sgw_td_launch_, SGW_N)(const sgw::TdCall* c) { return sgw::launch_td(c); }

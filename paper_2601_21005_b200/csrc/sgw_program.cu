@@ -162,6 +162,10 @@ int lean_apply(sgw_ctx* c, int nv, const LeanOp& op, int kind_tag, bool allow_pl
 
 }  // namespace
 
+namespace {
+int acc_td_step(sgw_ctx* c, int nvec, const LeanOp& op);
+}
+
 namespace sgw {
 
 // out = (Tx + Ty + Tz + V_loc) in (the KB term is added by the caller)
@@ -233,6 +237,8 @@ int lean_td_step(sgw_ctx* c, int nvec, cd* psi, bool kb, bool accumulate_density
     if (accumulate_density && !kb) { op.fz |= F_DENS; op.rho = c->rho; op.dens_scale = c->rho_scale; }
     op.cplx = true;
     for (int a = 0; a < 3; ++a) op.kc[a] = c->td_kin[a];
+    const bool tma = c->tdk && (c->use_acc_td >= 0 ? c->use_acc_td != 0 : c->nx >= 256);
+    if (tma) return acc_td_step(c, nvec, op);
     return lean_apply(c, nvec, op, K_RT_TD);
 }
 
@@ -262,6 +268,38 @@ int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap*
         r = enc(mz, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dz, sz, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return set_error(SGW_ECUDA, "cuTensorMapEncodeTiled failed: " + std::to_string((int)r));
+    return 0;
+}
+
+// one split-operator step through the TMA kernel: three launches (x, y, z factors), each in place
+int acc_td_step(sgw_ctx* c, int nvec, const LeanOp& op) {
+    TdCall call;
+    memset(&call, 0, sizeof(call));
+    SGW_TRY(acc_maps(c, op.acc, nvec, &call.map_y, &call.map_z));
+    call.num_sms = c->num_sms;
+    call.occ = c->acc_occ;
+    call.stream = c->stream;
+    const long long n = c->nx;
+    const int flags[3] = {op.fx, op.fy, op.fz};
+    for (int axis = 0; axis < 3; ++axis) {
+        TdArgs& a = call.args;
+        a.psi = op.acc;
+        a.phase = (axis == 2 && op.phase_z) ? op.phase_z : op.phase;
+        a.rho = op.rho; a.dens_scale = op.dens_scale;
+        a.kc = op.kc[axis];
+        a.tw = c->tw[axis];
+        a.kind = axis;
+        a.flags = flags[axis];
+        a.nvec = nvec; a.nz = c->nz;
+        a.ntiles = (unsigned)(n * n / 8 * nvec);
+        cudaEvent_t e1 = prof_begin(c, axis * K_NKINDS + K_RT_TD);
+        const int rc = c->tdk(&call);
+        if (rc != 0)
+            return set_error(rc < 0 ? SGW_ECUDA : SGW_ESIZE, "TMA split-operator launch failed: stage " + std::to_string((-rc) / 1000) + ": " +
+                                                                 cudaGetErrorString((cudaError_t)((-rc) % 1000)));
+        prof_end(c, e1);
+        c->launches++;
+    }
     return 0;
 }
 

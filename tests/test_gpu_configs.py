@@ -449,6 +449,35 @@ def test_pair_propagation_with_xi_projection(api, torch_cuda, oracle, n, nvec, u
     ctx.close()
 
 
+@pytest.mark.parametrize("n,nvec,use_kb", [(32, 5, False), (48, 3, True), (64, 3, False), (96, 2, True)])
+def test_tma_split_operator_kernel(api, torch_cuda, oracle, monkeypatch, n, nvec, use_kb):
+    """The TMA split-operator kernel (sgw_acc.cuh: td_tma_kernel, one launch per axis: tile load, in-place round trip with
+    the complex k table, bulk store; default from 256 points per axis) forced on for small cubic grids: frozen potential,
+    Hartree rebuild with the density accumulated in the z launch, reverse time, and KB factors, against the oracle."""
+    torch = torch_cuda
+    monkeypatch.setenv("SGW_ACC_TD", "1")
+    g = W.Grid(n, n, n, 0.5, 0.45, 0.55)
+    rng = np.random.default_rng(5 * n)
+    centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    kb = W.kb_projectors(g, centers[:2], radius=1.8, sigma=0.7) if use_kb else W.KB.empty()
+    kbo = kb if kb.nsphere else None
+    psi = rng.standard_normal((nvec,) + g.shape) + 1j * rng.standard_normal((nvec,) + g.shape)
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    if kb.nsphere:
+        ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                             torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+    rs = 2.0 / (nvec * g.dV) * 0.01
+    for mode, dt, nsteps in ((0, 0.05, 1), (0, -0.05, 3), (1, 0.05, 4)):
+        ctx.sgw_set_td(mode, rs)
+        t = torch.from_numpy(psi).cuda()
+        ctx.sgw_td_propagate(t, dt, nsteps)
+        assert relerr(t.cpu().numpy(), oracle.td_propagate(g, vloc, kbo, psi, dt, nsteps, mode, rs, ld=True)) < TOL_FULL, (mode, dt)
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
+
+
 def test_cfg2_full_length_propagation_invariants(api, torch_cuda):
     """cfg2 at full size and full length (16 vectors, 2000 steps, dt = 0.05): properties that hold at any length.
     With the Hartree term rebuilt every step the propagator stays unitary (norms conserved); with a frozen potential
