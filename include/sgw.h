@@ -144,6 +144,26 @@ int sgw_apply_kick(sgw_ctx* ctx, int nvec, void* d_psi, const double* d_vpert, d
 int sgw_td_propagate_pair(sgw_ctx* ctx, int nvec, void* d_psi, void* d_psi_lambda, double dt, int nsteps, uint64_t xi_seed,
                           int nxi, int nfrag, double* d_out);
 
+/* The zeta pair of the Green's function (Eq. 4: "propagating the filtered zeta backwards in time while
+ * simultaneously propagating its orthogonal complement forwards in time"; packed as (N_g x 2); R-25).  d_pair holds
+ * two vectors: [0] the filtered zeta, propagated with -dt, [1] its complement, propagated with +dt, nsteps split-operator
+ * steps each, in place, under the frozen potential V_loc (+ V_NL).  At the start of step n the projections
+ * d_out[n][m][k] = dV <xi_m | phi psi_k(t_n)> (complex; d_out is [nsteps][nxi][2] complex) onto the xi of
+ * sgw_td_propagate_pair are recorded; d_phi: N_g device doubles, the orbital of Eq. 5. */
+int sgw_td_propagate_zeta(sgw_ctx* ctx, void* d_pair, const double* d_phi, double dt, int nsteps, uint64_t xi_seed, int nxi,
+                          int nfrag, void* d_out);
+
+/* Time-ordering of the retarded response ("we time-order the accumulated u^R(r,t) to produce the effective
+ * polarization potential u(r,t)"; a transform in time before and after a complex-conjugation step; R-24), on each of
+ * the nxi coefficient series c^R(t_n), n < nt, element (n, m) at d_cr[n * stride_n + m * stride_m] (real, causal): zero-
+ * padded to M = 2 nt samples, C(w_k) = sum_n c^R(t_n) e^{+2 pi i k n / M}, C^T = C for k >= 0 and its conjugate for k < 0,
+ * c^T(t_n) = (1/M) sum_k C^T(w_k) e^{-2 pi i k n / M}.  d_ct: [nt][nxi] complex.  nt up to about 5000. */
+int sgw_time_order(sgw_ctx* ctx, int nxi, int nt, const double* d_cr, int64_t stride_n, int64_t stride_m, void* d_ct);
+
+/* Sigma(t_n) in the xi basis (Eq. 5; R-26): d_sigma[n][k] = N_g / (nxi nfrag 32 dV) * sum_m c^T[n][m] p[n][m][k], with
+ * d_ct from sgw_time_order and d_p from sgw_td_propagate_zeta.  d_sigma: [nt][2] complex. */
+int sgw_sigma_t(sgw_ctx* ctx, int nt, int nxi, int nfrag, const void* d_ct, const void* d_p, void* d_sigma);
+
 /* Kinetic-energy cutoff ("apply an energy cutoff of 28 Hartrees to the kinetic energy operator"; it bounds
  * the spectral width and with it the number of Chebyshev terms; R-14).  ecut > 0 (Ha): from now on the kinetic operator
  * of sgw_apply_H, sgw_cheb_filter, sgw_td_propagate and sgw_spectral_bounds is F^-1 min(1/2 |k|^2, ecut) F.  That

@@ -381,6 +381,78 @@ void td_pair(const Grid& g, const double* vloc, const KBList& kb, int nvec, doub
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// NEXT-4: time-ordering of the retarded response, and the zeta pair with its sparse projections
+// ("we time-order the accumulated u^R(r,t) to produce the effective polarization potential u(r,t)"; "calling
+// the cuFFT library before and after an OpenACC kernel used for performing the complex conjugation step"; Eq. 4:
+// "propagating the filtered zeta backwards in time while simultaneously propagating its orthogonal complement forwards in
+// time"; "(N_g x 2)"; Eq. 5: <phi|Sigma(t)|phi> = (1/N_zeta) sum_zeta int phi(r) zeta(r,t) u(r,t) dr).
+// Readings R-24..R-26:
+//   * time-ordering acts on each coefficient series c^R(t_n), n < nt (real, causal: zero for t < 0), zero-padded to
+//     M = 2 nt samples: C(w_k) = sum_n c^R(t_n) e^{+i w_k t_n}, w_k = 2 pi k / (M dt), k = -M/2 .. M/2-1;
+//     C^T(w) = Re C(w) + i sgn(w) Im C(w) (= C(w) for w >= 0 and its conjugate for w < 0: the conjugation step);
+//     c^T(t_n) = (1/M) sum_k C^T(w_k) e^{-i w_k t_n}, n < nt;
+//   * the pair (psi_0 = filtered zeta, psi_1 = its complement) is propagated with the split-operator step under the
+//     frozen potential V_loc, psi_0 with -dt and psi_1 with +dt; at the start of step n the projections
+//     p[n][m][k] = dV sum_{f,j} sign * phi(point) * psi_k(point, t_n) onto the same xi_m as in td_pair are recorded;
+//   * Sigma(t_n) then is (N_g / (N_xi nfrag 32 dV)) sum_m c^T_m(t_n) p[n][m][k] (resolution of the identity in the xi
+//     basis), a contraction the tests do with numpy.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+void time_order(int nxi, int nt, const double* cr, int cr_stride_n, int cr_stride_m, double* ct) {
+    const int M = 2 * nt;
+    std::vector<C<T>> Cw(M);
+    for (int m = 0; m < nxi; ++m) {
+        for (int kk = 0; kk < M; ++kk) {
+            const int k = kk - M / 2;
+            C<T> acc(0, 0);
+            for (int n = 0; n < nt; ++n) {
+                const T ang = (T)2 * pi_v<T>() * (T)(((long long)k * n) % M) / (T)M;
+                acc += (T)cr[(size_t)n * cr_stride_n + (size_t)m * cr_stride_m] * C<T>(std::cos(ang), std::sin(ang));
+            }
+            Cw[kk] = k < 0 ? std::conj(acc) : acc;          // Re C + i sgn(w) Im C
+        }
+        for (int n = 0; n < nt; ++n) {
+            C<T> acc(0, 0);
+            for (int kk = 0; kk < M; ++kk) {
+                const int k = kk - M / 2;
+                const T ang = -(T)2 * pi_v<T>() * (T)(((long long)k * n) % M) / (T)M;
+                acc += Cw[kk] * C<T>(std::cos(ang), std::sin(ang));
+            }
+            ct[2 * ((size_t)n * nxi + m)] = (double)(acc.real() / (T)M);
+            ct[2 * ((size_t)n * nxi + m) + 1] = (double)(acc.imag() / (T)M);
+        }
+    }
+}
+
+template <class T>
+void td_zeta(const Grid& g, const double* vloc, const KBList& kb, double* pair, const double* phi, double dt, int nsteps,
+             uint64_t xi_seed, int nxi, int nfrag, double* out) {
+    const size_t ng = (size_t)g.nx * g.ny * g.nz;
+    const uint64_t nblocks = ng / XI_L;
+    const T dV = (T)g.hx * (T)g.hy * (T)g.hz;
+    for (int n = 0; n < nsteps; ++n) {
+        for (int k = 0; k < 2; ++k) {
+            const double* psi = pair + 2 * ng * k;
+            for (int m = 0; m < nxi; ++m) {
+                C<T> acc(0, 0);
+                for (int f = 0; f < nfrag; ++f) {
+                    const uint64_t b = keyed_hash(xi_seed, 2 * (uint64_t)m, (uint64_t)f) % nblocks;
+                    for (int j = 0; j < XI_L; ++j) {
+                        const T sg = (keyed_hash(xi_seed, 2 * (uint64_t)m + 1, (uint64_t)f * XI_L + j) >> 63) ? (T)-1 : (T)1;
+                        const size_t i = b * XI_L + j;
+                        acc += sg * (T)phi[i] * C<T>((T)psi[2 * i], (T)psi[2 * i + 1]);
+                    }
+                }
+                out[2 * (((size_t)n * nxi + m) * 2 + k)] = (double)(acc.real() * dV);
+                out[2 * (((size_t)n * nxi + m) * 2 + k) + 1] = (double)(acc.imag() * dV);
+            }
+        }
+        td_batch<T>(g, vloc, kb, 1, pair, -dt, 1, 0, 0.0);
+        td_batch<T>(g, vloc, kb, 1, pair + 2 * ng, dt, 1, 0, 0.0);
+    }
+}
+
 }  // namespace
 
 // =============================================================================================
@@ -542,6 +614,19 @@ void sgwo_td_pair(GRID_ARGS, const double* vloc, KB_ARGS, int nvec, double* psi,
     MK
     if (use_ld) td_pair<long double>(g, vloc, kb, nvec, psi, psi_lam, dt, nsteps, rho_scale, xi_seed, nxi, nfrag, out);
     else td_pair<double>(g, vloc, kb, nvec, psi, psi_lam, dt, nsteps, rho_scale, xi_seed, nxi, nfrag, out);
+}
+
+// cr: [nt][nxi] real (element (n, m) at cr[n * stride_n + m * stride_m]); ct: [nt][nxi] complex
+void sgwo_time_order(int nxi, int nt, const double* cr, int stride_n, int stride_m, double* ct, int use_ld) {
+    if (use_ld) time_order<long double>(nxi, nt, cr, stride_n, stride_m, ct);
+    else time_order<double>(nxi, nt, cr, stride_n, stride_m, ct);
+}
+
+void sgwo_td_zeta(GRID_ARGS, const double* vloc, KB_ARGS, double* pair, const double* phi, double dt, int nsteps, uint64_t xi_seed,
+                  int nxi, int nfrag, double* out, int use_ld) {
+    MK
+    if (use_ld) td_zeta<long double>(g, vloc, kb, pair, phi, dt, nsteps, xi_seed, nxi, nfrag, out);
+    else td_zeta<double>(g, vloc, kb, pair, phi, dt, nsteps, xi_seed, nxi, nfrag, out);
 }
 
 void sgwo_spectral_bounds(GRID_ARGS, const double* vloc, KB_ARGS, int niter, uint64_t seed, double* emin, double* emax,

@@ -183,3 +183,26 @@ def td_pair(grid, vloc, kb, psi, psi_lam, dt, nsteps, rho_scale, xi_seed, nxi, n
     lib().sgwo_td_pair(*_grid_args(grid), _p(v), *kba, C.c_int(a.shape[0]), _p(a), _p(b), C.c_double(dt), C.c_int(nsteps),
                        C.c_double(rho_scale), C.c_uint64(xi_seed), C.c_int(nxi), C.c_int(nfrag), _p(out), C.c_int(int(ld)))
     return a, b, out
+
+
+def time_order(cr, ld: bool = False):
+    """Time-ordering of retarded coefficient series cr[nt, nxi] (real) -> ct[nt, nxi] (complex); R-24."""
+    cr = np.ascontiguousarray(cr, np.float64)
+    nt, nxi = cr.shape
+    ct = np.zeros((nt, nxi), np.complex128)
+    lib().sgwo_time_order(C.c_int(nxi), C.c_int(nt), _p(cr), C.c_int(nxi), C.c_int(1), _p(ct), C.c_int(int(ld)))
+    return ct
+
+
+def td_zeta(grid, vloc, kb, pair, phi, dt, nsteps, xi_seed, nxi, nfrag, ld: bool = False):
+    """zeta pair (pair[0] backwards, pair[1] forwards, frozen V_loc) with the phi-weighted xi projections at the start of
+    every step (Eq. 5; R-25).  Returns (pair, p[nsteps, nxi, 2] complex)."""
+    pair = _vec(pair).copy()
+    assert pair.shape[0] == 2
+    kba, keep = _kb_args(kb)
+    v = None if vloc is None else np.ascontiguousarray(vloc, np.float64)
+    ph = np.ascontiguousarray(phi, np.float64)
+    out = np.zeros((nsteps, nxi, 2), np.complex128)
+    lib().sgwo_td_zeta(*_grid_args(grid), _p(v), *kba, _p(pair), _p(ph), C.c_double(dt), C.c_int(nsteps), C.c_uint64(xi_seed),
+                       C.c_int(nxi), C.c_int(nfrag), _p(out), C.c_int(int(ld)))
+    return pair, out

@@ -21,7 +21,7 @@ EXPORTS = ["sgw_init_grid", "sgw_destroy", "sgw_set_vloc", "sgw_set_nonlocal", "
            "sgw_apply_H", "sgw_cheb_filter", "sgw_hartree", "sgw_set_td", "sgw_td_propagate", "sgw_norms",
            "sgw_launch_count", "sgw_last_error", "sgw_sync_check", "sgw_spectral_bounds", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get",
            "sgw_probe_fp64", "sgw_set_kinetic_cutoff", "sgw_apply_kick",
-           "sgw_td_propagate_pair"]
+           "sgw_td_propagate_pair", "sgw_td_propagate_zeta", "sgw_time_order", "sgw_sigma_t"]
 
 
 class SGWError(RuntimeError):
@@ -61,6 +61,9 @@ def load():
         lib.sgw_set_kinetic_cutoff.argtypes = [vp, d]
         lib.sgw_apply_kick.argtypes = [vp, i, vp, vp, d]
         lib.sgw_td_propagate_pair.argtypes = [vp, i, vp, vp, d, i, u64, i, i, vp]
+        lib.sgw_td_propagate_zeta.argtypes = [vp, vp, vp, d, i, u64, i, i, vp]
+        lib.sgw_time_order.argtypes = [vp, i, i, vp, i64, i64, vp]
+        lib.sgw_sigma_t.argtypes = [vp, i, i, i, vp, vp, vp]
         _lib = lib
     return _lib
 
@@ -194,6 +197,29 @@ class Context:
         _check(self.lib.sgw_td_propagate_pair(self._h, nvec, _ptr(psi), _ptr(psi_lam), float(dt), int(nsteps), int(xi_seed),
                                               int(nxi), int(nfrag), _ptr(out)))
         return out
+
+    def sgw_td_propagate_zeta(self, pair, phi, dt, nsteps, xi_seed, nxi, nfrag):
+        assert _cvec(pair, self.ng) == 2
+        _real(phi, self.ng)
+        out = torch.empty((nsteps, nxi, 2), dtype=torch.complex128, device=self.device)
+        _check(self.lib.sgw_td_propagate_zeta(self._h, _ptr(pair), _ptr(phi), float(dt), int(nsteps), int(xi_seed), int(nxi),
+                                              int(nfrag), _ptr(out)))
+        return out
+
+    def sgw_time_order(self, cr):
+        """cr: [nt, nxi] float64 CUDA tensor (any strides) -> [nt, nxi] complex128."""
+        assert cr.dtype == torch.float64 and cr.is_cuda and cr.dim() == 2
+        nt, nxi = cr.shape
+        ct = torch.empty((nt, nxi), dtype=torch.complex128, device=self.device)
+        _check(self.lib.sgw_time_order(self._h, nxi, nt, _ptr(cr), cr.stride(0), cr.stride(1), _ptr(ct)))
+        return ct
+
+    def sgw_sigma_t(self, ct, p, nfrag):
+        nt, nxi = ct.shape
+        assert p.shape == (nt, nxi, 2) and ct.is_contiguous() and p.is_contiguous()
+        sig = torch.empty((nt, 2), dtype=torch.complex128, device=self.device)
+        _check(self.lib.sgw_sigma_t(self._h, nt, nxi, int(nfrag), _ptr(ct), _ptr(p), _ptr(sig)))
+        return sig
 
     def sgw_set_kinetic_cutoff(self, ecut):
         _check(self.lib.sgw_set_kinetic_cutoff(self._h, float(ecut)))

@@ -191,6 +191,100 @@ static __global__ void __launch_bounds__(256) xi_project_kernel(const double* __
     }
 }
 
+// ---- NEXT-4: zeta-pair projections, time-ordering, Sigma(t) (R-24..R-26) ----------------------
+// out[m * stride] = dV * sum over xi_m's fragments of sign * phi(point) * psi(point): the complex, phi-weighted form of
+// xi_project_kernel (same xi, same segments of L = 32, one atomic pair per segment).  grid (nxi), out zeroed by the caller.
+static __global__ void __launch_bounds__(256) xi_project_weighted_kernel(const cd* __restrict__ psi, const double* __restrict__ phi, long long ng,
+                                                                          uint64_t seed_mixed, int nfrag, double dV, cd* __restrict__ out,
+                                                                          int stride) {
+    const int m = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const uint64_t kpos = sm64(seed_mixed ^ (uint64_t)(2 * m)), ksgn = sm64(seed_mixed ^ (uint64_t)(2 * m + 1));
+    const uint64_t nblocks = (uint64_t)(ng / 32);
+    for (int f = warp; f < nfrag; f += nwarps) {
+        const uint64_t b = sm64(kpos ^ (uint64_t)f) % nblocks;
+        const double sg = (sm64(ksgn ^ ((uint64_t)f * 32 + lane)) >> 63) ? -1.0 : 1.0;
+        const long long i = (long long)(b * 32 + lane);
+        const cd z = psi[i];
+        const double w = sg * phi[i];
+        double ar = w * z.x, ai = w * z.y;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { ar += __shfl_down_sync(0xffffffffu, ar, o); ai += __shfl_down_sync(0xffffffffu, ai, o); }
+        if (lane == 0) {
+            double* dst = reinterpret_cast<double*>(out + (long long)m * stride);
+            atomicAdd(dst, ar * dV);
+            atomicAdd(dst + 1, ai * dV);
+        }
+    }
+}
+
+// Time-ordering of one coefficient series per block (R-24): C(w_k) = sum_n c(t_n) e^{+2 pi i k n / M} on the zero-padded
+// series (M = 2 nt), conjugate for k < 0, c^T(t_n) = (1/M) sum_k C^T(w_k) e^{-2 pi i k n / M}.  Direct sums with exactly
+// reduced angles (nt is N_tau ~ 1000 in the paper, not an FFT-friendly length; the step is a vanishing share of the
+// work: P:104).  dynamic shared memory: nt doubles + M complex.
+static __global__ void time_order_kernel(const double* __restrict__ cr, long long stride_n, long long stride_m, int nt, int nxi,
+                                         cd* __restrict__ ct) {
+    extern __shared__ double tsm[];
+    const int m = blockIdx.x, M = 2 * nt;
+    double* c = tsm;
+    cd* Cw = reinterpret_cast<cd*>(tsm + nt + (nt & 1));
+    for (int n = threadIdx.x; n < nt; n += blockDim.x) c[n] = cr[n * stride_n + m * stride_m];
+    __syncthreads();
+    for (int kk = threadIdx.x; kk < M; kk += blockDim.x) {
+        const int k = kk - M / 2;
+        double re = 0.0, im = 0.0;
+        for (int n = 0; n < nt; ++n) {
+            long long r = ((long long)k * n) % M;
+            if (r < 0) r += M;
+            double s, co;
+            sincospi(2.0 * (double)r / (double)M, &s, &co);
+            re += c[n] * co; im += c[n] * s;
+        }
+        Cw[kk] = make_double2(re, k < 0 ? -im : im);
+    }
+    __syncthreads();
+    for (int n = threadIdx.x; n < nt; n += blockDim.x) {
+        double re = 0.0, im = 0.0;
+        for (int kk = 0; kk < M; ++kk) {
+            const int k = kk - M / 2;
+            long long r = ((long long)k * n) % M;
+            if (r < 0) r += M;
+            double s, co;
+            sincospi(-2.0 * (double)r / (double)M, &s, &co);
+            const cd z = Cw[kk];
+            re += z.x * co - z.y * s; im += z.x * s + z.y * co;
+        }
+        ct[(long long)n * nxi + m] = make_double2(re / M, im / M);
+    }
+}
+
+// sigma[n][k] = norm * sum_m ct[n][m] * p[n][m][k]   (Eq. 5 in the xi basis, R-26); grid (nt), one block per time
+static __global__ void sigma_kernel(const cd* __restrict__ ct, const cd* __restrict__ p, int nxi, double norm, cd* __restrict__ sigma) {
+    const int n = blockIdx.x;
+    double a[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int m = threadIdx.x; m < nxi; m += blockDim.x) {
+        const cd c = ct[(long long)n * nxi + m];
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const cd z = p[((long long)n * nxi + m) * 2 + k];
+            a[2 * k] += c.x * z.x - c.y * z.y;
+            a[2 * k + 1] += c.x * z.y + c.y * z.x;
+        }
+    }
+    __shared__ double red[8][4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) a[q] += __shfl_down_sync(0xffffffffu, a[q], o);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5][q] = a[q];
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w][threadIdx.x];
+        reinterpret_cast<double*>(sigma + (long long)n * 2)[threadIdx.x] = t * norm;
+    }
+}
+
 // ---- a6: Kleinman-Bylander gather-dot (R-12) --------------------------------------------
 // grid (nsphere, nvec), 128 threads: c[v][s][p] = dV * sum_j beta[j][p] * psi_v[idx[j]]
 template <int NP>

@@ -444,3 +444,53 @@ extern "C" int sgw_td_propagate_pair(sgw_ctx* c, int nvec, void* d_psi, void* d_
     }
     return SGW_OK;
 }
+
+// =====================================================================================================
+// NEXT-4: zeta pair with its projections, time-ordering, Sigma(t)
+// =====================================================================================================
+extern "C" int sgw_td_propagate_zeta(sgw_ctx* c, void* d_pair, const double* d_phi, double dt, int nsteps, uint64_t xi_seed, int nxi,
+                                     int nfrag, void* d_out) {
+    if (!c || !d_pair || nsteps < 0 || nxi < 0 || nfrag < 0 || (nxi > 0 && nsteps > 0 && (!d_out || !d_phi)))
+        return set_error(SGW_EINVAL, "sgw_td_propagate_zeta: bad argument");
+    if (c->ng % 32) return set_error(SGW_ESIZE, "sgw_td_propagate_zeta: N_g must be a multiple of the segment length 32");
+    if (nsteps == 0) return SGW_OK;
+    const double dV = c->hx * c->hy * c->hz;
+    const int saved_mode = c->hartree_mode;
+    c->hartree_mode = 0;                                   // the pair moves under the frozen potential (R-25)
+    cd* pair = (cd*)d_pair;
+    cd* out = (cd*)d_out;
+    int rc = SGW_OK;
+    if (nxi > 0) rc = check_cuda(cudaMemsetAsync(d_out, 0, (size_t)nsteps * nxi * 2 * sizeof(cd), c->stream), "clear projections");
+    for (int n = 0; n < nsteps && !rc; ++n) {
+        for (int k = 0; k < 2 && !rc; ++k) {
+            if (nxi > 0) {
+                xi_project_weighted_kernel<<<nxi, 256, 0, c->stream>>>(pair + (long long)k * c->ng, d_phi, c->ng, sm64(xi_seed), nfrag, dV,
+                                                                       out + ((size_t)n * nxi) * 2 + k, 2);
+                rc = launched(c, "xi_project_weighted");
+            }
+            if (!rc) rc = sgw_td_propagate(c, 1, pair + (long long)k * c->ng, k == 0 ? -dt : dt, 1);
+        }
+    }
+    c->hartree_mode = saved_mode;
+    return rc;
+}
+
+extern "C" int sgw_time_order(sgw_ctx* c, int nxi, int nt, const double* d_cr, int64_t stride_n, int64_t stride_m, void* d_ct) {
+    if (!c || nxi < 0 || nt < 0 || (nxi > 0 && nt > 0 && (!d_cr || !d_ct))) return set_error(SGW_EINVAL, "sgw_time_order: bad argument");
+    if (nxi == 0 || nt == 0) return SGW_OK;
+    const size_t smem = (size_t)(nt + (nt & 1)) * sizeof(double) + (size_t)2 * nt * sizeof(cd);
+    if (smem > 200 * 1024) return set_error(SGW_ESIZE, "sgw_time_order: series too long (at most about 5000 samples)");
+    if (smem > 48 * 1024)
+        SGW_TRY(check_cuda(cudaFuncSetAttribute(time_order_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "time_order attribute"));
+    time_order_kernel<<<nxi, 256, smem, c->stream>>>(d_cr, stride_n, stride_m, nt, nxi, (cd*)d_ct);
+    return launched(c, "time_order");
+}
+
+extern "C" int sgw_sigma_t(sgw_ctx* c, int nt, int nxi, int nfrag, const void* d_ct, const void* d_p, void* d_sigma) {
+    if (!c || nt < 0 || nxi <= 0 || nfrag <= 0 || (nt > 0 && (!d_ct || !d_p || !d_sigma))) return set_error(SGW_EINVAL, "sgw_sigma_t: bad argument");
+    if (nt == 0) return SGW_OK;
+    const double dV = c->hx * c->hy * c->hz;
+    const double norm = (double)c->ng / ((double)nxi * (double)nfrag * 32.0 * dV);
+    sigma_kernel<<<nt, 256, 0, c->stream>>>((const cd*)d_ct, (const cd*)d_p, nxi, norm, (cd*)d_sigma);
+    return launched(c, "sigma");
+}

@@ -41,6 +41,9 @@ int main(void) {
     CHECK(sgw_profile_enable(NULL, 1) == SGW_EINVAL);
     CHECK(sgw_profile_reset(NULL) == SGW_EINVAL);
     CHECK(sgw_profile_get(NULL, 0, 0, &cnt, &ms) == SGW_EINVAL);
+    CHECK(sgw_td_propagate_zeta(NULL, NULL, NULL, 0.05, 1, 1, 1, 1, NULL) == SGW_EINVAL);
+    CHECK(sgw_time_order(NULL, 1, 1, NULL, 1, 1, NULL) == SGW_EINVAL);
+    CHECK(sgw_sigma_t(NULL, 1, 1, 1, NULL, NULL, NULL) == SGW_EINVAL);
     CHECK(sgw_set_kinetic_cutoff(NULL, 28.0) == SGW_EINVAL);
     CHECK(sgw_apply_kick(NULL, 1, NULL, NULL, 0.1) == SGW_EINVAL);
     CHECK(sgw_td_propagate_pair(NULL, 1, NULL, NULL, 0.05, 1, 1, 1, 1, NULL) == SGW_EINVAL);
@@ -80,6 +83,18 @@ int main(void) {
     CHECK(sgw_profile_enable(ctx, 0) == SGW_OK);
     CHECK(sgw_apply_kick(ctx, 2, out, vloc, 0.01) == SGW_OK);
     CHECK(sgw_td_propagate_pair(ctx, 2, psi, out, 0.05, 2, 7, 1, 3, nrm) == SGW_OK);    /* nrm: 2 steps x 1 xi x 2 = 4 doubles */
+    {   /* NEXT-4: 3 steps, 2 xi of 2 fragments */
+        void *zp = NULL, *ct = NULL, *sg = NULL;
+        double* cr = NULL;
+        CHECK(cudaMalloc(&zp, 3 * 2 * 2 * 16) == cudaSuccess && cudaMalloc(&ct, 3 * 2 * 16) == cudaSuccess);
+        CHECK(cudaMalloc(&sg, 3 * 2 * 16) == cudaSuccess && cudaMalloc((void**)&cr, 3 * 2 * 8) == cudaSuccess);
+        CHECK(cudaMemset(cr, 0, 3 * 2 * 8) == cudaSuccess);
+        CHECK(sgw_td_propagate_zeta(ctx, psi, vloc, 0.05, 3, 7, 2, 2, zp) == SGW_OK);
+        CHECK(sgw_time_order(ctx, 2, 3, cr, 2, 1, ct) == SGW_OK);
+        CHECK(sgw_sigma_t(ctx, 3, 2, 2, ct, zp, sg) == SGW_OK);
+        CHECK(sgw_sync_check(ctx) == SGW_OK);
+        cudaFree(zp); cudaFree(ct); cudaFree(sg); cudaFree(cr);
+    }
     CHECK(sgw_set_kinetic_cutoff(ctx, 5.0) == SGW_OK);
     CHECK(sgw_apply_H(ctx, 2, psi, out) == SGW_OK);
     CHECK(sgw_cheb_filter(ctx, 2, psi, coeffs, -1.0, 20.0, 3) == SGW_OK);

@@ -478,6 +478,47 @@ def test_tma_split_operator_kernel(api, torch_cuda, oracle, monkeypatch, n, nvec
     ctx.close()
 
 
+def test_zeta_pair_time_ordering_and_sigma(api, torch_cuda, oracle):
+    """NEXT-4: the zeta pair (backward / forward under the frozen potential) with its
+    phi-weighted xi projections, the time-ordering of retarded coefficient series (a length that is no FFT length: 50),
+    and the Sigma(t) contraction of Eq. 5 in the xi basis, against the oracle and numpy."""
+    torch = torch_cuda
+    n = 32
+    g = W.Grid(n, n, n, 0.5, 0.5, 0.5)
+    rng = np.random.default_rng(8)
+    centers = rng.uniform(0, 1, size=(3, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5], [0.9, 1.2, 0.8])
+    kb = W.kb_projectors(g, centers[:2], radius=1.8, sigma=0.7)
+    zbar = rng.standard_normal(g.shape) + 0j
+    occ = 0.5 * zbar + 0.2 * (rng.standard_normal(g.shape) + 1j * rng.standard_normal(g.shape))
+    pair = np.stack([occ, zbar - occ])
+    phi = rng.standard_normal(g.shape)
+    dt, nsteps, seed, nxi, nfrag = 0.05, 5, 123, 11, 4
+    ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, 2)
+    ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+    ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                         torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+    ctx.sgw_set_td(1, 0.3)                                  # the zeta call must ignore the Hartree mode (frozen potential)
+    t = torch.from_numpy(pair).cuda()
+    p = ctx.sgw_td_propagate_zeta(t, torch.from_numpy(phi).cuda(), dt, nsteps, seed, nxi, nfrag)
+    rpair, rp = oracle.td_zeta(g, vloc, kb, pair, phi, dt, nsteps, seed, nxi, nfrag, ld=True)
+    assert relerr(t.cpu().numpy(), rpair) < TOL_FULL
+    assert np.max(np.abs(p.cpu().numpy() - rp)) < 1e-10 * np.max(np.abs(rp))
+    nt = 50
+    cr = rng.standard_normal((nt, nxi, 2))
+    crd = torch.from_numpy(cr).cuda()
+    ur = crd[:, :, 1]                                       # strided view, as the pair call's output is used
+    ct = ctx.sgw_time_order(ur)
+    want = oracle.time_order(cr[:, :, 1], ld=True)
+    assert np.max(np.abs(ct.cpu().numpy() - want)) < 1e-12 * np.max(np.abs(want)) * nt
+    ctn = torch.from_numpy(want[:nsteps].copy()).cuda()
+    sig = ctx.sgw_sigma_t(ctn, p, nfrag).cpu().numpy()
+    ref = g.ng / (nxi * nfrag * 32 * g.dV) * np.einsum("nm,nmk->nk", want[:nsteps], rp)
+    assert np.max(np.abs(sig - ref)) < 1e-10 * np.max(np.abs(ref))
+    assert ctx.sgw_sync_check() == 0
+    ctx.close()
+
+
 def test_cfg2_full_length_propagation_invariants(api, torch_cuda):
     """cfg2 at full size and full length (16 vectors, 2000 steps, dt = 0.05): properties that hold at any length.
     With the Hartree term rebuilt every step the propagator stays unitary (norms conserved); with a frozen potential

@@ -488,3 +488,53 @@ def test_pair_propagation_and_xi_projection(oracle):
     for n in (1, 2):
         t = n * dt
         assert np.max(np.abs(ur[n] - t * want1)) < 0.08 * np.max(np.abs(t * want1)), (n, ur[n], t * want1)
+
+
+# ------------------------------------------------------------------ NEXT-4: time-ordering, zeta pair, Sigma(t)
+def test_time_ordering_and_zeta_pair_projections(oracle):
+    """(i) time-ordering equals the definition written with numpy.fft on the zero-padded causal series (FFT, conjugate
+    the negative frequencies, inverse FFT: P:104); (ii) a real causal series gives Re c^T(t) = c^R(t)/2 for t > 0 and
+    c^R(0) at t = 0 (the even part of the causal function), and a weakly damped oscillation 2 sin(W t) e^{-g t} gives
+    approximately i e^{-i W t} e^{-g t}: only the e^{-i W |t|} branch survives, as in a time-ordered propagator (error O(g/W)); (iii) the zeta pair follows
+    td_propagate with -dt / +dt under the frozen potential and its projections are those of a dense xi built here;
+    (iv) with enough xi the contraction of R-26 reproduces the grid integral of Eq. 5."""
+    rng = np.random.default_rng(5)
+    nt, nxi, dt = 48, 3, 0.1
+    cr = rng.standard_normal((nt, nxi))
+    ct = oracle.time_order(cr, ld=True)
+    M = 2 * nt
+    pad = np.zeros((M, nxi)); pad[:nt] = cr
+    Cw = np.fft.ifft(pad, axis=0) * M                       # sum_n c e^{+i 2 pi k n / M}
+    k = np.fft.fftfreq(M, 1.0 / M)
+    CT = np.where((k < 0)[:, None], np.conj(Cw), Cw)
+    want = np.fft.fft(CT, axis=0)[:nt] / M                  # (1/M) sum_k C^T e^{-i 2 pi k n / M}
+    assert np.max(np.abs(ct - want)) < 1e-13 * np.max(np.abs(want)) * M
+    assert np.max(np.abs(ct.real[1:] - 0.5 * cr[1:])) < 1e-12 and np.max(np.abs(ct.real[0] - cr[0])) < 1e-12
+    nt2, Wf, gam = 400, 1.3, 0.02
+    t = np.arange(nt2) * dt
+    osc = (2 * np.sin(Wf * t) * np.exp(-gam * t))[:, None]
+    cto = oracle.time_order(osc, ld=False)[:, 0]
+    ref = 1j * np.exp(-1j * Wf * t) * np.exp(-gam * t)
+    assert np.max(np.abs(cto[5:nt2 // 2] - ref[5:nt2 // 2])) < 0.06
+    # zeta pair
+    g, vloc, kb, rng2 = small_problem(8, 0.7, True)
+    zbar = rvec(rng2, g, 1)[0]
+    occ = 0.6 * zbar + 0.1 * rvec(rng2, g, 1)[0]
+    pair = np.stack([occ, zbar - occ])
+    phi = rng2.standard_normal(g.shape)
+    seed, nxi2, nfrag, nsteps = 31, 5, 3, 3
+    out_pair, p = oracle.td_zeta(g, vloc, kb, pair, phi, 0.05, nsteps, seed, nxi2, nfrag, ld=True)
+    assert np.max(np.abs(out_pair[0] - oracle.td_propagate(g, vloc, kb, pair[:1], -0.05, nsteps, 0, 0.0, ld=True)[0])) < 1e-13
+    assert np.max(np.abs(out_pair[1] - oracle.td_propagate(g, vloc, kb, pair[1:], 0.05, nsteps, 0, 0.0, ld=True)[0])) < 1e-13
+    xi = _xi_dense(g, seed, nxi2, nfrag)
+    assert np.max(np.abs(p[0, :, 0] - g.dV * xi @ (phi.ravel() * pair[0].ravel()))) < 1e-12
+    mid = oracle.td_propagate(g, vloc, kb, pair[1:], 0.05, 2, 0, 0.0, ld=True)[0]
+    assert np.max(np.abs(p[2, :, 1] - g.dV * xi @ (phi.ravel() * mid.ravel()))) < 1e-12
+    # resolution of the identity in the xi basis (R-26): many xi reproduce dV sum phi zeta u
+    nbig, nf = 4000, 4
+    u = rng2.standard_normal(g.shape)
+    xib = _xi_dense(g, 7, nbig, nf)
+    lhs = g.dV * np.sum(phi * pair[0] * u)
+    cm, pm = g.dV * xib @ u.ravel(), g.dV * xib @ (phi.ravel() * pair[0].ravel())
+    rhs = g.ng / (nbig * nf * 32 * g.dV) * np.sum(cm * pm)
+    assert abs(rhs - lhs) < 0.25 * np.sqrt(np.sum(np.abs(phi * pair[0]) ** 2) * np.sum(u ** 2)) * g.dV * np.sqrt(g.ng / (nbig * nf * 32)) * 3
