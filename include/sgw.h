@@ -30,6 +30,8 @@
  *      SGW_ACC=0|1           H apply / Chebyshev filter through the TMA accumulate kernel (bulk-tensor loads, in-place
  *                            round trip in shared memory, bulk reduce-add; cubic grids with N a multiple of 8): default
  *                            on for N >= 64, else the register-operand passes below
+ *      SGW_ACC_TD=0|1        split-operator steps through the TMA kernel of the same design (one launch per axis, bulk
+ *                            stores; cubic grids): default on from N = 256, else the plane / axis passes below
  *      SGW_ACC_L2_MB=m       accumulate kernel: one launch per term while cur + acc + v of a vector are at most m MB
  *                            (default 48), else planes (x, y tiles) then z columns in two launches
  *      SGW_LEAN_B=4|8        pencils per tile of the fused passes (default 8 when nx and ny are multiples of 8)
