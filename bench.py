@@ -51,7 +51,7 @@ def ncu_traffic(kernel_key):
         return None, None
     d = json.load(open(TRAFFIC_JSON))
     e = d.get("kernels", {}).get(kernel_key)
-    return (e["dram_bytes_per_launch"], d.get("source")) if e else (None, d.get("source"))
+    return (e["dram_bytes_per_unit"], d.get("source")) if e else (None, d.get("source"))
 
 
 class ClockSampler:
@@ -319,7 +319,8 @@ def run_gpu(args):
         units_launch = g.ng * nvec
         avg_ms = dv["ms_total"] / dv["launches"]
         ach = bpu * units_launch / (avg_ms * 1e-3) / 1e9
-        traffic, traffic_src = ncu_traffic(dn)
+        traffic_pu, traffic_src = ncu_traffic(dn)          # ncu capture at fewer vectors: scaled per grid-pt*vector
+        traffic = traffic_pu * units_launch if traffic_pu else None
         lg = math.log2(g.ng)
         cheb = bound_fraction(80.0 + 8.0 / nvec, 10.0 * lg + 20.0, units_f * args.steps, ms_f * 1e-3, peak, fp64_flops)
         td = bound_fraction(32.0 + 40.0 / nvec, 10.0 * lg + 30.0, units_t * args.steps, ms_t * 1e-3, peak, fp64_flops)
@@ -495,10 +496,24 @@ def run_other_configs(torch, api, dev, stream, args, fp64_flops):
     return out
 
 
-def write_traffic(csv_path, source):
-    """Post-processing of an ncu raw page (ncu -i <rep> --page raw --csv > csv): dram bytes per launch per kernel kind,
-    written to profiles/r02_traffic.json, which the bench line's roofline.traffic reads."""
+def write_traffic(csv_paths, source, units_per_launch):
+    """Post-processing of ncu raw pages (ncu -i <rep> --page raw --csv > csv; several files separated by commas): dram
+    bytes per launch and per grid-pt*vector for every kernel kind, written to profiles/r02_traffic.json, which the bench
+    line's roofline.traffic reads (scaled to its own units per launch)."""
     import csv
+    acc = {}
+    nacc = 0
+    for csv_path in csv_paths.split(","):
+        nacc = _traffic_rows(csv, csv_path, acc, nacc)
+    out = {"source": source, "units_per_launch_in_capture": units_per_launch,
+           "kernels": {k: {"dram_bytes_per_launch": v["bytes"] / v["launches"], "dram_bytes_per_unit": v["bytes"] / v["launches"] / units_per_launch,
+                           "avg_ms_under_ncu": v["ms"] / v["launches"], "launches": v["launches"], "kernel": v["kernel"]}
+                       for k, v in acc.items()}}
+    json.dump(out, open(TRAFFIC_JSON, "w"), indent=1)
+    print(json.dumps(out, indent=1))
+
+
+def _traffic_rows(csv, csv_path, acc, nacc):
     rows = list(csv.reader(open(csv_path)))
     hdr = rows[0]
     col = {n: i for i, n in enumerate(hdr)}
@@ -509,6 +524,8 @@ def write_traffic(csv_path, source):
     def key_of(name):
         if "acc_tma" in name:
             return "acc"
+        if "td_tma" in name:
+            return "tdk"
         cplx = False
         if "<" in name:
             args_ = name.split("<")[1].split(">")[0].replace(" ", "").replace("(bool)", "").replace("(int)", "").split(",")
@@ -528,8 +545,7 @@ def write_traffic(csv_path, source):
                 return f"{axis}_td"
             return {"x": "x_store", "y": "y_acc", "z": "z_cheb"}[axis]
         return None
-    acc = {}
-    nacc = 0
+    ntd = 0
     for r in rows[2:]:
         k = key_of(r[nm])
         if not k:
@@ -537,14 +553,16 @@ def write_traffic(csv_path, source):
         if k == "acc":                      # two launches per term: planes (y_acc), then z columns (z_cheb)
             k = "y_acc" if nacc % 2 == 0 else "z_cheb"
             nacc += 1
+        if k == "tdk":                      # three launches per step: x, y, z
+            k = ("x_td", "y_td", "z_td")[ntd % 3]
+            ntd += 1
         b = float(r[rd].replace(",", "")) * scale.get(units[rd], 1.0) + float(r[wr].replace(",", "")) * scale.get(units[wr], 1.0)
-        e = acc.setdefault(k, {"launches": 0, "bytes": 0.0, "kernel": r[nm][:120]})
+        tscale = {"ns": 1e-6, "us": 1e-3, "ms": 1.0, "s": 1e3}.get(units[dur], 1.0)
+        e = acc.setdefault(k, {"launches": 0, "bytes": 0.0, "ms": 0.0, "kernel": r[nm][:120]})
         e["launches"] += 1
         e["bytes"] += b
-    out = {"source": source, "kernels": {k: {"dram_bytes_per_launch": v["bytes"] / v["launches"], "launches": v["launches"], "kernel": v["kernel"]}
-                                          for k, v in acc.items()}}
-    json.dump(out, open(TRAFFIC_JSON, "w"), indent=1)
-    print(json.dumps(out, indent=1))
+        e["ms"] += float(r[dur].replace(",", "")) * tscale
+    return nacc
 
 
 def spawn_ranks(args):
@@ -571,9 +589,10 @@ def main():
     ap.add_argument("--write-traffic", default=None, metavar="NCU_RAW_CSV",
                     help="post-process an ncu raw page into profiles/r02_traffic.json and exit (no GPU needed)")
     ap.add_argument("--traffic-source", default="profiles/r02_cfg4_ncu.md")
+    ap.add_argument("--traffic-units", type=float, default=8 * 384.0 ** 3, help="grid-pt*vectors per launch in the ncu capture")
     args = ap.parse_args()
     if args.write_traffic:
-        write_traffic(args.write_traffic, args.traffic_source)
+        write_traffic(args.write_traffic, args.traffic_source, args.traffic_units)
         return
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         spawn_ranks(args)

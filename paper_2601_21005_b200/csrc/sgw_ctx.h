@@ -29,6 +29,9 @@ struct sgw_ctx {
     int acc_occ[4];
     int use_acc;                             // real family through the TMA accumulate kernel (SGW_ACC; default: where it is built and measured faster)
     double acc_l2_bytes;                     // one-launch terms when cur + acc + v of a vector are at most this (SGW_ACC_L2_MB)
+    const void* tmap_base[8];                // small cache of tensor maps: (array, vectors) -> y and z maps
+    int tmap_nv[8], tmap_next;
+    CUtensorMap tmap_y[8], tmap_z[8];
     void* tmap_encode;                       // cuTensorMapEncodeTiled (driver entry point)
     int lean_occ[3][18];                     // occupancy results of the lean kernels, per axis length (filled on first use)
     int lean_G, lean_ctas;                   // plane kernel: planes per CTA-owned group, CTAs per SM (0 = auto)

@@ -256,6 +256,12 @@ typedef CUresult (*tmap_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t
 // tensor maps of one vector array (nv vectors of a cubic N^3 grid, interleaved complex = pairs of doubles) for the
 // strided tiles: y tiles (8 x-adjacent pencils along y of one plane) and z tiles (8 xy-adjacent pencils along z)
 int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap* mz) {
+    // the recurrence alternates between three arrays: keep their maps (encoding costs a few microseconds per map)
+    for (int i = 0; i < 8; ++i)
+        if (c->tmap_base[i] == base && c->tmap_nv[i] == nv) { *my = c->tmap_y[i]; *mz = c->tmap_z[i]; return 0; }
+    const int slot = c->tmap_next;
+    c->tmap_next = (c->tmap_next + 1) % 8;
+    c->tmap_base[slot] = nullptr;
     const cuuint64_t N = (cuuint64_t)c->nx;
     tmap_encode_fn enc = (tmap_encode_fn)c->tmap_encode;
     const cuuint32_t nbox = (cuuint32_t)(N <= 256 ? N : N / 2);
@@ -268,6 +274,7 @@ int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap*
         r = enc(mz, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dz, sz, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return set_error(SGW_ECUDA, "cuTensorMapEncodeTiled failed: " + std::to_string((int)r));
+    c->tmap_base[slot] = base; c->tmap_nv[slot] = nv; c->tmap_y[slot] = *my; c->tmap_z[slot] = *mz;
     return 0;
 }
 

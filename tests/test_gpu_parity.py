@@ -452,3 +452,24 @@ def test_plane_pass_H_cheb_td(api, torch_cuda, oracle, monkeypatch, n, nz, nvec,
     ctx.sgw_td_propagate(t, 0.05, 4)
     assert relerr(t.cpu().numpy(), oracle.td_propagate(g, vloc, None, psi, 0.05, 4, 1, rs, ld=True)) < TOL_FULL
     ctx.close()
+
+
+def test_context_on_a_non_default_stream_with_kb(api, torch_cuda, oracle):
+    """every setup copy (sphere lists, potential) is ordered on the context's stream, also when that is a
+    non-blocking side stream and the source tensors are freed right after the call."""
+    torch = torch_cuda
+    g, vloc, kb, rng = problem(32, 32, 32, seed=77)
+    psi = rvec(rng, g, 3)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, 3, stream=side)
+        ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+        ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                             torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+        junk = [torch.full((1 << 20,), 7.0, device="cuda") for _ in range(8)]      # recycle whatever the copies read
+        del junk
+        t = torch.from_numpy(psi).cuda()
+        out = ctx.sgw_apply_H(t)
+        side.synchronize()
+    assert relerr(out.cpu().numpy(), oracle.apply_H(g, vloc, kb, psi, ld=True)) < TOL_H
+    ctx.close()
