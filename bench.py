@@ -435,8 +435,7 @@ def run_other_configs(torch, api, dev, stream, args, fp64_flops):
     # the cost of the paper's operator with its kinetic-energy cutoff (non-separable, five-pass route)
     if hasattr(ctx, "sgw_set_kinetic_cutoff"):
         ctx.sgw_set_kinetic_cutoff(28.0)
-        wc = W.make_workload("cfg1")
-        emax_c = 3 * 0 + min(28.0, 0.5 * 3 * (math.pi / w.grid.hx) ** 2) + float(wc.vloc.max())
+        emax_c = min(28.0, 1.5 * (math.pi / w.grid.hx) ** 2) + float(w.vloc.max())      # the narrower window the cutoff buys
         co = W.cheb_coeffs(W.sqrt_fermi, w.emin, emax_c, 65)
         ctx.sgw_random_vectors(W.SEED_VEC, 0, w.nvec, psi)
         msc = timed(torch, stream, dev, lambda: ctx.sgw_cheb_filter(psi, co, w.emin, emax_c))
