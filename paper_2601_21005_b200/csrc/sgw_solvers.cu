@@ -337,34 +337,24 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
     // a call reads the vectors for the density; consecutive half-step phases are merged into one table applied on
     // load (R-8)
     const bool fuse_density = c->hartree_mode && !kb;
-    const bool merged = !kb;
+    // consecutive half-step potential factors are merged into one table applied on load (R-8).  With KB the closing
+    // factor of step n and the opening one of step n+1 are adjacent as well (the KB factors sit inside them), so the
+    // merged table serves both cases.
+    const bool merged = true;
     int chunk = nvec < c->max_nvec ? nvec : c->max_nvec;
     if (!kb && c->l2_chunk > 0 && c->l2_chunk < chunk) chunk = c->l2_chunk;   // chunks small enough to stay in L2 across the passes
     for (int step = 0; step < nsteps; ++step) {
         const bool last = step + 1 == nsteps;
         if (c->hartree_mode) {
             HartreeOut o;
-            if (merged) {
-                o.merge = true; o.first = step == 0 ? 1 : 0; o.half_dt = 0.5 * dt; o.last = last ? c->phase_last : nullptr;
-                o.rho_reset = (fuse_density && !last) ? c->rho : nullptr;
-            } else {
-                o.vh = c->vh;
-            }
+            o.merge = true; o.first = step == 0 ? 1 : 0; o.half_dt = 0.5 * dt; o.last = last ? c->phase_last : nullptr;
+            o.rho_reset = (fuse_density && !last) ? c->rho : nullptr;
             SGW_TRY(hartree_into(c, nvec, psi, c->rho_scale, nullptr, fuse_density && step > 0, o));
-            if (!merged) {
-                phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, c->vh, 0.5 * dt, c->phase, ng);
-                SGW_TRY(launched(c, "phase"));
-            }
-        } else if (merged) {
+        } else if (step <= 1 || last) {
             // frozen V: the merged table is exp(-i V dt/2) in step 0 and exp(-i V dt) from step 1 on
-            if (step <= 1 || last) {
-                phase_merge_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, c->vprev, 0.5 * dt, step == 0 ? 1 : 0,
-                                                                                c->phase, last ? c->phase_last : nullptr, ng);
-                SGW_TRY(launched(c, "phase_merge"));
-            }
-        } else if (step == 0) {
-            phase_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, nullptr, 0.5 * dt, c->phase, ng);
-            SGW_TRY(launched(c, "phase"));
+            phase_merge_kernel<<<blocks_for(ng, 256), 256, 0, c->stream>>>(c->vloc, c->vprev, 0.5 * dt, step == 0 ? 1 : 0,
+                                                                            c->phase, last ? c->phase_last : nullptr, ng);
+            SGW_TRY(launched(c, "phase_merge"));
         }
         for (int cv = 0; cv < nvec; cv += chunk) {
             const int nc = (nvec - cv < chunk) ? nvec - cv : chunk;
@@ -372,9 +362,12 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             // with KB: the potential phases stay fused in the passes (on load in x, on store in z); the KB factors,
             // which sit between them, are conjugated by the phase at their sphere points instead:
             //   P (psi + conj(P) S[P psi]) = P psi + S[P psi]   and   P psi3 + P S[conj(P) (P psi3)] = P (psi3 + S[psi3])
+            // opening KB factor: conjugated by the (merged) table the x pass multiplies by on load; closing KB factor:
+            // plain, because the closing potential factor is deferred to the next step's load -- except in the last
+            // step of the call, where the z pass multiplies by phase_last on store
             if (kb) SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, +1));
             SGW_TRY(lean_td_step(c, nc, ps, false, fuse_density && !last, merged, last));
-            if (kb) SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, -1));
+            if (kb) SGW_TRY(last ? kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase_last, -1) : kb_apply(c, nc, ps, ps, 1, 0.5 * dt));
         }
     }
     return SGW_OK;
