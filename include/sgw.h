@@ -117,6 +117,25 @@ int sgw_cheb_filter(sgw_ctx* ctx, int nvec, void* d_psi, const double* h_coeffs,
  * d_rho: N_g doubles out or NULL. */
 int sgw_hartree(sgw_ctx* ctx, int nvec, const void* d_psi, double rho_scale, double* d_vh, double* d_rho);
 
+/* The same Hartree rebuild for callers that cannot allocate device memory (code under stream capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same arguments, same kernels, same five passes and the same bits as
+ * sgw_hartree, but the two scratch arrays of the solve (N_g doubles of density, N_g complex for the transforms) live in
+ * one file-scope `static __device__` array of the library instead of the context's allocations.
+ *  - Limit: grids of at most SGW_STATIC_MAX_NG = 64^3 points (the array is 24 B x 64^3 = 6 MB, held by every GPU that
+ *    loads the library until the process exits).  Larger grids: SGW_ESIZE with a message naming the limit; use sgw_hartree.
+ *  - The call launches six kernels on the context's stream and calls no cudaMalloc, cudaFree or allocating library
+ *    routine.  The context's device must be the current device (SGW_EINVAL otherwise).  The device address of the array
+ *    is resolved once per device (cudaGetSymbolAddress) by the first call on that device, or ahead of time by
+ *    sgw_static_setup (for a caller that wants nothing but launches inside a capture).
+ *  - Every call, from every context on that GPU, shares the one array: calls that can overlap on the GPU (different
+ *    streams, different contexts) RACE; serialise them.  The array keeps the last call's contents; nothing in it has
+ *    to start at zero (the density kernel and the first pass overwrite the N_g elements the solve reads).
+ * sgw_static_max_grid_points returns the limit. */
+#define SGW_STATIC_MAX_NG (64LL * 64 * 64)
+int sgw_hartree_static(sgw_ctx* ctx, int nvec, const void* d_psi, double rho_scale, double* d_vh, double* d_rho);
+int sgw_static_setup(sgw_ctx* ctx);
+int64_t sgw_static_max_grid_points(void);
+
 /* Select the time-dependent part of the propagation Hamiltonian ("time-dependent
  * Hartree"; R-9): hartree_mode 0: V = V_loc frozen; 1: V = V_loc + V_H[rho(t_n)], rebuilt at the
  * start of every step from the current vectors with the given rho_scale. */

@@ -21,7 +21,8 @@ EXPORTS = ["sgw_init_grid", "sgw_destroy", "sgw_set_vloc", "sgw_set_nonlocal", "
            "sgw_apply_H", "sgw_cheb_filter", "sgw_hartree", "sgw_set_td", "sgw_td_propagate", "sgw_norms",
            "sgw_launch_count", "sgw_last_error", "sgw_sync_check", "sgw_spectral_bounds", "sgw_profile_enable", "sgw_profile_reset", "sgw_profile_get",
            "sgw_probe_fp64", "sgw_set_kinetic_cutoff", "sgw_apply_kick",
-           "sgw_td_propagate_pair", "sgw_td_propagate_zeta", "sgw_time_order", "sgw_sigma_t"]
+           "sgw_td_propagate_pair", "sgw_td_propagate_zeta", "sgw_time_order", "sgw_sigma_t",
+           "sgw_hartree_static", "sgw_static_setup", "sgw_static_max_grid_points"]
 
 
 class SGWError(RuntimeError):
@@ -46,6 +47,10 @@ def load():
         lib.sgw_apply_H.argtypes = [vp, i, vp, vp]
         lib.sgw_cheb_filter.argtypes = [vp, i, vp, C.POINTER(d), d, d, i]
         lib.sgw_hartree.argtypes = [vp, i, vp, d, vp, vp]
+        lib.sgw_hartree_static.argtypes = [vp, i, vp, d, vp, vp]
+        lib.sgw_static_setup.argtypes = [vp]
+        lib.sgw_static_max_grid_points.argtypes = []
+        lib.sgw_static_max_grid_points.restype = i64
         lib.sgw_set_td.argtypes = [vp, i, d]
         lib.sgw_td_propagate.argtypes = [vp, i, vp, d, i]
         lib.sgw_norms.argtypes = [vp, i, vp, vp]
@@ -158,6 +163,18 @@ class Context:
         rho = torch.empty(self.shape, dtype=torch.float64, device=self.device) if want_rho else None
         _check(self.lib.sgw_hartree(self._h, nvec, _ptr(psi), float(rho_scale), _ptr(vh), _ptr(rho)))
         return (vh, rho) if want_rho else vh
+
+    def sgw_hartree_static(self, psi, rho_scale, vh, rho=None):
+        """sgw_hartree with the solve's scratch in the library's static device array; the caller passes the outputs."""
+        nvec = _cvec(psi, self.ng)
+        _check(self.lib.sgw_hartree_static(self._h, nvec, _ptr(psi), float(rho_scale), _ptr(vh), _ptr(rho)))
+        return vh
+
+    def sgw_static_setup(self):
+        _check(self.lib.sgw_static_setup(self._h))
+
+    def sgw_static_max_grid_points(self):
+        return int(self.lib.sgw_static_max_grid_points())
 
     def sgw_set_td(self, hartree_mode, rho_scale):
         _check(self.lib.sgw_set_td(self._h, int(hartree_mode), float(rho_scale)))

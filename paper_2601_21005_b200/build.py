@@ -36,7 +36,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for n in SIZES:
         jobs.append([NVCC, *FLAGS, f"-DSGW_N={n}", "-c", os.path.join(CSRC, "sgw_pass_inst.cu"),
                      "-o", os.path.join(OBJ, f"pass_{n}.o")])
-    for src in ("sgw_core.cu", "sgw_solvers.cu", "sgw_program.cu", "sgw_cut.cu"):
+    for src in ("sgw_core.cu", "sgw_solvers.cu", "sgw_program.cu", "sgw_cut.cu", "sgw_static.cu"):
         jobs.append([NVCC, *FLAGS, "-c", os.path.join(CSRC, src), "-o", os.path.join(OBJ, src[:-3] + ".o")])
     if verbose:
         for j in jobs:

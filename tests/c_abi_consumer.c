@@ -48,6 +48,9 @@ int main(void) {
     CHECK(sgw_apply_kick(NULL, 1, NULL, NULL, 0.1) == SGW_EINVAL);
     CHECK(sgw_td_propagate_pair(NULL, 1, NULL, NULL, 0.05, 1, 1, 1, 1, NULL) == SGW_EINVAL);
     CHECK(sgw_probe_fp64(NULL, &ms) == SGW_EINVAL);
+    CHECK(sgw_hartree_static(NULL, 1, NULL, 1.0, NULL, NULL) == SGW_EINVAL);
+    CHECK(sgw_static_setup(NULL) == SGW_EINVAL);
+    CHECK(sgw_static_max_grid_points() == SGW_STATIC_MAX_NG);
     CHECK(sgw_sync_check(NULL) == SGW_EINVAL);
     CHECK(sgw_launch_count(NULL) == 0);
     CHECK(sgw_destroy(NULL) == SGW_OK);
