@@ -2,6 +2,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <algorithm>
 #include <cstring>
 
 #include "sgw_ctx.h"
@@ -212,7 +213,7 @@ extern "C" int sgw_destroy(sgw_ctx* c) {
         cudaFree(c->tw[a]); cudaFree(c->kin[a]); cudaFree(c->kin_raw[a]); cudaFree(c->cheb_kin[a]); cudaFree(c->td_kin[a]);
     }
     cudaFree(c->ws[0]); cudaFree(c->ws[1]);
-    cudaFree(c->vloc); cudaFree(c->vtab); cudaFree(c->vk3d); cudaFree(c->sph_ptr); cudaFree(c->sph_idx);
+    cudaFree(c->vloc); cudaFree(c->vtab); cudaFree(c->vk3d); cudaFree(c->sph_ptr); cudaFree(c->sph_idx); cudaFree(c->sph_uniq);
     cudaFree(c->beta); cudaFree(c->D); cudaFree(c->kbc); cudaFree(c->pois); cudaFree(c->rho); cudaFree(c->vh);
     cudaFree(c->phase); cudaFree(c->phase_last); cudaFree(c->vprev); cudaFree(c->red); cudaFree(c->team_cnt); cudaFree(c->kin3d); cudaFree(c->td_kin3d); cudaFree(c->wcut);
     delete c;
@@ -335,8 +336,9 @@ extern "C" int sgw_set_nonlocal(sgw_ctx* c, int nsphere, const int64_t* d_ptr, c
     if (!c || nsphere < 0) return set_error(SGW_EINVAL, "sgw_set_nonlocal: bad argument");
     cudaStreamSynchronize(c->stream);
     sgw::drop_filter_graph(c);
-    cudaFree(c->sph_ptr); cudaFree(c->sph_idx); cudaFree(c->beta); cudaFree(c->D); cudaFree(c->kbc);
+    cudaFree(c->sph_ptr); cudaFree(c->sph_idx); cudaFree(c->beta); cudaFree(c->D); cudaFree(c->kbc); cudaFree(c->sph_uniq);
     c->sph_ptr = nullptr; c->sph_idx = nullptr; c->beta = nullptr; c->D = nullptr; c->kbc = nullptr; c->nsphere = 0;
+    c->sph_uniq = nullptr; c->nuniq = 0;
     if (nsphere == 0) return SGW_OK;
     if (!d_ptr || !d_idx || !d_beta || !d_D || nproj < 1 || nproj > 8)
         return set_error(SGW_EINVAL, "sgw_set_nonlocal: bad argument");
@@ -357,8 +359,22 @@ extern "C" int sgw_set_nonlocal(sgw_ctx* c, int nsphere, const int64_t* d_ptr, c
     if (!rc && npts) rc = check_cuda(cudaMemcpyAsync(c->sph_idx, d_idx, npts * sizeof(int32_t), cudaMemcpyDeviceToDevice, st), "copy");
     if (!rc && npts) rc = check_cuda(cudaMemcpyAsync(c->beta, d_beta, npts * nproj * sizeof(double), cudaMemcpyDeviceToDevice, st), "copy");
     if (!rc) rc = check_cuda(cudaMemcpyAsync(c->D, d_D, (size_t)nsphere * nproj * sizeof(double), cudaMemcpyDeviceToDevice, st), "copy");
+    // the distinct sphere points (spheres overlap): where the closing nonlocal factor of a propagation step changes
+    // the vectors after the last pass has accumulated their density (sgw_td_propagate)
+    std::vector<int32_t> uniq((size_t)npts);
+    if (!rc && npts) rc = check_cuda(cudaMemcpyAsync(uniq.data(), d_idx, npts * sizeof(int32_t), cudaMemcpyDeviceToHost, st), "read sph_idx");
     if (!rc) rc = check_cuda(cudaStreamSynchronize(st), "sgw_set_nonlocal");
     if (rc) return rc;
+    std::sort(uniq.begin(), uniq.end());
+    uniq.erase(std::unique(uniq.begin(), uniq.end()), uniq.end());
+    if (!uniq.empty() && (uniq.front() < 0 || uniq.back() >= c->ng)) return set_error(SGW_EINVAL, "sgw_set_nonlocal: sphere point outside the grid");
+    if (!uniq.empty()) {
+        rc = dev_alloc(&c->sph_uniq, uniq.size());
+        if (!rc) rc = check_cuda(cudaMemcpyAsync(c->sph_uniq, uniq.data(), uniq.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st), "copy");
+        if (!rc) rc = check_cuda(cudaStreamSynchronize(st), "sgw_set_nonlocal");
+        if (rc) return rc;
+    }
+    c->nuniq = (int64_t)uniq.size();
     c->nsphere = nsphere; c->nproj = nproj;
     return SGW_OK;
 }

@@ -60,6 +60,8 @@ struct sgw_ctx {
     int nsphere, nproj;
     int64_t* sph_ptr;
     int32_t* sph_idx;
+    int32_t* sph_uniq;                       // the distinct grid points of all spheres, ascending (density correction of the propagator)
+    int64_t nuniq;
     double* beta;
     double* D;
     sgw::cd* kbc;                            // [max_nvec][nsphere][nproj] projections (allocated by sgw_set_nonlocal)

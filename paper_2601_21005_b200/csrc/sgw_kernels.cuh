@@ -44,6 +44,21 @@ static __global__ void density_kernel(const cd* __restrict__ psi, int nvec, long
     if (rho2) rho2[i] = s;
 }
 
+// rho[g] += scale * sum_v |psi_v[g]|^2 at the listed (distinct) grid points only: corrects a density accumulated by the
+// last pass of a step for the points the closing nonlocal factor changes afterwards (scale < 0 before it, > 0 after)
+static __global__ void density_points_kernel(const cd* __restrict__ psi, int nvec, long long ng, const int32_t* __restrict__ pts,
+                                             long long npts, double scale, double* __restrict__ rho) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= npts) return;
+    const long long g = pts[i];
+    double s = 0.0;
+    for (int v = 0; v < nvec; ++v) {
+        const cd a = psi[(long long)v * ng + g];
+        s += a.x * a.x + a.y * a.y;
+    }
+    rho[g] += scale * s;
+}
+
 // phase[g] = exp(-i (vloc[g] + vh[g]) * half_dt)
 static __global__ void phase_kernel(const double* __restrict__ vloc, const double* __restrict__ vh, double half_dt,
                                     cd* __restrict__ phase, long long n) {

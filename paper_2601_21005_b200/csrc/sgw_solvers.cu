@@ -333,10 +333,11 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
         c->td_dt = dt; c->td_kin_valid = true;
     }
     const bool kb = c->nsphere > 0;
-    // without KB: the last pass of a step accumulates the density of its result (atomics), so only the first step of
-    // a call reads the vectors for the density; consecutive half-step phases are merged into one table applied on
-    // load (R-8)
-    const bool fuse_density = c->hartree_mode && !kb;
+    // The last pass of a step accumulates the density of its result (atomics), so only the first step of a call reads
+    // the vectors for the density.  With KB the closing nonlocal factor changes the vectors at the sphere points after that pass: the accumulated
+    // density is corrected there (minus the old values before the factor, plus the new ones after it) instead of
+    // reading all vectors again.
+    const bool fuse_density = c->hartree_mode != 0;
     // consecutive half-step potential factors are merged into one table applied on load (R-8).  With KB the closing
     // factor of step n and the opening one of step n+1 are adjacent as well (the KB factors sit inside them), so the
     // merged table serves both cases.
@@ -367,7 +368,20 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             // step of the call, where the z pass multiplies by phase_last on store
             if (kb) SGW_TRY(kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase, +1));
             SGW_TRY(lean_td_step(c, nc, ps, false, fuse_density && !last, merged, last));
+            const bool fix = kb && fuse_density && !last && c->nuniq > 0;
+            if (fix) {
+                cudaEvent_t e1 = prof_begin(c, K_DENSITY);
+                density_points_kernel<<<blocks_for(c->nuniq, 128), 128, 0, c->stream>>>(ps, nc, ng, c->sph_uniq, c->nuniq, -c->rho_scale, c->rho);
+                prof_end(c, e1);
+                SGW_TRY(launched(c, "density_points"));
+            }
             if (kb) SGW_TRY(last ? kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase_last, -1) : kb_apply(c, nc, ps, ps, 1, 0.5 * dt));
+            if (fix) {
+                cudaEvent_t e1 = prof_begin(c, K_DENSITY);
+                density_points_kernel<<<blocks_for(c->nuniq, 128), 128, 0, c->stream>>>(ps, nc, ng, c->sph_uniq, c->nuniq, c->rho_scale, c->rho);
+                prof_end(c, e1);
+                SGW_TRY(launched(c, "density_points"));
+            }
         }
     }
     return SGW_OK;
