@@ -16,7 +16,7 @@ LIB = os.path.join(HERE, "libsgw.so")
 SIZES = [8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256, 384]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "--fmad=true"]
+         "-Xcompiler", "-fPIC", "--fmad=true"] + os.environ.get("SGW_XFLAGS", "").split()
 
 
 def _newest(paths):

@@ -51,7 +51,16 @@ struct AccCfg {
     static constexpr int NOPS = N / NBOX;
     // consumer groups: as many as leave each thread ~128-146 registers
     static constexpr int NG = (GW == 1) ? 8 : (GW == 2 ? 7 : (GW <= 4 ? 3 : 2));
-    static constexpr int T = 64 + NG * GT;                   // loader warp, storer warp, consumers
+    // warp-specialised register budget (setmaxnreg): where the consumers fill whole warpgroups, the CTA is 16 warps at
+    // 128 registers, the first warpgroup (loader warp, storer warp, two idle warps) hands back all but 40 registers per
+    // thread and the consumer warpgroups take 152
+    static constexpr bool WS = (NG * GT) % 128 == 0 && NG * GT <= 384;
+    static constexpr int PRODT = WS ? 128 : 64;              // threads before the consumers
+    static constexpr int T = PRODT + NG * GT;                // loader warp, storer warp, consumers
+    // the accumulate kernel keeps the plain layout at N = 384 (measured: its x tiles lose with the larger budget)
+    static constexpr bool WS_ACC = WS && N <= 256;
+    static constexpr int PRODT_ACC = WS_ACC ? 128 : 64;
+    static constexpr int T_ACC = PRODT_ACC + NG * GT;
     static constexpr int MAXS = 24;
     // x tiles: the pointwise part w = (c vtab) cur + e v either goes through a second slot of the tile (v is brought in
     // by the loader) or, where a slot is too precious (few, large slots), is read from global memory after the inverse
@@ -264,7 +273,7 @@ __device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, cd*
 }
 
 template <int N>
-__global__ void __launch_bounds__(AccCfg<N>::T, 1)
+__global__ void __launch_bounds__(AccCfg<N>::T_ACC, 1)
 acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const __grid_constant__ CUtensorMap cur_z,
                const __grid_constant__ CUtensorMap acc_y, const __grid_constant__ CUtensorMap acc_z, int nslots) {
     using C = AccCfg<N>;
@@ -279,7 +288,7 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
     uint64_t* done = full + C::MAXS;
     uint64_t* empty = done + C::MAXS;
     const int tid = threadIdx.x;
-    for (int i = tid; i < N; i += C::T) {
+    for (int i = tid; i < N; i += C::T_ACC) {
         twA[i] = a.tw[(i % C::R2) * (i / C::R2)];
         twB[i] = a.tw[(i / C::R1) * (i % C::R1)];
 #pragma unroll
@@ -294,7 +303,8 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
     const bool usev = a.v != nullptr;
     const long long ng = (long long)N * N * a.nz;
 
-    if (tid < 64) {
+    if (tid < C::PRODT_ACC) {
+        if (C::WS_ACC) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
         if (tid == 0) {
             // ---------------- loader: one slot per tile (two for an x tile with a v operand), in tile order
             unsigned seq = 0;
@@ -365,7 +375,8 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
     }
 
     // ---------------- consumers: group g takes the CTA's tiles g, g + NG, ...
-    const int ct = tid - 64, grp = ct / GT, gt = ct % GT;
+    if (C::WS_ACC) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;\n");
+    const int ct = tid - C::PRODT_ACC, grp = ct / GT, gt = ct % GT;
     unsigned seq = 0, i = 0;
     AccIter<N> tl;
     for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next(), ++i) {
@@ -503,7 +514,9 @@ __device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, const void* s
                  "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 
-template <int N>
+// one instantiation per axis (KIND): the kind-specific address arithmetic and tile layout are compile-time, which
+// keeps the consumers within the register budget
+template <int N, int KIND>
 __global__ void __launch_bounds__(AccCfg<N>::T, 1)
 td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_z, int nslots) {
     using C = AccCfg<N>;
@@ -531,7 +544,8 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
     const unsigned S = (unsigned)nslots, nvec = (unsigned)a.nvec;
     // tile t -> block q of the vector's N*N/8 blocks (x: 8 rows; y: plane z = q / (N/8), 8 columns; z: 8 xy points), vector v;
     // vectors fastest, so that consecutive tiles read the same part of the phase table
-    if (tid < 64) {
+    if (tid < C::PRODT) {
+        if (C::WS) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
         if (tid == 0) {
             unsigned seq = 0;
             for (unsigned t = blockIdx.x; t < a.ntiles; t += gridDim.x, ++seq) {
@@ -539,15 +553,15 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
                 if (round > 0) mbar_wait(empty + s, (round - 1) & 1);
                 char* dst = slots + (size_t)s * TILE;
                 mbar_expect_tx(full + s, TILEB);
-                if (a.kind == KX) {
+                if (KIND == KX) {
                     const cd* row0 = a.psi + ((long long)v * a.nz * N + (long long)q * B) * N;
 #pragma unroll
                     for (int b = 0; b < B; ++b) bulk_load(dst + (size_t)b * C::XP * 16, row0 + b * N, ROWB, full + s);
                 } else {
-                    const CUtensorMap* m = a.kind == KY ? &map_y : &map_z;
+                    const CUtensorMap* m = KIND == KY ? &map_y : &map_z;
                     const unsigned tpp = N / 8;
-                    const int c0 = a.kind == KY ? (int)(q % tpp) * 16 : (int)q * 16;
-                    const int c2 = a.kind == KY ? (int)(v * (unsigned)a.nz + q / tpp) : (int)v;
+                    const int c0 = KIND == KY ? (int)(q % tpp) * 16 : (int)q * 16;
+                    const int c2 = KIND == KY ? (int)(v * (unsigned)a.nz + q / tpp) : (int)v;
 #pragma unroll
                     for (int o = 0; o < C::NOPS; ++o) tma_load_3d(dst + (size_t)o * C::NBOX * B * 16, m, c0, o * C::NBOX, c2, full + s);
                 }
@@ -565,15 +579,15 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
                     mbar_wait(done + s, round & 1);
                 }
                 const char* src = slots + (size_t)s * TILE;
-                if (a.kind == KX) {
+                if (KIND == KX) {
                     cd* row0 = a.psi + ((long long)v * a.nz * N + (long long)q * B) * N;
 #pragma unroll
                     for (int b = 0; b < B; ++b) bulk_store(row0 + b * N, src + (size_t)b * C::XP * 16, ROWB);
                 } else {
-                    const CUtensorMap* m = a.kind == KY ? &map_y : &map_z;
+                    const CUtensorMap* m = KIND == KY ? &map_y : &map_z;
                     const unsigned tpp = N / 8;
-                    const int c0 = a.kind == KY ? (int)(q % tpp) * 16 : (int)q * 16;
-                    const int c2 = a.kind == KY ? (int)(v * (unsigned)a.nz + q / tpp) : (int)v;
+                    const int c0 = KIND == KY ? (int)(q % tpp) * 16 : (int)q * 16;
+                    const int c2 = KIND == KY ? (int)(v * (unsigned)a.nz + q / tpp) : (int)v;
 #pragma unroll
                     for (int o = 0; o < C::NOPS; ++o) tma_store_3d(m, src + (size_t)o * C::NBOX * B * 16, c0, o * C::NBOX, c2);
                 }
@@ -589,7 +603,8 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
         }
         return;
     }
-    const int ct = tid - 64, grp = ct / GT, gt = ct % GT;
+    if (C::WS) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;\n");
+    const int ct = tid - C::PRODT, grp = ct / GT, gt = ct % GT;
     unsigned seq = (unsigned)grp;
     for (unsigned t = blockIdx.x + (unsigned)grp * gridDim.x; t < a.ntiles; t += NG * gridDim.x, seq += NG) {
         const unsigned q = t / nvec, s = seq % S, round = seq / S;
@@ -597,11 +612,11 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
         // grid index of this thread's first element and the step between its elements (phase table, density)
         long long g0;
         int gstep;
-        if (a.kind == KX) { g0 = (long long)q * (B * N) + (gt / C::R2) * N + gt % C::R2; gstep = C::R2; }
-        else if (a.kind == KY) { const unsigned tpp = N / 8, z = q / tpp, cb = q - z * tpp; g0 = (long long)z * (N * N) + cb * B + gt % B + (long long)(gt / B) * N; gstep = C::R2 * N; }
+        if (KIND == KX) { g0 = (long long)q * (B * N) + (gt / C::R2) * N + gt % C::R2; gstep = C::R2; }
+        else if (KIND == KY) { const unsigned tpp = N / 8, z = q / tpp, cb = q - z * tpp; g0 = (long long)z * (N * N) + cb * B + gt % B + (long long)(gt / B) * N; gstep = C::R2 * N; }
         else { g0 = (long long)q * B + gt % B + (long long)(gt / B) * (N * N); gstep = C::R2 * N * N; }
         mbar_wait(full + s, round & 1);
-        if (a.kind == KX) td_tile_compute<N, true>(a, tile, a.phase + g0, a.rho + g0, gstep, twA, twB, ktab, gt, grp);
+        if (KIND == KX) td_tile_compute<N, true>(a, tile, a.phase + g0, a.rho + g0, gstep, twA, twB, ktab, gt, grp);
         else td_tile_compute<N, false>(a, tile, a.phase + g0, a.rho + g0, gstep, twA, twB, ktab, gt, grp);
         if (gt == 0) mbar_arrive(done + s);
     }

@@ -186,7 +186,7 @@ static int launch_acc(const AccCall* c) {
     long long grid = c->num_sms;
     if (grid > (long long)c->args.ntiles) grid = c->args.ntiles;
     if (grid <= 0) return 0;
-    kern<<<(unsigned)grid, Cfg::T, smem, c->stream>>>(c->args, c->cur_y, c->cur_z, c->acc_y, c->acc_z, nslots);
+    kern<<<(unsigned)grid, Cfg::T_ACC, smem, c->stream>>>(c->args, c->cur_y, c->cur_z, c->acc_y, c->acc_z, nslots);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? 0 : -(4000 + (int)e);
 #else
@@ -199,16 +199,18 @@ static int launch_td(const TdCall* c) {
 #if SGW_N >= 32 && SGW_N % 8 == 0
     constexpr int N = SGW_N;
     using Cfg = AccCfg<N>;
-    auto kern = td_tma_kernel<N>;
     const int fixed = 3 * N * 16 + 3 * Cfg::MAXS * 8 + 128;
     int nslots = (227 * 1024 - fixed) / Cfg::TILE;
     if (nslots > Cfg::MAXS) nslots = Cfg::MAXS;
     if (nslots < 3) return 1;
     const size_t smem = (size_t)nslots * Cfg::TILE + fixed;
-    if (!c->occ[1]) {
+    const int kind = c->args.kind;
+    if (kind < 0 || kind > 2) return -(2000);
+    auto kern = kind == KX ? td_tma_kernel<N, KX> : (kind == KY ? td_tma_kernel<N, KY> : td_tma_kernel<N, KZ>);
+    if (!c->occ[1 + kind]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return -(1000 + (int)e);
-        c->occ[1] = 1;
+        c->occ[1 + kind] = 1;
     }
     long long grid = c->num_sms;
     if (grid > (long long)c->args.ntiles) grid = c->args.ntiles;
