@@ -58,6 +58,9 @@ struct AccCfg {
     static constexpr int PRODT = WS ? 128 : 64;              // threads before the consumers
     static constexpr int T = PRODT + NG * GT;                // loader warp, storer warp, consumers
     // the accumulate kernel keeps the plain layout at N = 384 (measured: its x tiles lose with the larger budget)
+    // split-operator x launch: how many of a thread's R1 phases stay in registers across the tiles of a block (the rest
+    // are read again for every tile); all of them where the register budget allows
+    static constexpr int NPRO = N > 256 ? R1 / 2 : R1;
     static constexpr bool WS_ACC = WS && N <= 256;
     static constexpr int PRODT_ACC = WS_ACC ? 128 : 64;
     static constexpr int T_ACC = PRODT_ACC + NG * GT;
@@ -451,10 +454,14 @@ struct TdArgs {
     unsigned ntiles;          // nvec * N * N / 8
 };
 
-template <int N, bool XK>
-__device__ __forceinline__ void td_tile_compute(const TdArgs& a, cd* tile, const cd* __restrict__ ph, double* __restrict__ rp, int gstep,
-                                                const cd* twA, const cd* twB, const cd* ktab, int gt, int bar_id) {
+// pro: the thread's phases applied on load (x launch only); racc: its sums of |psi|^2 over the vectors of the block (z
+// launch only); both live in registers across the tiles of a block
+template <int N, int KIND>
+__device__ __forceinline__ void td_tile_compute(const TdArgs& a, cd* tile, const cd* __restrict__ ph, long long gstep,
+                                                const cd* twA, const cd* twB, const cd* ktab, int gt, int bar_id,
+                                                const cd (&pro)[KIND == KX ? AccCfg<N>::NPRO : 1], double (&racc)[KIND == KZ ? AccCfg<N>::R1 : 1]) {
     using C = AccCfg<N>;
+    constexpr bool XK = KIND == KX;
     constexpr int R1 = C::R1, R2 = C::R2, TG = C::TG, GW = C::GW, GT = C::GT, TASKS = C::TASKS, ROUNDS = C::ROUNDS, B = C::B;
     constexpr bool WCACHE = R2 <= 8;
     constexpr int SB = XK ? C::XP : 1, SI = XK ? 1 : B;
@@ -465,9 +472,12 @@ __device__ __forceinline__ void td_tile_compute(const TdArgs& a, cd* tile, const
     if (actA) {
 #pragma unroll
         for (int n1 = 0; n1 < R1; ++n1) x[n1] = eA[n1 * R2 * SI];
-        if (a.flags & F_PRO) {
+        if (KIND == KX && (a.flags & F_PRO)) {
+            constexpr int NP = KIND == KX ? C::NPRO : 0;
 #pragma unroll
-            for (int n1 = 0; n1 < R1; ++n1) x[n1] = cmul(x[n1], __ldg(ph + (long long)n1 * gstep));
+            for (int n1 = NP; n1 < R1; ++n1) x[n1] = cmul(x[n1], __ldg(ph + (long long)n1 * gstep));
+#pragma unroll
+            for (int n1 = 0; n1 < NP; ++n1) x[n1] = cmul(x[n1], pro[n1]);
         }
         Dft<R1, -1>::run(x);
         if (WCACHE) {
@@ -510,14 +520,13 @@ __device__ __forceinline__ void td_tile_compute(const TdArgs& a, cd* tile, const
 #pragma unroll
         for (int j = 0; j < R1; ++j) x[j] = eA[j * R2 * SI];
         Dft<R1, +1>::run(x);
-        if (a.flags & F_EPI) {
+        if (KIND == KZ && (a.flags & F_EPI)) {               // closing factor of the last step of a call
 #pragma unroll
             for (int n1 = 0; n1 < R1; ++n1) x[n1] = cmul(x[n1], __ldg(ph + (long long)n1 * gstep));
         }
-        if (a.flags & F_DENS) {
-            const double ds = a.dens_scale;
+        if (KIND == KZ && (a.flags & F_DENS)) {
 #pragma unroll
-            for (int n1 = 0; n1 < R1; ++n1) atomicAdd(rp + (long long)n1 * gstep, ds * (x[n1].x * x[n1].x + x[n1].y * x[n1].y));
+            for (int n1 = 0; n1 < R1; ++n1) racc[KIND == KZ ? n1 : 0] += x[n1].x * x[n1].x + x[n1].y * x[n1].y;
         }
 #pragma unroll
         for (int n1 = 0; n1 < R1; ++n1) eA[n1 * R2 * SI] = x[n1];
@@ -561,15 +570,18 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     __syncthreads();
-    const unsigned S = (unsigned)nslots, nvec = (unsigned)a.nvec;
-    // tile t -> block q of the vector's N*N/8 blocks (x: 8 rows; y: plane z = q / (N/8), 8 columns; z: 8 xy points), vector v;
-    // vectors fastest, so that consecutive tiles read the same part of the phase table
+    const unsigned S = (unsigned)nslots, nvec = (unsigned)a.nvec, G = gridDim.x;
+    // Tile sequence of a CTA: block q = blockIdx.x, blockIdx.x + G, ... of a vector's N*N/8 blocks (x: 8 rows; y: plane
+    // z = q / (N/8), 8 columns; z: 8 xy points), and for each block all nvec vectors in turn.  One CTA therefore sees
+    // every vector of a block back to back: the owning thread reads its phases once per block (not once per tile) and
+    // sums |psi|^2 over the vectors in registers, one atomic per element and block; and at any moment the CTAs work on
+    // G adjacent blocks of the same few vectors (contiguous in memory).  The phase table comes from HBM once per launch.
     if (tid < C::PRODT) {
         if (C::WS) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
         if (tid == 0) {
-            unsigned seq = 0;
-            for (unsigned t = blockIdx.x; t < a.ntiles; t += gridDim.x, ++seq) {
-                const unsigned q = t / nvec, v = t - q * nvec, s = seq % S, round = seq / S;
+            unsigned seq = 0, q = blockIdx.x, v = 0;
+            for (; q < TPV; ++seq) {
+                const unsigned s = seq % S, round = seq / S;
                 if (round > 0) mbar_wait(empty + s, (round - 1) & 1);
                 char* dst = slots + (size_t)s * TILE;
                 mbar_expect_tx(full + s, TILEB);
@@ -585,11 +597,12 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
 #pragma unroll
                     for (int o = 0; o < C::NOPS; ++o) tma_load_3d(dst + (size_t)o * C::NBOX * B * 16, m, c0, o * C::NBOX, c2, full + s);
                 }
+                if (++v == nvec) { v = 0; q += G; }
             }
         } else if (tid == 32) {
-            unsigned seq = 0, pend[2], npend = 0;
-            for (unsigned t = blockIdx.x; t < a.ntiles; t += gridDim.x, ++seq) {
-                const unsigned q = t / nvec, v = t - q * nvec, s = seq % S, round = seq / S;
+            unsigned seq = 0, pend[2], npend = 0, q = blockIdx.x, v = 0;
+            for (; q < TPV; ++seq) {
+                const unsigned s = seq % S, round = seq / S;
                 if (!mbar_test(done + s, round & 1)) {
                     if (npend) {
                         bulk_wait_read<0>();
@@ -618,6 +631,7 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
                     pend[0] = pend[1]; npend = 1;
                 }
                 pend[npend++] = s;
+                if (++v == nvec) { v = 0; q += G; }
             }
             asm volatile("cp.async.bulk.wait_group 0;\n" ::: "memory");
         }
@@ -625,21 +639,52 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
     }
     if (C::WS) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;\n");
     const int ct = tid - C::PRODT, grp = ct / GT, gt = ct % GT;
-    unsigned seq = (unsigned)grp;
-    for (unsigned t = blockIdx.x + (unsigned)grp * gridDim.x; t < a.ntiles; t += NG * gridDim.x, seq += NG) {
-        const unsigned q = t / nvec, s = seq % S, round = seq / S;
+    const bool act = gt < C::TG;                              // owns elements in the first / last stage
+    // grid index of this thread's first element inside block 0 and the step between its elements (phase table, density)
+    long long goff, gstep;
+    if (KIND == KX) { goff = (long long)(gt / C::R2) * N + gt % C::R2; gstep = C::R2; }
+    else if (KIND == KY) { goff = gt % B + (long long)(gt / B) * N; gstep = (long long)C::R2 * N; }
+    else { goff = gt % B + (long long)(gt / B) * (N * N); gstep = (long long)C::R2 * N * N; }
+    auto block_base = [&](unsigned q) -> long long {
+        if (KIND == KX) return (long long)q * (B * N);
+        if (KIND == KY) { const unsigned tpp = N / 8, z = q / tpp, cb = q - z * tpp; return (long long)z * (N * N) + (long long)cb * B; }
+        return (long long)q * B;
+    };
+    constexpr int NPRO = KIND == KX ? C::NPRO : 1, NRHO = KIND == KZ ? C::R1 : 1;
+    cd pro[NPRO];
+    double racc[NRHO];
+#pragma unroll
+    for (int n1 = 0; n1 < NPRO; ++n1) pro[n1] = make_double2(1.0, 0.0);
+#pragma unroll
+    for (int n1 = 0; n1 < NRHO; ++n1) racc[n1] = 0.0;
+    auto flush = [&](unsigned q) {                            // one atomic per element for all the vectors of the block
+        if (KIND != KZ || !(a.flags & F_DENS) || !act) return;
+        double* rp = a.rho + block_base(q) + goff;
+        const double ds = a.dens_scale;
+#pragma unroll
+        for (int n1 = 0; n1 < NRHO; ++n1) { atomicAdd(rp + n1 * gstep, ds * racc[n1]); racc[n1] = 0.0; }
+    };
+    unsigned q = blockIdx.x, v = (unsigned)grp, qcur = 0xffffffffu;
+    while (v >= nvec) { v -= nvec; q += G; }
+    for (unsigned seq = (unsigned)grp; q < TPV; seq += NG) {
+        const unsigned s = seq % S, round = seq / S;
         cd* tile = reinterpret_cast<cd*>(slots + (size_t)s * TILE);
-        // grid index of this thread's first element and the step between its elements (phase table, density)
-        long long g0;
-        int gstep;
-        if (KIND == KX) { g0 = (long long)q * (B * N) + (gt / C::R2) * N + gt % C::R2; gstep = C::R2; }
-        else if (KIND == KY) { const unsigned tpp = N / 8, z = q / tpp, cb = q - z * tpp; g0 = (long long)z * (N * N) + cb * B + gt % B + (long long)(gt / B) * N; gstep = C::R2 * N; }
-        else { g0 = (long long)q * B + gt % B + (long long)(gt / B) * (N * N); gstep = C::R2 * N * N; }
+        if (q != qcur) {
+            if (qcur != 0xffffffffu) flush(qcur);
+            qcur = q;
+            if (KIND == KX && (a.flags & F_PRO) && act) {
+                const cd* ph = a.phase + block_base(q) + goff;
+#pragma unroll
+                for (int n1 = 0; n1 < NPRO; ++n1) pro[n1] = __ldg(ph + n1 * gstep);
+            }
+        }
         mbar_wait(full + s, round & 1);
-        if (KIND == KX) td_tile_compute<N, true>(a, tile, a.phase + g0, a.rho + g0, gstep, twA, twB, ktab, gt, grp);
-        else td_tile_compute<N, false>(a, tile, a.phase + g0, a.rho + g0, gstep, twA, twB, ktab, gt, grp);
+        td_tile_compute<N, KIND>(a, tile, a.phase + block_base(q) + goff, gstep, twA, twB, ktab, gt, grp, pro, racc);
         if (gt == 0) mbar_arrive(done + s);
+        v += NG;
+        while (v >= nvec) { v -= nvec; q += G; }
     }
+    if (qcur != 0xffffffffu) flush(qcur);
 }
 
 struct TdCall {

@@ -212,9 +212,9 @@ static int launch_td(const TdCall* c) {
         if (e != cudaSuccess) return -(1000 + (int)e);
         c->occ[1 + kind] = 1;
     }
-    long long grid = c->num_sms;
-    if (grid > (long long)c->args.ntiles) grid = c->args.ntiles;
-    if (grid <= 0) return 0;
+    long long grid = c->num_sms;                              // one CTA per SM; a CTA takes whole blocks (all vectors of 8 pencils)
+    if (grid > (long long)N * N / 8) grid = (long long)N * N / 8;
+    if (grid <= 0 || c->args.nvec <= 0) return 0;
     kern<<<(unsigned)grid, Cfg::T, smem, c->stream>>>(c->args, c->map_y, c->map_z, nslots);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? 0 : -(4000 + (int)e);
