@@ -301,48 +301,66 @@ static __global__ void sigma_kernel(const cd* __restrict__ ct, const cd* __restr
 }
 
 // ---- a6: Kleinman-Bylander gather-dot (R-12) --------------------------------------------
-// grid (nsphere, nvec), 128 threads: c[v][s][p] = dV * sum_j beta[j][p] * psi_v[idx[j]]
+// grid (nsphere, ceil(nvec / KB_VB)), 128 threads: c[v][s][p] = dV * sum_j beta[j][p] * psi_v[idx[j]].  A block takes
+// KB_VB vectors of one sphere: the point list, the projector values and (propagator) the phases are read once for all
+// of them.
+constexpr int KB_VB = 4;
+
 template <int NP>
-static __global__ void __launch_bounds__(128) kb_project_kernel(const cd* __restrict__ psi, long long ng,
+static __global__ void __launch_bounds__(128) kb_project_kernel(const cd* __restrict__ psi, long long ng, int nvec,
                                                                  const int64_t* __restrict__ ptr,
                                                                  const int32_t* __restrict__ idx,
                                                                  const double* __restrict__ beta, double dV,
                                                                  cd* __restrict__ cout, int nsphere,
                                                                  const cd* __restrict__ phase = nullptr, int phase_conj = 0) {
-    const int s = blockIdx.x, v = blockIdx.y;
-    const cd* p = psi + (long long)v * ng;
-    double ar[NP], ai[NP];
+    const int s = blockIdx.x, v0 = blockIdx.y * KB_VB;
+    const int nv = nvec - v0 < KB_VB ? nvec - v0 : KB_VB;
+    const cd* p = psi + (long long)v0 * ng;
+    double ar[KB_VB][NP], ai[KB_VB][NP];
 #pragma unroll
-    for (int q = 0; q < NP; ++q) ar[q] = ai[q] = 0.0;
+    for (int u = 0; u < KB_VB; ++u)
+#pragma unroll
+        for (int q = 0; q < NP; ++q) ar[u][q] = ai[u][q] = 0.0;
     for (int64_t j = ptr[s] + threadIdx.x; j < ptr[s + 1]; j += blockDim.x) {
-        cd a = p[idx[j]];
-        if (phase) {               // the projections are those of phase * psi (or conj(phase) * psi): see sgw_td_propagate
-            const cd ph = phase[idx[j]];
-            a = phase_conj ? cmulc(a, ph) : cmul(a, ph);
+        const long long g = idx[j];
+        double b[NP];
+#pragma unroll
+        for (int q = 0; q < NP; ++q) b[q] = beta[j * NP + q];
+        cd ph = make_double2(1.0, 0.0);
+        if (phase) ph = phase[g];  // the projections are those of phase * psi (or conj(phase) * psi): see sgw_td_propagate
+#pragma unroll
+        for (int u = 0; u < KB_VB; ++u) {
+            if (u < nv) {
+                cd a = p[(long long)u * ng + g];
+                if (phase) a = phase_conj ? cmulc(a, ph) : cmul(a, ph);
+#pragma unroll
+                for (int q = 0; q < NP; ++q) {
+                    ar[u][q] += b[q] * a.x;
+                    ai[u][q] += b[q] * a.y;
+                }
+            }
         }
+    }
+    __shared__ double red[4][KB_VB][2 * NP];
+#pragma unroll
+    for (int u = 0; u < KB_VB; ++u)
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
-            const double b = beta[j * NP + q];
-            ar[q] += b * a.x;
-            ai[q] += b * a.y;
-        }
-    }
-    __shared__ double red[4][2 * NP];
 #pragma unroll
-    for (int q = 0; q < NP; ++q) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            ar[q] += __shfl_down_sync(0xffffffffu, ar[q], o);
-            ai[q] += __shfl_down_sync(0xffffffffu, ai[q], o);
+            for (int o = 16; o > 0; o >>= 1) {
+                ar[u][q] += __shfl_down_sync(0xffffffffu, ar[u][q], o);
+                ai[u][q] += __shfl_down_sync(0xffffffffu, ai[u][q], o);
+            }
+            if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5][u][2 * q] = ar[u][q]; red[threadIdx.x >> 5][u][2 * q + 1] = ai[u][q]; }
         }
-        if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5][2 * q] = ar[q]; red[threadIdx.x >> 5][2 * q + 1] = ai[q]; }
-    }
     __syncthreads();
-    if (threadIdx.x < NP) {
-        const int q = threadIdx.x;
-        double re = 0.0, im = 0.0;
-        for (int w = 0; w < 4; ++w) { re += red[w][2 * q]; im += red[w][2 * q + 1]; }
-        cout[((long long)v * nsphere + s) * NP + q] = make_double2(re * dV, im * dV);
+    if (threadIdx.x < KB_VB * NP) {
+        const int u = threadIdx.x / NP, q = threadIdx.x % NP;
+        if (u < nv) {
+            double re = 0.0, im = 0.0;
+            for (int w = 0; w < 4; ++w) { re += red[w][u][2 * q]; im += red[w][u][2 * q + 1]; }
+            cout[((long long)(v0 + u) * nsphere + s) * NP + q] = make_double2(re * dV, im * dV);
+        }
     }
 }
 
@@ -350,7 +368,7 @@ static __global__ void __launch_bounds__(128) kb_project_kernel(const cd* __rest
 //   mode 0: f_p = scale * D[s][p]                         (H apply / Chebyshev term)
 //   mode 1: f_p = exp(-i D[s][p] tau) - 1                 (propagator factor NL(tau), R-11)
 template <int NP>
-static __global__ void __launch_bounds__(128) kb_scatter_kernel(cd* __restrict__ dst, long long ng,
+static __global__ void __launch_bounds__(128) kb_scatter_kernel(cd* __restrict__ dst, long long ng, int nvec,
                                                                  const int64_t* __restrict__ ptr,
                                                                  const int32_t* __restrict__ idx,
                                                                  const double* __restrict__ beta,
@@ -358,37 +376,48 @@ static __global__ void __launch_bounds__(128) kb_scatter_kernel(cd* __restrict__
                                                                  const cd* __restrict__ cin, int nsphere, int mode,
                                                                  double scale_or_tau, const cd* __restrict__ phase = nullptr,
                                                                  int phase_conj = 0) {
-    const int s = blockIdx.x, v = blockIdx.y;
-    __shared__ cd f[NP];
-    if (threadIdx.x < NP) {
-        const int q = threadIdx.x;
-        const cd c = cin[((long long)v * nsphere + s) * NP + q];
-        const double d = D[s * NP + q];
-        if (mode == 0) f[q] = cscale(c, scale_or_tau * d);
-        else {
-            double sn, cs;
-            sincos(d * scale_or_tau, &sn, &cs);
-            f[q] = cmul(make_double2(cs - 1.0, -sn), c);
+    const int s = blockIdx.x, v0 = blockIdx.y * KB_VB;
+    const int nv = nvec - v0 < KB_VB ? nvec - v0 : KB_VB;
+    __shared__ cd f[KB_VB][NP];
+    if (threadIdx.x < KB_VB * NP) {
+        const int u = threadIdx.x / NP, q = threadIdx.x % NP;
+        if (u < nv) {
+            const cd c = cin[((long long)(v0 + u) * nsphere + s) * NP + q];
+            const double d = D[s * NP + q];
+            if (mode == 0) f[u][q] = cscale(c, scale_or_tau * d);
+            else {
+                double sn, cs;
+                sincos(d * scale_or_tau, &sn, &cs);
+                f[u][q] = cmul(make_double2(cs - 1.0, -sn), c);
+            }
         }
     }
     __syncthreads();
-    double* out = reinterpret_cast<double*>(dst + (long long)v * ng);
     for (int64_t j = ptr[s] + threadIdx.x; j < ptr[s + 1]; j += blockDim.x) {
-        double re = 0.0, im = 0.0;
-#pragma unroll
-        for (int q = 0; q < NP; ++q) {
-            const double b = beta[j * NP + q];
-            re += b * f[q].x;
-            im += b * f[q].y;
-        }
         const long long g = idx[j];
-        if (phase) {               // the contribution is added to phase^-1 * (...) or phase * (...): |phase| = 1
-            const cd ph = phase[g];
-            const cd t = phase_conj ? cmulc(make_double2(re, im), ph) : cmul(make_double2(re, im), ph);
-            re = t.x; im = t.y;
+        double b[NP];
+#pragma unroll
+        for (int q = 0; q < NP; ++q) b[q] = beta[j * NP + q];
+        cd ph = make_double2(1.0, 0.0);
+        if (phase) ph = phase[g];  // the contribution is added to phase^-1 * (...) or phase * (...): |phase| = 1
+#pragma unroll
+        for (int u = 0; u < KB_VB; ++u) {
+            if (u < nv) {
+                double re = 0.0, im = 0.0;
+#pragma unroll
+                for (int q = 0; q < NP; ++q) {
+                    re += b[q] * f[u][q].x;
+                    im += b[q] * f[u][q].y;
+                }
+                if (phase) {
+                    const cd t = phase_conj ? cmulc(make_double2(re, im), ph) : cmul(make_double2(re, im), ph);
+                    re = t.x; im = t.y;
+                }
+                double* out = reinterpret_cast<double*>(dst + (long long)(v0 + u) * ng);
+                atomicAdd(out + 2 * g, re);
+                atomicAdd(out + 2 * g + 1, im);
+            }
         }
-        atomicAdd(out + 2 * g, re);
-        atomicAdd(out + 2 * g + 1, im);
     }
 }
 

@@ -44,17 +44,17 @@ int sgw::ensure_ws(sgw_ctx* c, int n) {
 namespace {
 template <int NP>
 int kb_apply_np(sgw_ctx* c, int nvec, const cd* src, cd* dst, int mode, double scale_or_tau, const cd* phase, int fold) {
-    dim3 grid(c->nsphere, nvec);
+    dim3 grid(c->nsphere, (nvec + KB_VB - 1) / KB_VB);
     const double dV = c->hx * c->hy * c->hz;
     // fold = +1: projections of phase*src, contribution times conj(phase)  (opening half step: the pass multiplies by phase on load)
     // fold = -1: projections of conj(phase)*src, contribution times phase  (closing half step: the pass multiplied by phase on store)
     cudaEvent_t e1 = prof_begin(c, K_KB_PROJECT);
-    kb_project_kernel<NP><<<grid, 128, 0, c->stream>>>(src, c->ng, c->sph_ptr, c->sph_idx, c->beta, dV, c->kbc, c->nsphere,
+    kb_project_kernel<NP><<<grid, 128, 0, c->stream>>>(src, c->ng, nvec, c->sph_ptr, c->sph_idx, c->beta, dV, c->kbc, c->nsphere,
                                                        fold ? phase : nullptr, fold < 0 ? 1 : 0);
     prof_end(c, e1);
     SGW_TRY(launched(c, "kb_project"));
     e1 = prof_begin(c, K_KB_SCATTER);
-    kb_scatter_kernel<NP><<<grid, 128, 0, c->stream>>>(dst, c->ng, c->sph_ptr, c->sph_idx, c->beta, c->D, c->kbc,
+    kb_scatter_kernel<NP><<<grid, 128, 0, c->stream>>>(dst, c->ng, nvec, c->sph_ptr, c->sph_idx, c->beta, c->D, c->kbc,
                                                        c->nsphere, mode, scale_or_tau, fold ? phase : nullptr, fold > 0 ? 1 : 0);
     prof_end(c, e1);
     return launched(c, "kb_scatter");
