@@ -175,30 +175,35 @@ def collect_passes(ctx):
         for k in range(len(KINDS)):
             n, ms = ctx.sgw_profile_get(a, k)
             if n:
-                out[f"{AXES[a]}_{KINDS[k]}" if k < 8 else KINDS[k]] = {"launches": n, "ms_total": ms}
+                name = f"{AXES[a]}_{KINDS[k]}" if k < 8 else (KINDS[k] if a == 0 else KINDS[k] + "_points")
+                out[name] = {"launches": n, "ms_total": ms}
     return out
 
 
-def pass_model(passes, nvec, n, kb_frac):
+def pass_model(passes, nvec, n, kb_frac, uniq_frac=0.0):
     """Algorithmic bytes per grid-pt*vector of each profiled launch kind and a display name.
     Filter launches: 'y_acc' + 'z_cheb' = accumulate kernel in two launches (planes: w, x, y tiles; then z tiles),
     'y_acc' alone = accumulate kernel in one launch, 'x_store' present = three register-operand axis passes."""
     acc2 = "x_store" not in passes and "z_cheb" in passes
     acc1 = "x_store" not in passes and "z_cheb" not in passes
     plane_t = "x_td" not in passes
+    tma_t = not plane_t and n >= 256
     m = {
         "x_store": (48.0 + 16.0 + 8.0 / nvec, f"axis_lean_kernel<{n},8,real,x> (x round trip, potential, recurrence, series every 2nd term)"),
         "y_acc": ((64.0 + 8.0 / nvec, f"acc_tma_kernel<{n}> (x and y tiles of whole planes: TMA loads, in-place round trips, bulk reduce-add; Clenshaw v read)") if acc2
                   else ((64.0 + 8.0 / nvec, f"acc_tma_kernel<{n}> (x, y and z tiles of whole vectors in one launch)") if acc1
                         else (48.0, f"axis_lean_kernel<{n},8,real,y> (y round trip, accumulate)"))),
         "z_cheb": (48.0, f"acc_tma_kernel<{n}> (z tiles: TMA tensor loads, bulk reduce-add)" if acc2 else f"axis_lean_kernel<{n},8,real,z> (z round trip, accumulate)"),
-        "x_td": (32.0 + 16.0 / nvec, f"axis_lean_kernel<{n},8,complex,x> (x factor of exp(-iT dt), phase on load)"),
+        "x_td": (32.0 + 16.0 / nvec, f"td_tma_kernel<{n},x> (x factor of exp(-iT dt), phases kept in registers across a block's vectors)" if tma_t
+                 else f"axis_lean_kernel<{n},8,complex,x> (x factor of exp(-iT dt), phase on load)"),
         "y_td": ((32.0 + 16.0 / nvec, f"plane kernel<{n},8,complex> (x and y factors of exp(-iT dt), team- or CTA-owned planes)") if plane_t
-                 else (32.0, f"axis_lean_kernel<{n},8,complex,y> (y factor of exp(-iT dt))")),
-        "z_td": (32.0 + 16.0 / nvec, f"axis_lean_kernel<{n},8,complex,z> (z factor, phase / density on store)"),
+                 else (32.0, f"td_tma_kernel<{n},y> (y factor of exp(-iT dt))" if tma_t else f"axis_lean_kernel<{n},8,complex,y> (y factor of exp(-iT dt))")),
+        "z_td": (32.0 + 8.0 / nvec, f"td_tma_kernel<{n},z> (z factor, density summed in registers over a block's vectors)" if tma_t
+                 else f"axis_lean_kernel<{n},8,complex,z> (z factor, phase / density on store)"),
         "kb_project": (16.0 * kb_frac + 32.0 * kb_frac / nvec, "kb_project_kernel<4> (gather-dot over sphere points)"),
         "kb_scatter": (32.0 * kb_frac + 32.0 * kb_frac / nvec, "kb_scatter_kernel<4> (FP64 atomics where spheres overlap)"),
-        "density": (16.0, "density_kernel (rho from all vectors)"),
+        "density": (16.0, "density_kernel (rho from all vectors; first step of a call only)"),
+        "density_points": (16.0 * uniq_frac + 16.0 * uniq_frac / nvec, "density_points_kernel (rho corrected at the distinct sphere points around the closing nonlocal factor)"),
     }
     return m
 
@@ -311,7 +316,8 @@ def run_gpu(args):
     if rank == 0:
         peak, peak_src = measured_peaks()
         kb_frac = float(w.kb.sph_idx.size) / g.ng
-        model = pass_model({**passes_f, **passes_t}, nvec, g.nx, kb_frac)
+        uniq_frac = float(np.unique(w.kb.sph_idx).size) / g.ng if w.kb.sph_idx.size else 0.0
+        model = pass_model({**passes_f, **passes_t}, nvec, g.nx, kb_frac, uniq_frac)
         allp = {k: dict(v, stage="filter") for k, v in passes_f.items()}
         allp.update({k: dict(v, stage="td") for k, v in passes_t.items()})
         dn, dv = max(allp.items(), key=lambda kv: kv[1]["ms_total"])
@@ -563,8 +569,9 @@ def _traffic_rows(csv, csv_path, acc, nacc):
     def key_of(name):
         if "acc_tma" in name:
             return "acc"
-        if "td_tma" in name:
-            return "tdk"
+        if "td_tma" in name:                # td_tma_kernel<N, axis>
+            ax = name.split("<")[1].split(">")[0].replace(" ", "").replace("(int)", "").split(",")
+            return {"0": "x_td", "1": "y_td", "2": "z_td"}.get(ax[1] if len(ax) > 1 else "", "tdk")
         cplx = False
         if "<" in name:
             args_ = name.split("<")[1].split(">")[0].replace(" ", "").replace("(bool)", "").replace("(int)", "").split(",")
@@ -574,6 +581,8 @@ def _traffic_rows(csv, csv_path, acc, nacc):
             return "kb_project"
         if "kb_scatter" in name:
             return "kb_scatter"
+        if "density_points" in name:
+            return "density_points"
         if "density" in name:
             return "density"
         if "plane" in name:

@@ -217,7 +217,7 @@ int64_t sgw_launch_count(const sgw_ctx* ctx);
  * H apply, 3 z pass of a Chebyshev term, 4 split-operator passes, 5 / 6 / 7 Poisson z round trip / forward /
  * inverse passes), the number of launches timed and their summed duration in ms since the last
  * sgw_profile_reset.  Booked under axis 0 as well: kind 8 / 9 the gather-dot / scatter kernels of the nonlocal term,
- * kind 10 the density kernel. */
+ * kind 10 the density kernel; under axis 1 of kind 10 its sphere-point correction in the propagator (density_points_kernel). */
 int sgw_profile_enable(sgw_ctx* ctx, int on);
 int sgw_profile_reset(sgw_ctx* ctx);
 int sgw_profile_get(sgw_ctx* ctx, int axis, int kind, int64_t* count, double* total_ms);

@@ -370,14 +370,14 @@ extern "C" int sgw_td_propagate(sgw_ctx* c, int nvec, void* d_psi, double dt, in
             SGW_TRY(lean_td_step(c, nc, ps, false, fuse_density && !last, merged, last));
             const bool fix = kb && fuse_density && !last && c->nuniq > 0;
             if (fix) {
-                cudaEvent_t e1 = prof_begin(c, K_DENSITY);
+                cudaEvent_t e1 = prof_begin(c, 1 * K_NKINDS + K_DENSITY);     // booked under axis 1 of the density kind
                 density_points_kernel<<<blocks_for(c->nuniq, 128), 128, 0, c->stream>>>(ps, nc, ng, c->sph_uniq, c->nuniq, -c->rho_scale, c->rho);
                 prof_end(c, e1);
                 SGW_TRY(launched(c, "density_points"));
             }
             if (kb) SGW_TRY(last ? kb_apply(c, nc, ps, ps, 1, 0.5 * dt, c->phase_last, -1) : kb_apply(c, nc, ps, ps, 1, 0.5 * dt));
             if (fix) {
-                cudaEvent_t e1 = prof_begin(c, K_DENSITY);
+                cudaEvent_t e1 = prof_begin(c, 1 * K_NKINDS + K_DENSITY);     // booked under axis 1 of the density kind
                 density_points_kernel<<<blocks_for(c->nuniq, 128), 128, 0, c->stream>>>(ps, nc, ng, c->sph_uniq, c->nuniq, c->rho_scale, c->rho);
                 prof_end(c, e1);
                 SGW_TRY(launched(c, "density_points"));
