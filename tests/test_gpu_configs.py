@@ -478,6 +478,44 @@ def test_tma_split_operator_kernel(api, torch_cuda, oracle, monkeypatch, n, nvec
     ctx.close()
 
 
+def test_tma_kernels_at_256_agree_with_the_register_operand_passes(api, torch_cuda, monkeypatch):
+    """256 points per axis is where the TMA kernels run in their warp-specialised layout (setmaxnreg: 16 warps, consumer
+    warpgroups at 152 registers; three consumer groups) and the split-operator kernel is the default; the oracle reaches
+    that size only on the golden samples (tests/test_gpu_golden.py: 2 vectors).  Here 5 vectors -- not a multiple of the
+    3 groups nor of the 4 vectors a KB block takes -- with KB spheres, 3 TD-Hartree steps (density summed per block in
+    the z launch, sphere-point correction) and 3 filter applications are compared with the register-operand passes
+    (SGW_ACC=0 / SGW_ACC_TD=0), which the oracle pins on the small grids and on every golden config."""
+    torch = torch_cuda
+    n, nvec = 256, 5
+    g = W.Grid(n, n, n, 0.5, 0.5, 0.5)
+    rng = np.random.default_rng(77)
+    centers = rng.uniform(0.2, 0.8, size=(6, 3)) * np.array(g.box)
+    vloc = W.gaussian_vloc(g, centers, [1.0, 2.0, 1.5, 0.7, 1.1, 1.9], [0.9, 1.2, 0.8, 1.0, 1.4, 0.7])
+    kb = W.kb_projectors(g, centers[:4], radius=2.4, sigma=0.8)
+    coeffs = np.array([0.3, -0.2, 0.15, 0.1])
+    rs = 2.0 / (nvec * g.dV) * 0.01
+    out = {}
+    for tag, acc in (("tma", "1"), ("lean", "0")):
+        monkeypatch.setenv("SGW_ACC", acc)
+        monkeypatch.setenv("SGW_ACC_TD", acc)
+        ctx = api.Context(g.nx, g.ny, g.nz, g.hx, g.hy, g.hz, nvec)
+        ctx.sgw_set_vloc(torch.from_numpy(vloc).cuda())
+        ctx.sgw_set_nonlocal(torch.from_numpy(kb.sph_ptr).cuda(), torch.from_numpy(kb.sph_idx).cuda(),
+                             torch.from_numpy(kb.beta).cuda(), torch.from_numpy(kb.D).cuda())
+        psi = ctx.sgw_random_vectors(W.SEED_VEC, 3, nvec)
+        ctx.sgw_cheb_filter(psi, coeffs, -1.0, 45.0)
+        filt = psi.clone()
+        ctx.sgw_set_td(1, rs)
+        ctx.sgw_td_propagate(psi, 0.05, 3)
+        assert ctx.sgw_sync_check() == 0
+        out[tag] = (filt.cpu().numpy(), psi.cpu().numpy())
+        ctx.close()
+        del psi, filt
+        torch.cuda.empty_cache()
+    assert relerr(out["tma"][0], out["lean"][0]) < 1e-11
+    assert relerr(out["tma"][1], out["lean"][1]) < 1e-10
+
+
 def test_zeta_pair_time_ordering_and_sigma(api, torch_cuda, oracle):
     """NEXT-4: the zeta pair (backward / forward under the frozen potential) with its
     phi-weighted xi projections, the time-ordering of retarded coefficient series (a length that is no FFT length: 50),
