@@ -1,6 +1,8 @@
 """Builds libsgw.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2601_21005_b200.build [--force]
+    python -m paper_2601_21005_b200.build [--force] [-v]
+
+SGW_XFLAGS in the environment appends extra nvcc flags (e.g. -DNAME for a one-off experiment build; use --force).
 """
 from __future__ import annotations
 
