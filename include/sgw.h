@@ -34,6 +34,8 @@
  *                            stores; cubic grids): default on from N = 256, else the plane / axis passes below
  *      SGW_ACC_L2_MB=m       accumulate kernel: one launch per term while cur + acc + v of a vector are at most m MB
  *                            (default 104: up to 128^3; the L2 holds 126 MB), else planes (x, y tiles) then z columns in two launches
+ *      SGW_ACC_PAIRZ=0|1     accumulate kernel at N = 384: z tiles in pairs (16 pencils, 256-byte rows, one tensor operation per
+ *                            pair, each of the two consumer groups takes one half); default 1
  *      SGW_LEAN_B=4|8        pencils per tile of the fused passes (default 8 when nx and ny are multiples of 8)
  *      SGW_LEAN_G=n          plane kernel: planes per CTA-owned group (default 1)
  *      SGW_LEAN_CTAS=1|2     plane kernel: one 16-warp or two 8-warp CTAs per SM (default: by L2 footprint)

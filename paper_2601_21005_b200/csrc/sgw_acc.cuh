@@ -34,6 +34,8 @@ struct AccArgs {
     int nvec, nz;             // cubic grids only: nx = ny = nz = N
     int kinds;                // bit 0: x tiles, bit 1: y tiles, bit 2: z tiles
     int plane_major;          // 1: x and y tiles interleaved plane by plane (z tiles, if any, after all planes)
+    int pairz;                // z-only launch whose tiles are PAIRS (16 xy-adjacent pencils): ntiles counts pairs, the z maps
+                              // passed have 256-byte rows, and each of the two consumer groups takes one half of a pair
     unsigned ntiles;
 };
 
@@ -65,6 +67,7 @@ struct AccCfg {
     static constexpr int PRODT_ACC = WS_ACC ? 128 : 64;
     static constexpr int T_ACC = PRODT_ACC + NG * GT;
     static constexpr int MAXS = 24;
+    static constexpr bool PAIRZ = NG == 2;                   // tile pairs need exactly two consumer groups
     // x tiles: the pointwise part w = (c vtab) cur + e v either goes through a second slot of the tile (v is brought in
     // by the loader) or, where a slot is too precious (few, large slots), is read from global memory after the inverse
     // stage (cur is an L2 hit then)
@@ -136,7 +139,7 @@ struct AccIter {
     unsigned v, p, j;
     __device__ __forceinline__ void init(const AccArgs& a, unsigned t0, unsigned stride) {
         const unsigned nk = (unsigned)((a.kinds & 1) + ((a.kinds >> 1) & 1) + ((a.kinds >> 2) & 1));
-        seg = a.plane_major ? TPP : TPV;
+        seg = a.plane_major ? TPP : (a.pairz ? TPV / 2 : TPV);
         hasx = a.kinds & 1;
         period = nk * seg;
         t = t0; step = stride;
@@ -145,6 +148,7 @@ struct AccIter {
     // x tiles are the first segment of a period when the launch has any
     __device__ __forceinline__ bool is_x() const { return hasx && q < seg; }
     __device__ __forceinline__ void decode(const AccArgs& a) {
+        if (a.pairz) { kind = 2; v = u; j = q; p = 0; return; }   // pair j of vector u: xy points [16 j, 16 j + 16)
         if (a.plane_major) {
             const unsigned k = q / TPP;
             kind = (a.kinds & 1) ? (int)k : 1;
@@ -172,14 +176,14 @@ struct AccIter {
 //   wtile (x tiles): second slot of the tile.  On entry it holds the v tile (hasv) or nothing; the thread replaces its
 //   elements by w = (c * vtab) * cur + e * v, what the x tiles add besides the transform, and reads them back after the
 //   inverse stage, so that w costs no registers across the transform.
-template <int N, bool XK>
+template <int N, bool XK, int PITCH = AccCfg<N>::B>
 __device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, cd* wtile, bool hasv, const double* __restrict__ vt, const cd* twA,
                                                  const cd* twB, const double* ktab, int gt, int bar_id, const cd* __restrict__ gcur = nullptr,
                                                  const cd* __restrict__ gv = nullptr) {
     using C = AccCfg<N>;
     constexpr int R1 = C::R1, R2 = C::R2, TG = C::TG, GW = C::GW, GT = C::GT, TASKS = C::TASKS, ROUNDS = C::ROUNDS, B = C::B;
     constexpr bool WCACHE = R2 <= 8;
-    constexpr int SB = XK ? C::XP : 1, SI = XK ? 1 : B;      // element strides of (pencil, point) inside the slot
+    constexpr int SB = XK ? C::XP : 1, SI = XK ? 1 : PITCH;  // element strides of (pencil, point) inside the slot (PITCH = 2 B: half of a tile pair)
     const bool actA = gt < TG;
     const int n2 = XK ? gt % R2 : gt / B, bA = XK ? gt / R2 : gt % B;
     cd* eA = tile + bA * SB + n2 * SI;
@@ -316,6 +320,18 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
             AccIter<N> tl;
             for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next()) {
                 tl.decode(a);
+                if (C::PAIRZ && a.pairz) {
+                    // a pair fills two adjacent slots (rows of 16 pencils = 256 bytes); only the first slot's barriers are used
+                    const unsigned s = seq % S, round = seq / S;
+                    if (round > 0) mbar_wait(empty + s, (round - 1) & 1);
+                    char* dst = slots + (size_t)s * TILE;
+                    mbar_expect_tx(full + s, 2 * YZB);
+#pragma unroll
+                    for (int o = 0; o < C::NOPS; ++o)
+                        tma_load_3d(dst + (size_t)o * C::NBOX * 2 * B * 16, &cur_z, (int)tl.j * 32, o * C::NBOX, (int)tl.v, full + s);
+                    seq += 2;
+                    continue;
+                }
                 const int nops = (tl.kind == 0 && !C::LATEW) ? 2 : 1;   // an x tile takes a second slot: the v tile, then scratch
                 for (int op = 0; op < nops; ++op, ++seq) {
                     const unsigned s = seq % S, round = seq / S;
@@ -344,7 +360,8 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
             for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next()) {
                 tl.decode(a);
                 const unsigned s = seq % S, round = seq / S;
-                seq += (tl.kind == 0 && !C::LATEW) ? 2 : 1;
+                const bool pair = C::PAIRZ && a.pairz;
+                seq += (pair || (tl.kind == 0 && !C::LATEW)) ? 2 : 1;
                 if (!mbar_test(done + s, round & 1)) {
                     // about to block: first hand back every slot whose reduce-add has been issued (with few slots the
                     // loader may need exactly those to bring in the tile this thread waits for)
@@ -355,6 +372,8 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
                     }
                     mbar_wait(done + s, round & 1);
                 }
+                if (pair) mbar_wait(done + s + 1, round & 1);            // the second group's half (it arrives on the second slot's barrier;
+                                                                         // that tile is loaded, so this wait cannot depend on the loader)
                 const char* src = slots + (size_t)s * TILE;
                 if (tl.kind == 0) {
                     cd* dst = a.acc + (long long)tl.p * (N * N) + (long long)tl.j * (B * N);
@@ -363,8 +382,13 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
                 } else {
                     const CUtensorMap* m = tl.kind == 1 ? &acc_y : &acc_z;
                     const int c2 = tl.kind == 1 ? (int)tl.p : (int)tl.v;
+                    if (pair) {
 #pragma unroll
-                    for (int o = 0; o < C::NOPS; ++o) tma_red_add_3d(m, src + (size_t)o * C::NBOX * B * 16, (int)tl.j * 16, o * C::NBOX, c2);
+                        for (int o = 0; o < C::NOPS; ++o) tma_red_add_3d(m, src + (size_t)o * C::NBOX * 2 * B * 16, (int)tl.j * 32, o * C::NBOX, c2);
+                    } else {
+#pragma unroll
+                        for (int o = 0; o < C::NOPS; ++o) tma_red_add_3d(m, src + (size_t)o * C::NBOX * B * 16, (int)tl.j * 16, o * C::NBOX, c2);
+                    }
                 }
                 bulk_commit();
                 if (npend == 2) {
@@ -426,6 +450,17 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
             process(seq);
         }
     } else {
+        if (C::PAIRZ && a.pairz) {
+            // every pair is worked on by both groups: group g takes pencils [8 g, 8 g + 8) of the 16, in place, rows 256 bytes apart
+            for (; tl.t < a.ntiles; tl.next(), seq += 2) {
+                const unsigned s = seq % S, round = seq / S;
+                cd* tile = reinterpret_cast<cd*>(slots + (size_t)s * TILE) + grp * B;
+                mbar_wait(full + s, round & 1);
+                acc_tile_compute<N, false, 2 * B>(a, tile, nullptr, false, nullptr, twA, twB, ktab + 2 * N, gt, grp);
+                if (gt == 0) mbar_arrive(done + s + grp);
+            }
+            return;
+        }
         for (; tl.t < a.ntiles; tl.next(), ++i, ++seq) {
             if ((int)(i % NG) != grp) continue;
             process(seq);

@@ -253,6 +253,7 @@ extern "C" int sgw_init_grid(sgw_ctx** out, int nx, int ny, int nz, double hx, d
     c->lean_cluster = env_int("SGW_LEAN_CLUSTER", -1);
     c->lean_team = env_int("SGW_LEAN_TEAM", -1);
     c->use_acc = env_int("SGW_ACC", -1);
+    c->acc_pairz = (nx == 384 && ny == 384) ? env_int("SGW_ACC_PAIRZ", 1) : 0;
     c->acc_l2_bytes = 1.0e6 * env_int("SGW_ACC_L2_MB", 104);   // 128^3: 101 MB, one launch 0.61 ms against 0.76 ms in two
     c->acc = (nx == ny && ny == nz && nx >= 32 && nx % 8 == 0) ? acc_launcher_for(nx) : nullptr;
     {

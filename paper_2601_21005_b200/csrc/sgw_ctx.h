@@ -27,11 +27,12 @@ struct sgw_ctx {
     sgw::td_launch_fn tdk;                   // TMA split-operator kernel (cubic grids) or NULL
     int use_acc_td;                          // complex family through it (SGW_ACC_TD; default: from 256 points per axis)
     int acc_occ[4];
+    int acc_pairz;                           // z launch of the accumulate kernel in tile pairs (N = 384; SGW_ACC_PAIRZ=0 disables)
     int use_acc;                             // real family through the TMA accumulate kernel (SGW_ACC; default: where it is built and measured faster)
     double acc_l2_bytes;                     // one-launch terms when cur + acc + v of a vector are at most this (SGW_ACC_L2_MB)
     const void* tmap_base[8];                // small cache of tensor maps: (array, vectors) -> y and z maps
     int tmap_nv[8], tmap_next;
-    CUtensorMap tmap_y[8], tmap_z[8];
+    CUtensorMap tmap_y[8], tmap_z[8], tmap_z2[8];   // z2: z tiles in pairs (16 xy-adjacent pencils, 256-byte rows)
     void* tmap_encode;                       // cuTensorMapEncodeTiled (driver entry point)
     int lean_occ[3][18];                     // occupancy results of the lean kernels, per axis length (filled on first use)
     int lean_G, lean_ctas;                   // plane kernel: planes per CTA-owned group, CTAs per SM (0 = auto)

@@ -255,17 +255,21 @@ typedef CUresult (*tmap_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t
 
 // tensor maps of one vector array (nv vectors of a cubic N^3 grid, interleaved complex = pairs of doubles) for the
 // strided tiles: y tiles (8 x-adjacent pencils along y of one plane) and z tiles (8 xy-adjacent pencils along z)
-int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap* mz) {
+int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap* mz, CUtensorMap* mz2 = nullptr) {
     // the recurrence alternates between three arrays: keep their maps (encoding costs a few microseconds per map)
     for (int i = 0; i < 8; ++i)
-        if (c->tmap_base[i] == base && c->tmap_nv[i] == nv) { *my = c->tmap_y[i]; *mz = c->tmap_z[i]; return 0; }
+        if (c->tmap_base[i] == base && c->tmap_nv[i] == nv) {
+            *my = c->tmap_y[i]; *mz = c->tmap_z[i];
+            if (mz2) *mz2 = c->tmap_z2[i];
+            return 0;
+        }
     const int slot = c->tmap_next;
     c->tmap_next = (c->tmap_next + 1) % 8;
     c->tmap_base[slot] = nullptr;
     const cuuint64_t N = (cuuint64_t)c->nx;
     tmap_encode_fn enc = (tmap_encode_fn)c->tmap_encode;
     const cuuint32_t nbox = (cuuint32_t)(N <= 256 ? N : N / 2);
-    const cuuint32_t box[3] = {16, nbox, 1}, es[3] = {1, 1, 1};
+    const cuuint32_t box[3] = {16, nbox, 1}, box2[3] = {32, nbox, 1}, es[3] = {1, 1, 1};
     const cuuint64_t dy[3] = {2 * N, N, N * (cuuint64_t)nv}, sy[2] = {N * 16, N * N * 16};
     const cuuint64_t dz[3] = {2 * N * N, N, (cuuint64_t)nv}, sz[2] = {N * N * 16, N * N * N * 16};
     CUresult r = enc(my, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dy, sy, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -273,8 +277,13 @@ int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap*
     if (r == CUDA_SUCCESS)
         r = enc(mz, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dz, sz, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUtensorMap z2;
+    if (r == CUDA_SUCCESS)
+        r = enc(&z2, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dz, sz, box2, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return set_error(SGW_ECUDA, "cuTensorMapEncodeTiled failed: " + std::to_string((int)r));
-    c->tmap_base[slot] = base; c->tmap_nv[slot] = nv; c->tmap_y[slot] = *my; c->tmap_z[slot] = *mz;
+    c->tmap_base[slot] = base; c->tmap_nv[slot] = nv; c->tmap_y[slot] = *my; c->tmap_z[slot] = *mz; c->tmap_z2[slot] = z2;
+    if (mz2) *mz2 = z2;
     return 0;
 }
 
@@ -315,6 +324,7 @@ struct AccOp {
     const double* vtab;
     const double* kre[3];
     double c, e;
+    int pairz;                // z-only launch with tiles in pairs (the z maps passed are the pair maps)
 };
 
 int acc_launch_one(sgw_ctx* c, int nv, const AccOp& op, const AccCall& maps, int kinds, int plane_major, int prof_tag) {
@@ -328,7 +338,8 @@ int acc_launch_one(sgw_ctx* c, int nv, const AccOp& op, const AccCall& maps, int
     a.nvec = nv; a.nz = c->nz;
     a.kinds = kinds; a.plane_major = plane_major;
     const long long n = c->nx, tpv = n * n / 8, nk = (kinds & 1) + ((kinds >> 1) & 1) + ((kinds >> 2) & 1);
-    const long long ntiles = plane_major ? nk * (n / 8) * c->nz * nv : nk * tpv * nv;
+    a.pairz = op.pairz;
+    const long long ntiles = plane_major ? nk * (n / 8) * c->nz * nv : (op.pairz ? tpv / 2 * nv : nk * tpv * nv);
     if (ntiles > 0xffffffffLL - 1024) return set_error(SGW_EINVAL, "too many tiles for one launch");
     a.ntiles = (unsigned)ntiles;
     call.num_sms = c->num_sms;
@@ -355,6 +366,18 @@ int acc_apply(sgw_ctx* c, int nv, const AccOp& op, int z_tag) {
     const double per_vec = 16.0 * (double)c->ng * (op.v ? 3.0 : 2.0);
     if (per_vec <= c->acc_l2_bytes) return acc_launch_one(c, nv, op, maps, 7, 0, 1 * K_NKINDS + K_RT_ACC);
     SGW_TRY(acc_launch_one(c, nv, op, maps, 3, 1, 1 * K_NKINDS + K_RT_ACC));
+    // z launch: where two consumer groups work side by side (N = 384) a tile pair (16 xy-adjacent pencils, 256-byte
+    // rows) is loaded and reduce-added as one tensor operation and each group takes one half: the strided rows are what
+    // bounds this launch, and 256-byte rows move at 6.3 TB/s where 128-byte rows reach 4.9
+    if (c->acc_pairz) {
+        AccOp op2 = op;
+        op2.pairz = 1;
+        AccCall m2 = maps;
+        CUtensorMap dummy_y, dummy_z;
+        SGW_TRY(acc_maps(c, op.cur, nv, &dummy_y, &dummy_z, &m2.cur_z));
+        SGW_TRY(acc_maps(c, op.acc, nv, &dummy_y, &dummy_z, &m2.acc_z));
+        return acc_launch_one(c, nv, op2, m2, 4, 0, 2 * K_NKINDS + z_tag);
+    }
     return acc_launch_one(c, nv, op, maps, 4, 0, 2 * K_NKINDS + z_tag);
 }
 
