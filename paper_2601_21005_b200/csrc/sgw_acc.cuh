@@ -499,7 +499,7 @@ __device__ __forceinline__ void td_tile_compute(const TdArgs& a, cd* tile, const
     constexpr bool XK = KIND == KX;
     constexpr int R1 = C::R1, R2 = C::R2, TG = C::TG, GW = C::GW, GT = C::GT, TASKS = C::TASKS, ROUNDS = C::ROUNDS, B = C::B;
     constexpr bool WCACHE = R2 <= 8;
-    constexpr int SB = XK ? C::XP : 1, SI = XK ? 1 : B;
+    constexpr int SB = XK ? C::XP : 1, SI = XK ? 1 : ((C::PAIRZ && !XK) ? 2 * B : B);   // y / z tiles in pairs: rows of 16 pencils
     const bool actA = gt < TG;
     const int n2 = XK ? gt % R2 : gt / B, bA = XK ? gt / R2 : gt % B;
     cd* eA = tile + bA * SB + n2 * SI;
@@ -606,37 +606,43 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
     }
     __syncthreads();
     const unsigned S = (unsigned)nslots, nvec = (unsigned)a.nvec, G = gridDim.x;
-    // Tile sequence of a CTA: block q = blockIdx.x, blockIdx.x + G, ... of a vector's N*N/8 blocks (x: 8 rows; y: plane
-    // z = q / (N/8), 8 columns; z: 8 xy points), and for each block all nvec vectors in turn.  One CTA therefore sees
-    // every vector of a block back to back: the owning thread reads its phases once per block (not once per tile) and
-    // sums |psi|^2 over the vectors in registers, one atomic per element and block; and at any moment the CTAs work on
-    // G adjacent blocks of the same few vectors (contiguous in memory).  The phase table comes from HBM once per launch.
+    // Tile sequence of a CTA: block q = blockIdx.x, blockIdx.x + G, ... of a vector's blocks (x: 8 rows; y: plane z, 8
+    // columns; z: 8 xy points), and for each block all nvec vectors in turn.  One CTA therefore sees every vector of a
+    // block back to back: the owning thread reads its phases once per block (not once per tile) and sums |psi|^2 over the
+    // vectors in registers, one atomic per element and block; and at any moment the CTAs work on G adjacent blocks of the
+    // same few vectors (contiguous in memory).  The phase table comes from HBM once per launch.
+    // PAIR (y and z launches with two consumer groups, N = 384): a block is 16 pencils, loaded and stored as one tensor
+    // operation with 256-byte rows into two adjacent slots; both groups work on every tile, each on its 8 pencils (the
+    // strided 128-byte rows are what bounds these launches; only the first slot's full / empty barriers are used, group g
+    // arrives on done[s + g]).
+    constexpr bool PAIR = C::PAIRZ && KIND != KX;
+    constexpr unsigned NBLK = PAIR ? TPV / 2 : TPV, STEP = PAIR ? 2 : 1, PB = PAIR ? 2 * B : B;
+    constexpr unsigned TPPB = N / PB;                          // y blocks per plane
     if (tid < C::PRODT) {
         if (C::WS) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
         if (tid == 0) {
             unsigned seq = 0, q = blockIdx.x, v = 0;
-            for (; q < TPV; ++seq) {
+            for (; q < NBLK; seq += STEP) {
                 const unsigned s = seq % S, round = seq / S;
                 if (round > 0) mbar_wait(empty + s, (round - 1) & 1);
                 char* dst = slots + (size_t)s * TILE;
-                mbar_expect_tx(full + s, TILEB);
+                mbar_expect_tx(full + s, STEP * TILEB);
                 if (KIND == KX) {
                     const cd* row0 = a.psi + ((long long)v * a.nz * N + (long long)q * B) * N;
 #pragma unroll
                     for (int b = 0; b < B; ++b) bulk_load(dst + (size_t)b * C::XP * 16, row0 + b * N, ROWB, full + s);
                 } else {
                     const CUtensorMap* m = KIND == KY ? &map_y : &map_z;
-                    const unsigned tpp = N / 8;
-                    const int c0 = KIND == KY ? (int)(q % tpp) * 16 : (int)q * 16;
-                    const int c2 = KIND == KY ? (int)(v * (unsigned)a.nz + q / tpp) : (int)v;
+                    const int c0 = KIND == KY ? (int)(q % TPPB) * (2 * PB) : (int)q * (2 * PB);
+                    const int c2 = KIND == KY ? (int)(v * (unsigned)a.nz + q / TPPB) : (int)v;
 #pragma unroll
-                    for (int o = 0; o < C::NOPS; ++o) tma_load_3d(dst + (size_t)o * C::NBOX * B * 16, m, c0, o * C::NBOX, c2, full + s);
+                    for (int o = 0; o < C::NOPS; ++o) tma_load_3d(dst + (size_t)o * C::NBOX * PB * 16, m, c0, o * C::NBOX, c2, full + s);
                 }
                 if (++v == nvec) { v = 0; q += G; }
             }
         } else if (tid == 32) {
             unsigned seq = 0, pend[2], npend = 0, q = blockIdx.x, v = 0;
-            for (; q < TPV; ++seq) {
+            for (; q < NBLK; seq += STEP) {
                 const unsigned s = seq % S, round = seq / S;
                 if (!mbar_test(done + s, round & 1)) {
                     if (npend) {
@@ -646,6 +652,7 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
                     }
                     mbar_wait(done + s, round & 1);
                 }
+                if (PAIR) mbar_wait(done + s + 1, round & 1);          // the second group's half (loaded already: cannot depend on the loader)
                 const char* src = slots + (size_t)s * TILE;
                 if (KIND == KX) {
                     cd* row0 = a.psi + ((long long)v * a.nz * N + (long long)q * B) * N;
@@ -653,11 +660,10 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
                     for (int b = 0; b < B; ++b) bulk_store(row0 + b * N, src + (size_t)b * C::XP * 16, ROWB);
                 } else {
                     const CUtensorMap* m = KIND == KY ? &map_y : &map_z;
-                    const unsigned tpp = N / 8;
-                    const int c0 = KIND == KY ? (int)(q % tpp) * 16 : (int)q * 16;
-                    const int c2 = KIND == KY ? (int)(v * (unsigned)a.nz + q / tpp) : (int)v;
+                    const int c0 = KIND == KY ? (int)(q % TPPB) * (2 * PB) : (int)q * (2 * PB);
+                    const int c2 = KIND == KY ? (int)(v * (unsigned)a.nz + q / TPPB) : (int)v;
 #pragma unroll
-                    for (int o = 0; o < C::NOPS; ++o) tma_store_3d(m, src + (size_t)o * C::NBOX * B * 16, c0, o * C::NBOX, c2);
+                    for (int o = 0; o < C::NOPS; ++o) tma_store_3d(m, src + (size_t)o * C::NBOX * PB * 16, c0, o * C::NBOX, c2);
                 }
                 bulk_commit();
                 if (npend == 2) {
@@ -675,15 +681,16 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
     if (C::WS) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;\n");
     const int ct = tid - C::PRODT, grp = ct / GT, gt = ct % GT;
     const bool act = gt < C::TG;                              // owns elements in the first / last stage
+    const int half = PAIR ? grp * B : 0;                      // this group's pencils inside a pair
     // grid index of this thread's first element inside block 0 and the step between its elements (phase table, density)
     long long goff, gstep;
     if (KIND == KX) { goff = (long long)(gt / C::R2) * N + gt % C::R2; gstep = C::R2; }
-    else if (KIND == KY) { goff = gt % B + (long long)(gt / B) * N; gstep = (long long)C::R2 * N; }
-    else { goff = gt % B + (long long)(gt / B) * (N * N); gstep = (long long)C::R2 * N * N; }
+    else if (KIND == KY) { goff = half + gt % B + (long long)(gt / B) * N; gstep = (long long)C::R2 * N; }
+    else { goff = half + gt % B + (long long)(gt / B) * (N * N); gstep = (long long)C::R2 * N * N; }
     auto block_base = [&](unsigned q) -> long long {
         if (KIND == KX) return (long long)q * (B * N);
-        if (KIND == KY) { const unsigned tpp = N / 8, z = q / tpp, cb = q - z * tpp; return (long long)z * (N * N) + (long long)cb * B; }
-        return (long long)q * B;
+        if (KIND == KY) { const unsigned z = q / TPPB, cb = q - z * TPPB; return (long long)z * (N * N) + (long long)cb * PB; }
+        return (long long)q * PB;
     };
     constexpr int NPRO = KIND == KX ? C::NPRO : 1, NRHO = KIND == KZ ? C::R1 : 1;
     cd pro[NPRO];
@@ -699,11 +706,13 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
 #pragma unroll
         for (int n1 = 0; n1 < NRHO; ++n1) { atomicAdd(rp + n1 * gstep, ds * racc[n1]); racc[n1] = 0.0; }
     };
-    unsigned q = blockIdx.x, v = (unsigned)grp, qcur = 0xffffffffu;
+    // without pairs group g takes the CTA's tiles g, g + NG, ...; with pairs both groups take every tile
+    unsigned q = blockIdx.x, v = PAIR ? 0u : (unsigned)grp, qcur = 0xffffffffu;
+    constexpr unsigned VSTEP = PAIR ? 1 : NG;
     while (v >= nvec) { v -= nvec; q += G; }
-    for (unsigned seq = (unsigned)grp; q < TPV; seq += NG) {
+    for (unsigned seq = PAIR ? 0u : (unsigned)grp; q < NBLK; seq += PAIR ? 2 : NG) {
         const unsigned s = seq % S, round = seq / S;
-        cd* tile = reinterpret_cast<cd*>(slots + (size_t)s * TILE);
+        cd* tile = reinterpret_cast<cd*>(slots + (size_t)s * TILE) + half;
         if (q != qcur) {
             if (qcur != 0xffffffffu) flush(qcur);
             qcur = q;
@@ -715,8 +724,8 @@ td_tma_kernel(const TdArgs a, const __grid_constant__ CUtensorMap map_y, const _
         }
         mbar_wait(full + s, round & 1);
         td_tile_compute<N, KIND>(a, tile, a.phase + block_base(q) + goff, gstep, twA, twB, ktab, gt, grp, pro, racc);
-        if (gt == 0) mbar_arrive(done + s);
-        v += NG;
+        if (gt == 0) mbar_arrive(done + s + (PAIR ? grp : 0));
+        v += VSTEP;
         while (v >= nvec) { v -= nvec; q += G; }
     }
     if (qcur != 0xffffffffu) flush(qcur);

@@ -32,7 +32,7 @@ struct sgw_ctx {
     double acc_l2_bytes;                     // one-launch terms when cur + acc + v of a vector are at most this (SGW_ACC_L2_MB)
     const void* tmap_base[8];                // small cache of tensor maps: (array, vectors) -> y and z maps
     int tmap_nv[8], tmap_next;
-    CUtensorMap tmap_y[8], tmap_z[8], tmap_z2[8];   // z2: z tiles in pairs (16 xy-adjacent pencils, 256-byte rows)
+    CUtensorMap tmap_y[8], tmap_z[8], tmap_z2[8], tmap_y2[8];   // z2 / y2: tiles in pairs (16 adjacent pencils, 256-byte rows)
     void* tmap_encode;                       // cuTensorMapEncodeTiled (driver entry point)
     int lean_occ[3][18];                     // occupancy results of the lean kernels, per axis length (filled on first use)
     int lean_G, lean_ctas;                   // plane kernel: planes per CTA-owned group, CTAs per SM (0 = auto)

@@ -213,7 +213,8 @@ static int launch_td(const TdCall* c) {
         c->occ[1 + kind] = 1;
     }
     long long grid = c->num_sms;                              // one CTA per SM; a CTA takes whole blocks (all vectors of 8 pencils)
-    if (grid > (long long)N * N / 8) grid = (long long)N * N / 8;
+    const long long nblk = (Cfg::PAIRZ && kind != KX) ? (long long)N * N / 16 : (long long)N * N / 8;
+    if (grid > nblk) grid = nblk;
     if (grid <= 0 || c->args.nvec <= 0) return 0;
     kern<<<(unsigned)grid, Cfg::T, smem, c->stream>>>(c->args, c->map_y, c->map_z, nslots);
     cudaError_t e = cudaGetLastError();

@@ -255,12 +255,13 @@ typedef CUresult (*tmap_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t
 
 // tensor maps of one vector array (nv vectors of a cubic N^3 grid, interleaved complex = pairs of doubles) for the
 // strided tiles: y tiles (8 x-adjacent pencils along y of one plane) and z tiles (8 xy-adjacent pencils along z)
-int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap* mz, CUtensorMap* mz2 = nullptr) {
+int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap* mz, CUtensorMap* mz2 = nullptr, CUtensorMap* my2 = nullptr) {
     // the recurrence alternates between three arrays: keep their maps (encoding costs a few microseconds per map)
     for (int i = 0; i < 8; ++i)
         if (c->tmap_base[i] == base && c->tmap_nv[i] == nv) {
             *my = c->tmap_y[i]; *mz = c->tmap_z[i];
             if (mz2) *mz2 = c->tmap_z2[i];
+            if (my2) *my2 = c->tmap_y2[i];
             return 0;
         }
     const int slot = c->tmap_next;
@@ -277,13 +278,17 @@ int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap*
     if (r == CUDA_SUCCESS)
         r = enc(mz, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dz, sz, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    CUtensorMap z2;
+    CUtensorMap z2, y2;
     if (r == CUDA_SUCCESS)
         r = enc(&z2, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dz, sz, box2, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r == CUDA_SUCCESS)
+        r = enc(&y2, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dy, sy, box2, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return set_error(SGW_ECUDA, "cuTensorMapEncodeTiled failed: " + std::to_string((int)r));
-    c->tmap_base[slot] = base; c->tmap_nv[slot] = nv; c->tmap_y[slot] = *my; c->tmap_z[slot] = *mz; c->tmap_z2[slot] = z2;
+    c->tmap_base[slot] = base; c->tmap_nv[slot] = nv; c->tmap_y[slot] = *my; c->tmap_z[slot] = *mz; c->tmap_z2[slot] = z2; c->tmap_y2[slot] = y2;
     if (mz2) *mz2 = z2;
+    if (my2) *my2 = y2;
     return 0;
 }
 
@@ -291,7 +296,12 @@ int acc_maps(sgw_ctx* c, const void* base, int nv, CUtensorMap* my, CUtensorMap*
 int acc_td_step(sgw_ctx* c, int nvec, const LeanOp& op) {
     TdCall call;
     memset(&call, 0, sizeof(call));
-    SGW_TRY(acc_maps(c, op.acc, nvec, &call.map_y, &call.map_z));
+    if (c->nx == 384) {           // two consumer groups: the y and z launches work on tile pairs (maps with 256-byte rows)
+        CUtensorMap y1, z1;
+        SGW_TRY(acc_maps(c, op.acc, nvec, &y1, &z1, &call.map_z, &call.map_y));
+    } else {
+        SGW_TRY(acc_maps(c, op.acc, nvec, &call.map_y, &call.map_z));
+    }
     call.num_sms = c->num_sms;
     call.occ = c->acc_occ;
     call.stream = c->stream;
