@@ -130,7 +130,7 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 //   vector-major: the tiles of a vector are [x tiles | y tiles | z tiles] (kinds present in the launch), vector after vector
 //   plane-major (x and y kinds only): the tiles of a plane are [x tiles | y tiles], plane after plane
 // kind 0 x: rows [j*8, j*8+8) of plane p;  1 y: columns [j*8, ..) of plane p;  2 z: xy points [j*8, ..) of vector v.
-template <int N>
+template <int N, bool PZ = false>
 struct AccIter {
     static constexpr unsigned TPP = N / 8, TPV = (unsigned)N * N / 8;
     unsigned t, q, u, period, step, seg; // u = vector (vector-major) or plane (plane-major), q = offset inside it
@@ -139,7 +139,7 @@ struct AccIter {
     unsigned v, p, j;
     __device__ __forceinline__ void init(const AccArgs& a, unsigned t0, unsigned stride) {
         const unsigned nk = (unsigned)((a.kinds & 1) + ((a.kinds >> 1) & 1) + ((a.kinds >> 2) & 1));
-        seg = a.plane_major ? TPP : (a.pairz ? TPV / 2 : TPV);
+        seg = a.plane_major ? TPP : (PZ ? TPV / 2 : TPV);
         hasx = a.kinds & 1;
         period = nk * seg;
         t = t0; step = stride;
@@ -148,7 +148,7 @@ struct AccIter {
     // x tiles are the first segment of a period when the launch has any
     __device__ __forceinline__ bool is_x() const { return hasx && q < seg; }
     __device__ __forceinline__ void decode(const AccArgs& a) {
-        if (a.pairz) { kind = 2; v = u; j = q; p = 0; return; }   // pair j of vector u: xy points [16 j, 16 j + 16)
+        if (PZ) { kind = 2; v = u; j = q; p = 0; return; }   // pair j of vector u: xy points [16 j, 16 j + 16)
         if (a.plane_major) {
             const unsigned k = q / TPP;
             kind = (a.kinds & 1) ? (int)k : 1;
@@ -279,7 +279,8 @@ __device__ __forceinline__ void acc_tile_compute(const AccArgs& a, cd* tile, cd*
     lean_sync<GW>(bar_id);
 }
 
-template <int N>
+// PZ: the z-only launch in tile pairs, a separate instantiation so that the code of the other launches is untouched by it
+template <int N, bool PZ = false>
 __global__ void __launch_bounds__(AccCfg<N>::T_ACC, 1)
 acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const __grid_constant__ CUtensorMap cur_z,
                const __grid_constant__ CUtensorMap acc_y, const __grid_constant__ CUtensorMap acc_z, int nslots) {
@@ -317,10 +318,10 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
         if (tid == 0) {
             // ---------------- loader: one slot per tile (two for an x tile with a v operand), in tile order
             unsigned seq = 0;
-            AccIter<N> tl;
+            AccIter<N, PZ> tl;
             for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next()) {
                 tl.decode(a);
-                if (C::PAIRZ && a.pairz) {
+                if (PZ) {
                     // a pair fills two adjacent slots (rows of 16 pencils = 256 bytes); only the first slot's barriers are used
                     const unsigned s = seq % S, round = seq / S;
                     if (round > 0) mbar_wait(empty + s, (round - 1) & 1);
@@ -356,11 +357,11 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
         } else if (tid == 32) {
             // ---------------- storer: reduce-add of finished tiles, slots released when the engine has read them
             unsigned seq = 0, pend[2], npend = 0;
-            AccIter<N> tl;
+            AccIter<N, PZ> tl;
             for (tl.init(a, blockIdx.x, gridDim.x); tl.t < a.ntiles; tl.next()) {
                 tl.decode(a);
                 const unsigned s = seq % S, round = seq / S;
-                const bool pair = C::PAIRZ && a.pairz;
+                constexpr bool pair = PZ;
                 seq += (pair || (tl.kind == 0 && !C::LATEW)) ? 2 : 1;
                 if (!mbar_test(done + s, round & 1)) {
                     // about to block: first hand back every slot whose reduce-add has been issued (with few slots the
@@ -411,7 +412,7 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
     if (C::WS_ACC) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;\n");
     const int ct = tid - C::PRODT_ACC, grp = ct / GT, gt = ct % GT;
     unsigned seq = 0, i = 0;
-    AccIter<N> tl;
+    AccIter<N, PZ> tl;
     tl.init(a, blockIdx.x, gridDim.x);
     // one tile: the slot(s) follow from its position seq in the CTA's slot sequence
     auto process = [&](unsigned seq) {
@@ -450,7 +451,7 @@ acc_tma_kernel(const AccArgs a, const __grid_constant__ CUtensorMap cur_y, const
             process(seq);
         }
     } else {
-        if (C::PAIRZ && a.pairz) {
+        if (PZ) {
             // every pair is worked on by both groups: group g takes pencils [8 g, 8 g + 8) of the 16, in place, rows 256 bytes apart
             for (; tl.t < a.ntiles; tl.next(), seq += 2) {
                 const unsigned s = seq % S, round = seq / S;

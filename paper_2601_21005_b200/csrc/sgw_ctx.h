@@ -26,7 +26,7 @@ struct sgw_ctx {
     sgw::acc_launch_fn acc;                  // TMA accumulate kernel (cubic grids) or NULL
     sgw::td_launch_fn tdk;                   // TMA split-operator kernel (cubic grids) or NULL
     int use_acc_td;                          // complex family through it (SGW_ACC_TD; default: from 256 points per axis)
-    int acc_occ[4];
+    int acc_occ[5];                          // kernel attribute set: accumulate, split-operator x / y / z, accumulate in tile pairs
     int acc_pairz;                           // z launch of the accumulate kernel in tile pairs (N = 384; SGW_ACC_PAIRZ=0 disables)
     int use_acc;                             // real family through the TMA accumulate kernel (SGW_ACC; default: where it is built and measured faster)
     double acc_l2_bytes;                     // one-launch terms when cur + acc + v of a vector are at most this (SGW_ACC_L2_MB)

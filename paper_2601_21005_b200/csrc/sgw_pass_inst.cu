@@ -172,16 +172,19 @@ static int launch_acc(const AccCall* c) {
 #if SGW_N >= 32 && SGW_N % 8 == 0
     constexpr int N = SGW_N;
     using Cfg = AccCfg<N>;
-    auto kern = acc_tma_kernel<N>;
+    const bool pz = Cfg::PAIRZ && c->args.pairz;
+    auto kern = pz ? acc_tma_kernel<N, Cfg::PAIRZ> : acc_tma_kernel<N, false>;
+    if (c->args.pairz && !Cfg::PAIRZ) return -(2000);
     const int fixed = Cfg::TABLES + 3 * Cfg::MAXS * 8 + 128;
     int nslots = (227 * 1024 - fixed) / Cfg::TILE;
     if (nslots > Cfg::MAXS) nslots = Cfg::MAXS;
     if (nslots < 4) return 1;
     const size_t smem = (size_t)nslots * Cfg::TILE + fixed;
-    if (!c->occ[0]) {
+    int* attr_set = c->occ + (pz ? 4 : 0);
+    if (!*attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return -(1000 + (int)e);
-        c->occ[0] = 1;
+        *attr_set = 1;
     }
     long long grid = c->num_sms;
     if (grid > (long long)c->args.ntiles) grid = c->args.ntiles;
