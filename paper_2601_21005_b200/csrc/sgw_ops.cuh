@@ -83,12 +83,14 @@ struct OpToReal : OpStore {
 struct OpPhaseMerge : OpStore {
     __device__ __forceinline__ void epi(cd r, long long off, long long) const {
         const double v = (p.vloc ? p.vloc[off] : 0.0) + r.x;
+        // sincospi: no large-argument reduction path; the 1/pi factor costs half an ulp of the angle (~1e-16 absolute here)
+        const double hp = p.half_dt * 0.318309886183790671537767526745028724;
         double s, c;
-        sincos((p.first ? v : v + p.vprev[off]) * p.half_dt, &s, &c);
+        sincospi((p.first ? v : v + p.vprev[off]) * hp, &s, &c);
         p.table[off] = make_double2(c, -s);
         p.vprev[off] = v;
         if (p.last) {
-            sincos(v * p.half_dt, &s, &c);
+            sincospi(v * hp, &s, &c);
             p.last[off] = make_double2(c, -s);
         }
         if (p.rho_reset) p.rho_reset[off] = 0.0;
