@@ -478,15 +478,17 @@ def test_tma_split_operator_kernel(api, torch_cuda, oracle, monkeypatch, n, nvec
     ctx.close()
 
 
-def test_tma_kernels_at_256_agree_with_the_register_operand_passes(api, torch_cuda, monkeypatch):
-    """256 points per axis is where the TMA kernels run in their warp-specialised layout (setmaxnreg: 16 warps, consumer
-    warpgroups at 152 registers; three consumer groups) and the split-operator kernel is the default; the oracle reaches
-    that size only on the golden samples (tests/test_gpu_golden.py: 2 vectors).  Here 5 vectors -- not a multiple of the
-    3 groups nor of the 4 vectors a KB block takes -- with KB spheres, 3 TD-Hartree steps (density summed per block in
-    the z launch, sphere-point correction) and 3 filter applications are compared with the register-operand passes
-    (SGW_ACC=0 / SGW_ACC_TD=0), which the oracle pins on the small grids and on every golden config."""
+@pytest.mark.parametrize("n", [256, 384])
+def test_tma_kernels_at_256_and_384_agree_with_the_register_operand_passes(api, torch_cuda, monkeypatch, n):
+    """256 and 384 points per axis are where the TMA kernels run in their warp-specialised layout (setmaxnreg: 16 warps,
+    consumer warpgroups at 152 registers; three / two consumer groups), where the split-operator kernel is the default
+    and, at 384, where the strided launches move tile pairs; the oracle reaches these sizes only on the golden samples
+    (tests/test_gpu_golden.py: 2 vectors / 1 vector in the TD part).  Here 5 vectors -- not a multiple of the groups nor
+    of the 4 vectors a KB block takes -- with KB spheres, 3 TD-Hartree steps (density summed per block in the z launch,
+    sphere-point correction) and 3 filter applications are compared with the register-operand passes (SGW_ACC=0 /
+    SGW_ACC_TD=0), which the oracle pins on the small grids and on every golden config."""
     torch = torch_cuda
-    n, nvec = 256, 5
+    nvec = 5
     g = W.Grid(n, n, n, 0.5, 0.5, 0.5)
     rng = np.random.default_rng(77)
     centers = rng.uniform(0.2, 0.8, size=(6, 3)) * np.array(g.box)
