@@ -31,7 +31,8 @@
  *                            round trip in shared memory, bulk reduce-add; cubic grids with N a multiple of 8): default
  *                            on for N >= 64, else the register-operand passes below
  *      SGW_ACC_TD=0|1        split-operator steps through the TMA kernel of the same design (one launch per axis, bulk
- *                            stores; cubic grids): default on from N = 256, else the plane / axis passes below
+ *                            stores; a CTA owns blocks of 8 pencils with all their vectors; at N = 384 the y and z launches
+ *                            move tile pairs; cubic grids): default on from N = 256, else the plane / axis passes below
  *      SGW_ACC_L2_MB=m       accumulate kernel: one launch per term while cur + acc + v of a vector are at most m MB
  *                            (default 104: up to 128^3; the L2 holds 126 MB), else planes (x, y tiles) then z columns in two launches
  *      SGW_ACC_PAIRZ=0|1     accumulate kernel at N = 384: z tiles in pairs (16 pencils, 256-byte rows, one tensor operation per
